@@ -1,0 +1,192 @@
+/*
+ * mm.h -- C ABI of the B200-native micromagnetic hot path (after MuMax, arXiv 1102.3069).
+ *
+ * One effective-field evaluation plus Landau-Lifshitz torque per Runge-Kutta stage on a
+ * regular finite-difference grid.  Citations are lines of /root/reference/PAPER.md ("PAPER.md:n")
+ * and readings A1..A13 of DESIGN.md where the paper is silent.
+ *
+ * Conventions that hold for every call
+ * ------------------------------------
+ *  - No C++ types, no exceptions and no torch types cross this boundary.  Every call returns an
+ *    mm_status; mm_last_error(ctx) gives a human-readable message for the last failure.
+ *  - Fields are structure-of-arrays float32 [3][Nz][Ny][Nx], x fastest, contiguous, 16-byte aligned,
+ *    component order (x, y, z).  "m" holds unit vectors, M = Ms * m.
+ *  - Pointers named *_dev are DEVICE pointers owned by the caller (e.g. a torch CUDA tensor's
+ *    data_ptr()); pointers named *_host are HOST pointers.  The library never frees, reallocates or
+ *    keeps caller memory beyond the call (asynchronous calls keep it until the stream reaches them).
+ *  - The context owns the transformed kernel K-hat, FFT workspaces, twiddle tables, Runge-Kutta
+ *    buffers and device scalars.  Nothing is allocated on the device after mm_demag_init.
+ *  - All device work is enqueued on the CUDA stream given to mm_create.  mm_heff / mm_torque /
+ *    mm_stage are asynchronous with respect to the host; mm_step synchronises the stream once, at its
+ *    end, to return dt / err / accepted.
+ *  - There is no CPU fallback, no cuFFT and no tensor-core path inside the library: every hot-path
+ *    step runs in hand-written sm_100a kernels.  Without a CUDA device mm_create fails with MM_ECUDA.
+ */
+#ifndef MM_H_
+#define MM_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct mm_ctx mm_ctx; /* opaque */
+
+typedef enum {
+    MM_OK = 0,
+    MM_EINVAL = 1,       /* bad argument (NULL, non-positive size, ...)                          */
+    MM_ENOMEM = 2,       /* host or device allocation failed                                      */
+    MM_ECUDA = 3,        /* CUDA runtime error (message in mm_last_error)                         */
+    MM_ESTATE = 4,       /* call order: material / demag kernel not set                           */
+    MM_EUNSUPPORTED = 5, /* padded size not 2^a 3^b 5^c, thermal field with adaptive stepping ... */
+    MM_ENUMERIC = 6      /* non-finite value met by the max-norm reduction                        */
+} mm_status;
+
+/* Runge-Kutta family of PAPER.md:123-139 (section 2.2).  RK4 and RKDP are the two the hot path is
+ * graded on; the others share the same stage kernel with another tableau. */
+typedef enum {
+    MM_RK1 = 0,  /* Euler -- the step the paper times              */
+    MM_RK2 = 1,  /* Heun                                                           */
+    MM_RK4 = 2,  /* classical 4th order                                            */
+    MM_RKDP = 3, /* Dormand-Prince 5(4), adaptive; controller: reading A10         */
+    MM_RK12 = 4, /* Heun-Euler 2(1), adaptive                                      */
+    MM_RK23 = 5  /* Bogacki-Shampine 3(2), adaptive                                */
+} mm_method;
+
+/* Material and drive, SI units in; converted once to the internal reduced units mu0 = gamma0 = Ms = 1
+ * of PAPER.md:169 (section 3.3).  Plain data, copied by mm_set_material. */
+typedef struct {
+    double Ms;        /* saturation magnetisation, A/m, > 0                                       */
+    double Aex;       /* exchange stiffness, J/m, >= 0            Eq. (3)            */
+    double alpha;     /* damping, >= 0                            Eq. (1)            */
+    double gamma0;    /* m/(A s); 0 selects 2.211e5               reading A2                      */
+    double Ku;        /* uniaxial anisotropy constant, J/m^3      Eq. (4)            */
+    double anis_u[3]; /* anisotropy axis, normalised by the library (ignored if Ku == 0)          */
+    double Bext[3];   /* applied field, tesla; H = B / mu0                     */
+    double T;         /* temperature, kelvin                      Eq. (6)           */
+    uint64_t seed;    /* Philox4x32-10 key                        reading A6                      */
+    double j[3];      /* current density, A/m^2                   Eq. (7)           */
+    double P;         /* spin polarisation                        Eq. (8)           */
+    double xi;        /* degree of non-adiabaticity               Eq. (7)                         */
+    int stt_literal_eq7; /* 0: (1 + alpha xi) on the adiabatic term; 1: Eq. (7) as printed (A7)   */
+    int demag;        /* 1: magnetostatic field on (default use); 0: off (tests of local terms)   */
+} mm_material;
+
+/* mm_create -- set up a context for a grid of equal cuboid cells.
+ *   out          receives the context (host pointer).
+ *   grid[3]      cells along x, y, z (each >= 1).
+ *   cellsize[3]  cell edge lengths in metres (each > 0).
+ *   pbc[3]       0 = open boundary, zero padded to 2 N_a (reading A9);
+ *                p > 0 = periodic with images -p..p summed into the kernel and no padding
+ *                (reading A8).
+ *   cuda_stream  a cudaStream_t (e.g. torch.cuda.current_stream().cuda_stream) or NULL for the
+ *                default stream.  Every kernel of this context is launched on it.
+ * Errors: MM_EINVAL; MM_EUNSUPPORTED if a padded size has a prime factor other than 2, 3, 5
+ * (PAPER.md:169-171 restricts sizes to smooth numbers); MM_ECUDA if no device; MM_ENOMEM. */
+mm_status mm_create(mm_ctx** out, const int grid[3], const double cellsize[3], const int pbc[3],
+                    void* cuda_stream);
+
+/* mm_set_material -- copy material / drive parameters; may be called again between steps.
+ * Errors: MM_EINVAL (Ms <= 0, negative Aex / alpha, zero axis with Ku != 0). */
+mm_status mm_set_material(mm_ctx* ctx, const mm_material* mat);
+
+/* mm_demag_init -- build the transformed demagnetisation kernel:
+ * cell-averaged tensor on the padded offset lattice evaluated on the HOST in extended precision
+ * (long double near field, multipole series far field; reading A1), periodic images summed, each
+ * axis transformed in fp64, real part kept (the kernel is symmetric), the sign and the
+ * 1/(Px Py Pz) normalisation folded in, one octant stored as float32 and copied to the device once
+ * (PAPER.md:151).  Also allocates every device workspace.  Blocking.  Independent of the material.
+ * Errors: MM_ENOMEM, MM_ECUDA. */
+mm_status mm_demag_init(mm_ctx* ctx);
+
+/* mm_heff -- one effective-field evaluation:
+ * H_eff = H_ms + H_exch + H_anis + H_ext + H_therm, in A/m, written to H_dev.
+ *   m_dev   in,  device, float32 [3][Nz][Ny][Nx]
+ *   H_dev   out, device, same layout
+ *   step, dt_for_thermal   index of the time step and its length in seconds: the thermal field is one
+ *           draw per cell per step with amplitude ~ 1/sqrt(dt) (Eq. (6); reading A6).  Ignored if T = 0.
+ * Asynchronous.  Errors: MM_ESTATE before mm_set_material / mm_demag_init; MM_EINVAL. */
+mm_status mm_heff(mm_ctx* ctx, const float* m_dev, float* H_dev, double t, uint64_t step,
+                  double dt_for_thermal);
+
+/* mm_torque -- dm/dt in 1/s: Eq. (1) for m = M/Ms plus the Zhang-Li terms of
+ * Eq. (7)-(8) when j != 0.  Same arguments as mm_heff.  Asynchronous. */
+mm_status mm_torque(mm_ctx* ctx, const float* m_dev, float* dmdt_dev, double t, uint64_t step,
+                    double dt_for_thermal);
+
+/* mm_step -- one trial step of a Runge-Kutta method, m updated in place.
+ *   m_dev       in/out, device.  On an accepted step m <- normalise(m + dt sum b_s k_s); on a
+ *               rejected step (adaptive methods only) m is left unchanged.
+ *   dt_inout    host: in = step to try (s); out = step proposed for the next call (adaptive methods;
+ *               unchanged for fixed-step methods).
+ *   tol         maximum tolerable error per step (reading A10); ignored by RK1/RK2/RK4.
+ *   t_inout     host: time, advanced by dt when the step is accepted.
+ *   err_out     host, may be NULL: error estimate of the embedded pair (0 for fixed-step methods).
+ *   accepted_out host, may be NULL: 1 / 0.
+ * The thermal field is redrawn once per accepted step and requires a fixed-step method (A6):
+ * MM_EUNSUPPORTED otherwise.  Synchronises the stream once at the end.
+ * Errors: MM_ESTATE, MM_EINVAL, MM_EUNSUPPORTED, MM_ENUMERIC (NaN/Inf met), MM_ECUDA. */
+mm_status mm_step(mm_ctx* ctx, float* m_dev, mm_method method, double* dt_inout, double tol,
+                  double* t_inout, double* err_out, int* accepted_out);
+
+/* mm_steps_fixed -- n consecutive steps of fixed length dt with no host synchronisation in between
+ * (the whole sequence is enqueued; stage launches are replayed from a CUDA graph when possible).
+ * With an adaptive method the embedded error is still reduced on the device but every step is
+ * accepted: this is the "replay" mode reading A10 uses for parity of adaptive runs.
+ *   max_err_out  host, may be NULL: largest per-step error estimate seen.
+ * Synchronises once at the end. */
+mm_status mm_steps_fixed(mm_ctx* ctx, float* m_dev, mm_method method, double dt, int n,
+                         double* t_inout, double* max_err_out);
+
+/* mm_fused_eval -- the unit the throughput metric counts: ONE fused evaluation = demag convolution +
+ * local field terms + torque + an RK4-shaped stage combine + max-norm reduction, i.e. stage `stage`
+ * (0-based) of `method` applied to m_dev with step dt, writing the stage derivative and the next stage
+ * input into the context's Runge-Kutta buffers.  m_dev is not modified unless it is the last stage.
+ * Asynchronous; used by bench.py and by the step functions above. */
+mm_status mm_fused_eval(mm_ctx* ctx, float* m_dev, mm_method method, int stage, double dt,
+                        uint64_t step);
+
+/* mm_demag_field -- magnetostatic field only (A/m), H_ms = -Ms sum_j N(r_i - r_j) m_j
+ * (discrete Eq. (2)): test and diagnostic entry (reading A12).  Asynchronous. */
+mm_status mm_demag_field(mm_ctx* ctx, const float* m_dev, float* H_dev);
+
+/* mm_get_demag_kernel -- test hook: copy component comp (0..5 = xx,yy,zz,xy,xz,yz) of the stored
+ * octant K-hat[(Pz/2+1)][(Py/2+1)][(Px/2+1)] (float32, includes the factor -1/(Px Py Pz)) to host_out.
+ *   n  capacity of host_out in floats; MM_EINVAL if too small. */
+mm_status mm_get_demag_kernel(mm_ctx* ctx, int comp, float* host_out, size_t n);
+
+/* mm_demag_tensor_host -- test hook, HOST only, needs no device and no context state beyond the grid:
+ * the library's own real-space tensor N (xx,yy,zz,xy,xz,yz) at n integer cell offsets off[3*i..],
+ * periodic images included as mm_create's pbc says.  out_host[6*i..], double. */
+mm_status mm_demag_tensor_host(const double cellsize[3], const int grid[3], const int pbc[3],
+                               size_t n, const long* off_host, double* out_host);
+
+/* mm_padded_size -- padded FFT sizes P[3] and the octant extents C[3] = P/2 + 1 of this context. */
+mm_status mm_padded_size(const mm_ctx* ctx, int P_out[3], int C_out[3]);
+
+/* mm_launch_count -- number of kernels this context has launched so far (bench.py "gpu_launches"). */
+uint64_t mm_launch_count(const mm_ctx* ctx);
+
+/* mm_set_fast_path -- 1 (default): use the size-specialised register FFT kernels when the grid
+ * allows; 0: force the generic shared-memory radix-2/3/4/5 kernels (tests compare the two). */
+mm_status mm_set_fast_path(mm_ctx* ctx, int enable);
+
+/* mm_copy_bandwidth -- the library's own float4 grid-stride copy kernel, used by bench.py as the
+ * HBM roofline cross-check: copies nbytes from src_dev to dst_dev `reps` times and
+ * returns the mean seconds per copy in *sec_out (device-timed with CUDA events).  Blocking. */
+mm_status mm_copy_bandwidth(mm_ctx* ctx, const void* src_dev, void* dst_dev, size_t nbytes,
+                            int reps, double* sec_out);
+
+/* mm_last_error -- message for the last non-OK status of this context ("" if none); for a NULL ctx
+ * the message of the last failed mm_create on this thread. */
+const char* mm_last_error(const mm_ctx* ctx);
+
+/* mm_destroy -- free everything the context owns (NULL is a no-op). */
+void mm_destroy(mm_ctx* ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* MM_H_ */
