@@ -148,6 +148,11 @@ mm_status mm_steps_fixed(mm_ctx* ctx, float* m_dev, mm_method method, double dt,
 mm_status mm_fused_eval(mm_ctx* ctx, float* m_dev, mm_method method, int stage, double dt,
                         uint64_t step);
 
+/* mm_reset_stepper -- set the index of the next time step (it selects the thermal draw, reading A6;
+ * mm_step / mm_steps_fixed advance it by one per accepted step) and forget the saved first stage of
+ * the FSAL methods.  Call it after writing into m_dev from outside between two steps. */
+mm_status mm_reset_stepper(mm_ctx* ctx, uint64_t step_index);
+
 /* mm_demag_field -- magnetostatic field only (A/m), H_ms = -Ms sum_j N(r_i - r_j) m_j
  * (discrete Eq. (2)): test and diagnostic entry (reading A12).  Asynchronous. */
 mm_status mm_demag_field(mm_ctx* ctx, const float* m_dev, float* H_dev);
@@ -162,6 +167,11 @@ mm_status mm_get_demag_kernel(mm_ctx* ctx, int comp, float* host_out, size_t n);
  * periodic images included as mm_create's pbc says.  out_host[6*i..], double. */
 mm_status mm_demag_tensor_host(const double cellsize[3], const int grid[3], const int pbc[3],
                                size_t n, const long* off_host, double* out_host);
+
+/* mm_demag_khat_host -- test hook, HOST only, needs no device: the transformed kernel exactly as
+ * mm_demag_init would upload it, out_host[6][Cz][Cy][Cx] float32 (n = capacity in floats). */
+mm_status mm_demag_khat_host(const double cellsize[3], const int grid[3], const int pbc[3],
+                             float* out_host, size_t n);
 
 /* mm_padded_size -- padded FFT sizes P[3] and the octant extents C[3] = P/2 + 1 of this context. */
 mm_status mm_padded_size(const mm_ctx* ctx, int P_out[3], int C_out[3]);

@@ -1,0 +1,198 @@
+// epilogue.cuh -- per-cell tail of one evaluation (steps a6-a10 of DESIGN.md): exchange stencil,
+// anisotropy, Zeeman and thermal fields, Landau-Lifshitz torque with the Zhang-Li terms, the
+// Runge-Kutta stage combine and the max-norm reduction.  Called by the inverse x pass with the
+// magnetostatic field of the cell still in registers.
+//
+// Product code; shares nothing with oracle/.
+#pragma once
+#include "mm_common.cuh"
+
+namespace mm {
+
+// ---- Philox4x32-10 (reading A6: key = seed, counter = (cell lo, cell hi, step lo, step hi)) ----
+__device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3,
+                                              uint32_t k0, uint32_t k1, uint32_t out[4])
+{
+#pragma unroll
+    for (int r = 0; r < 10; ++r) {
+        const uint32_t h0 = __umulhi(0xD2511F53u, c0), l0 = 0xD2511F53u * c0;
+        const uint32_t h1 = __umulhi(0xCD9E8D57u, c2), l1 = 0xCD9E8D57u * c2;
+        c0 = h1 ^ c1 ^ k0;
+        c1 = l1;
+        c2 = h0 ^ c3 ^ k1;
+        c3 = l0;
+        k0 += 0x9E3779B9u;
+        k1 += 0xBB67AE85u;
+    }
+    out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+
+// -2 ln u for u = (x+1) 2^-32 without losing the resolution of u near 1 (reading A6)
+__device__ __forceinline__ float neg2ln_u(uint32_t x)
+{
+    if (x >= 0x80000000u) {
+        const float d = (float)(0xFFFFFFFFu - x) * 2.3283064365386963e-10f;   // 1 - u, exact scaling
+        return -2.0f * log1pf(-d);
+    }
+    const float u = ((float)x + 1.0f) * 2.3283064365386963e-10f;
+    return -2.0f * logf(u);
+}
+
+// three N(0,1) numbers of cell `cell` at step (step0, step1): Box-Muller on the four Philox words
+__device__ __forceinline__ void thermal_eta(const EpiParams& p, uint64_t cell, float eta[3])
+{
+    uint32_t w[4];
+    philox4x32_10((uint32_t)cell, (uint32_t)(cell >> 32), p.step0, p.step1, p.key0, p.key1, w);
+    const float r1 = sqrtf(neg2ln_u(w[0]));
+    const float r2 = sqrtf(neg2ln_u(w[2]));
+    float s1, c1, s2, c2;
+    // angle = 2 pi w 2^-32 = pi * (w 2^-31); w -> float keeps 24 bits (error <= 2 pi 2^-25 rad)
+    sincospif((float)w[1] * 4.656612873077393e-10f, &s1, &c1);
+    sincospif((float)w[3] * 4.656612873077393e-10f, &s2, &c2);
+    eta[0] = r1 * c1;
+    eta[1] = r1 * s1;
+    eta[2] = r2 * c2;
+}
+
+__device__ __forceinline__ void cross3(const float a[3], const float b[3], float c[3])
+{
+    c[0] = a[1] * b[2] - a[2] * b[1];
+    c[1] = a[2] * b[0] - a[0] * b[2];
+    c[2] = a[0] * b[1] - a[1] * b[0];
+}
+
+// One cell.  hms = magnetostatic field in units of Ms.  Returns the value to be max-reduced
+// (error norm or |dm/dtau|), 0 when no reduction is asked for.
+__device__ __forceinline__ float epilogue_cell(const Geom& g, const EpiParams& p, int x, int y, int z,
+                                               float hx, float hy, float hz)
+{
+    const size_t plane = (size_t)g.Ny * g.Nx;
+    const size_t n = plane * g.Nz;
+    const size_t idx = (size_t)z * plane + (size_t)y * g.Nx + x;
+    const float* __restrict__ mi = p.m_in;
+    float m[3] = { mi[idx], mi[idx + n], mi[idx + 2 * n] };
+    float h[3] = { hx, hy, hz };
+    if (p.mode == EPI_HMS) {
+        p.out[idx] = p.out_scale * h[0];
+        p.out[idx + n] = p.out_scale * h[1];
+        p.out[idx + 2 * n] = p.out_scale * h[2];
+        return 0.f;
+    }
+    // ---- neighbours: exchange (Eq. (3), reading A3) and (j.grad) m (Eq. (7), reading A7) ----
+    float D[3] = { 0.f, 0.f, 0.f };
+    {
+        const int pos[3] = { x, y, z };
+        const int ext[3] = { g.Nx, g.Ny, g.Nz };
+        const int per[3] = { g.perx, g.pery, g.perz };
+        const size_t str[3] = { (size_t)1, (size_t)g.Nx, plane };
+#pragma unroll
+        for (int a = 0; a < 3; ++a) {
+            if (ext[a] == 1) continue;
+            const bool need_ex = p.wex[a] != 0.f;
+            const bool need_j = p.stt && p.cj[a] != 0.f;
+            if (!need_ex && !need_j) continue;
+            // index of the +/- neighbours; a missing neighbour is replaced by the cell itself
+            size_t ip = idx, im = idx;
+            if (pos[a] + 1 < ext[a]) ip = idx + str[a];
+            else if (per[a]) ip = idx - (size_t)(ext[a] - 1) * str[a];
+            if (pos[a] > 0) im = idx - str[a];
+            else if (per[a]) im = idx + (size_t)(ext[a] - 1) * str[a];
+#pragma unroll
+            for (int c = 0; c < 3; ++c) {
+                const float mp = mi[ip + c * n], mm_ = mi[im + c * n];
+                h[c] += p.wex[a] * ((mp - m[c]) + (mm_ - m[c]));
+                D[c] += p.cj[a] * (mp - mm_);
+            }
+        }
+    }
+    // ---- anisotropy (Eq. (4), reading A5), Zeeman ----
+    {
+        const float mu = m[0] * p.u[0] + m[1] * p.u[1] + m[2] * p.u[2];
+        const float s = p.kan * mu;
+#pragma unroll
+        for (int c = 0; c < 3; ++c) h[c] += s * p.u[c] + p.hext[c];
+    }
+    // ---- thermal field (Eq. (6), reading A6) ----
+    if (p.thermal) {
+        float eta[3];
+        thermal_eta(p, (uint64_t)idx, eta);
+#pragma unroll
+        for (int c = 0; c < 3; ++c) h[c] += p.sig_th * eta[c];
+    }
+    if (p.mode == EPI_HEFF) {
+#pragma unroll
+        for (int c = 0; c < 3; ++c) p.out[idx + c * n] = p.out_scale * h[c];
+        return 0.f;
+    }
+    // ---- torque, Eq. (1): dm/dtau = -1/(1+alpha^2) [ m x h + alpha m x (m x h) ] ----
+    float mxh[3], mxmxh[3], k[3];
+    cross3(m, h, mxh);
+    cross3(m, mxh, mxmxh);
+#pragma unroll
+    for (int c = 0; c < 3; ++c) k[c] = -p.inv1pa2 * (mxh[c] + p.alpha * mxmxh[c]);
+    if (p.stt) {   // Eq. (7): - c_ad m x (m x D) - c_nad m x D
+        float mxD[3], mxmxD[3];
+        cross3(m, D, mxD);
+        cross3(m, mxD, mxmxD);
+#pragma unroll
+        for (int c = 0; c < 3; ++c) k[c] -= p.c_ad * mxmxD[c] + p.c_nad * mxD[c];
+    }
+    if (p.mode == EPI_TORQUE) {
+#pragma unroll
+        for (int c = 0; c < 3; ++c) p.out[idx + c * n] = p.out_scale * k[c];
+        return 0.f;
+    }
+    // ---- Runge-Kutta stage combine ----
+    if (p.k_out) {
+#pragma unroll
+        for (int c = 0; c < 3; ++c) p.k_out[idx + c * n] = k[c];
+    }
+    if (p.m_out) {
+        float acc[3] = { p.a_self * k[0], p.a_self * k[1], p.a_self * k[2] };
+        for (int j = 0; j < p.na; ++j) {
+            const float* __restrict__ kj = p.ka[j];
+#pragma unroll
+            for (int c = 0; c < 3; ++c) acc[c] += p.a[j] * kj[idx + c * n];
+        }
+        const float* __restrict__ mn = p.m_n;
+        float r[3] = { mn[idx] + acc[0], mn[idx + n] + acc[1], mn[idx + 2 * n] + acc[2] };
+        if (p.normalise) {
+            const float s = rsqrtf(r[0] * r[0] + r[1] * r[1] + r[2] * r[2]);
+            r[0] *= s; r[1] *= s; r[2] *= s;
+        }
+#pragma unroll
+        for (int c = 0; c < 3; ++c) p.m_out[idx + c * n] = r[c];
+    }
+    float red = 0.f;
+    if (p.do_err) {
+        float e[3] = { p.e_self * k[0], p.e_self * k[1], p.e_self * k[2] };
+        for (int j = 0; j < p.ne; ++j) {
+            const float* __restrict__ kj = p.ke[j];
+#pragma unroll
+            for (int c = 0; c < 3; ++c) e[c] += p.e[j] * kj[idx + c * n];
+        }
+        red = sqrtf(e[0] * e[0] + e[1] * e[1] + e[2] * e[2]);
+    }
+    return red;
+}
+
+// Block-wide max of non-negative floats (NaN wins), one atomicMax per block (step a10).
+// Order-independent, hence bit-reproducible.
+__device__ __forceinline__ void block_max_atomic(unsigned int b, unsigned int* target)
+{
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) b = max(b, __shfl_xor_sync(0xffffffffu, b, o));
+    __shared__ unsigned int wmax[32];
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    if (lane == 0) wmax[w] = b;
+    __syncthreads();
+    if (w == 0) {
+        const int nw = (blockDim.x + 31) >> 5;
+        b = lane < nw ? wmax[lane] : 0u;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) b = max(b, __shfl_xor_sync(0xffffffffu, b, o));
+        if (lane == 0 && b != 0u) atomicMax(target, b);
+    }
+}
+
+}  // namespace mm

@@ -1,0 +1,761 @@
+// mm_api.cu -- the C ABI of include/mm.h: context, plans, launches.
+//
+// Product code; shares nothing with oracle/.  No CPU fallback: without a CUDA device mm_create fails.
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "../../include/mm.h"
+#include "demag_host.h"
+#include "mm_common.cuh"
+#include "epilogue.cuh"
+#include "fft_generic.cuh"
+#include "fft_fast.cuh"
+
+using namespace mm;
+
+namespace {
+
+const double MU0 = 4e-7 * M_PI;
+const double KB = 1.380649e-23;
+const double MUB = 9.2740100783e-24;
+const double QE = 1.602176634e-19;
+const double GAMMA0_DEFAULT = 2.211e5;
+
+thread_local std::string g_create_error;
+
+// ---- Runge-Kutta tableaux ----
+struct Tableau {
+    int S;
+    double A[7][7];
+    double b[7];
+    double bs[7];
+    bool embedded;
+    bool fsal;      // last row of A equals b: the last stage is f(new state) and is reused
+};
+
+Tableau make_tableau(mm_method m)
+{
+    Tableau t;
+    std::memset(&t, 0, sizeof(t));
+    switch (m) {
+    case MM_RK1:
+        t.S = 1; t.b[0] = 1.0;
+        break;
+    case MM_RK2:    // Heun
+        t.S = 2; t.A[1][0] = 1.0; t.b[0] = 0.5; t.b[1] = 0.5;
+        break;
+    case MM_RK12:   // Heun-Euler 2(1)
+        t.S = 2; t.A[1][0] = 1.0; t.b[0] = 0.5; t.b[1] = 0.5; t.bs[0] = 1.0; t.embedded = true;
+        break;
+    case MM_RK4:
+        t.S = 4; t.A[1][0] = 0.5; t.A[2][1] = 0.5; t.A[3][2] = 1.0;
+        t.b[0] = 1.0 / 6; t.b[1] = 1.0 / 3; t.b[2] = 1.0 / 3; t.b[3] = 1.0 / 6;
+        break;
+    case MM_RK23:   // Bogacki-Shampine 3(2)
+        t.S = 4; t.A[1][0] = 0.5; t.A[2][1] = 0.75;
+        t.A[3][0] = 2.0 / 9; t.A[3][1] = 1.0 / 3; t.A[3][2] = 4.0 / 9;
+        t.b[0] = 2.0 / 9; t.b[1] = 1.0 / 3; t.b[2] = 4.0 / 9; t.b[3] = 0.0;
+        t.bs[0] = 7.0 / 24; t.bs[1] = 0.25; t.bs[2] = 1.0 / 3; t.bs[3] = 0.125;
+        t.embedded = true; t.fsal = true;
+        break;
+    case MM_RKDP: {  // Dormand-Prince 5(4)
+        t.S = 7;
+        const double A[7][7] = {
+            { 0 },
+            { 1.0 / 5 },
+            { 3.0 / 40, 9.0 / 40 },
+            { 44.0 / 45, -56.0 / 15, 32.0 / 9 },
+            { 19372.0 / 6561, -25360.0 / 2187, 64448.0 / 6561, -212.0 / 729 },
+            { 9017.0 / 3168, -355.0 / 33, 46732.0 / 5247, 49.0 / 176, -5103.0 / 18656 },
+            { 35.0 / 384, 0, 500.0 / 1113, 125.0 / 192, -2187.0 / 6784, 11.0 / 84 } };
+        std::memcpy(t.A, A, sizeof(A));
+        const double b[7] = { 35.0 / 384, 0, 500.0 / 1113, 125.0 / 192, -2187.0 / 6784, 11.0 / 84, 0 };
+        const double bs[7] = { 5179.0 / 57600, 0, 7571.0 / 16695, 393.0 / 640, -92097.0 / 339200,
+                               187.0 / 2100, 1.0 / 40 };
+        std::memcpy(t.b, b, sizeof(b));
+        std::memcpy(t.bs, bs, sizeof(bs));
+        t.embedded = true; t.fsal = true;
+        break;
+    }
+    default:
+        t.S = 0;
+    }
+    return t;
+}
+
+bool smooth235(int n)
+{
+    for (int p : { 2, 3, 5 })
+        while (n % p == 0) n /= p;
+    return n == 1;
+}
+
+}  // namespace
+
+struct mm_ctx {
+    Geom g;
+    double cell[3];
+    int pbc[3];
+    cudaStream_t stream;
+    bool has_mat, has_demag;
+    mm_material mat;
+    std::string err;
+    uint64_t launches;
+    int fast;
+    // device
+    float* khat;
+    float2 *specA, *specB;
+    float2* tw[3];
+    FftPlan plan[3];
+    float* kb[7];
+    float* ms[2];
+    float* mtmp;
+    unsigned int* maxbits;
+    // stepper state
+    uint64_t step_index;
+    bool k0_valid;
+    int k0_method;
+    FastPlan fp;
+};
+
+namespace {
+
+mm_status fail(mm_ctx* c, mm_status s, const std::string& msg)
+{
+    if (c) c->err = msg;
+    else g_create_error = msg;
+    return s;
+}
+
+#define CUDA_TRY(c, call)                                                                         \
+    do {                                                                                          \
+        cudaError_t e_ = (call);                                                                  \
+        if (e_ != cudaSuccess)                                                                    \
+            return fail((c), e_ == cudaErrorMemoryAllocation ? MM_ENOMEM : MM_ECUDA,             \
+                        std::string(#call) + ": " + cudaGetErrorString(e_));                      \
+    } while (0)
+
+size_t ncell(const Geom& g) { return (size_t)g.Nx * g.Ny * g.Nz; }
+
+void make_plan(FftPlan& pl, int L)
+{
+    pl.L = L;
+    pl.nrad = 0;
+    int m = L;
+    while (m % 4 == 0) { pl.rad[pl.nrad++] = 4; m /= 4; }
+    while (m % 2 == 0) { pl.rad[pl.nrad++] = 2; m /= 2; }
+    while (m % 3 == 0) { pl.rad[pl.nrad++] = 3; m /= 3; }
+    while (m % 5 == 0) { pl.rad[pl.nrad++] = 5; m /= 5; }
+}
+
+// largest column count from {16, 8, 4, 2, 1} (times `mult`, plus one pad column) whose tile fits
+int pick_tx(int L, int nbuf, int mult, size_t* bytes)
+{
+    const size_t soft = 110 * 1024, hard = 220 * 1024;
+    for (size_t lim : { soft, hard })
+        for (int tx : { 16, 8, 4, 2, 1 }) {
+            const size_t b = (size_t)nbuf * L * (mult * tx + 1) * sizeof(float2);
+            if (b <= lim) { *bytes = b; return tx; }
+        }
+    *bytes = 0;
+    return 0;
+}
+
+// fill the material-dependent part of the epilogue parameters
+void fill_material(const mm_ctx* c, EpiParams& p, uint64_t step, double dt_thermal)
+{
+    const mm_material& M = c->mat;
+    const Geom& g = c->g;
+    const double Ms = M.Ms;
+    const double g0 = M.gamma0 > 0 ? M.gamma0 : GAMMA0_DEFAULT;
+    const int ext[3] = { g.Nx, g.Ny, g.Nz };
+    p.demag = M.demag ? 1 : 0;
+    for (int a = 0; a < 3; ++a)
+        p.wex[a] = ext[a] > 1 ? (float)(2.0 * M.Aex / (MU0 * Ms * Ms * c->cell[a] * c->cell[a])) : 0.f;
+    double u[3] = { M.anis_u[0], M.anis_u[1], M.anis_u[2] };
+    const double un = std::sqrt(u[0] * u[0] + u[1] * u[1] + u[2] * u[2]);
+    p.kan = (M.Ku != 0.0 && un > 0) ? (float)(2.0 * M.Ku / (MU0 * Ms * Ms)) : 0.f;
+    for (int a = 0; a < 3; ++a) {
+        p.u[a] = un > 0 ? (float)(u[a] / un) : 0.f;
+        p.hext[a] = (float)(M.Bext[a] / (MU0 * Ms));
+    }
+    p.thermal = (M.T > 0.0 && dt_thermal > 0.0) ? 1 : 0;
+    p.sig_th = 0.f;
+    if (p.thermal) {
+        const double V = c->cell[0] * c->cell[1] * c->cell[2];
+        p.sig_th = (float)(std::sqrt(2.0 * M.alpha * KB * M.T / (g0 * MU0 * Ms * V * dt_thermal)) / Ms);
+    }
+    p.key0 = (uint32_t)(M.seed & 0xffffffffu);
+    p.key1 = (uint32_t)(M.seed >> 32);
+    p.step0 = (uint32_t)(step & 0xffffffffu);
+    p.step1 = (uint32_t)(step >> 32);
+    p.alpha = (float)M.alpha;
+    p.inv1pa2 = (float)(1.0 / (1.0 + M.alpha * M.alpha));
+    p.stt = (M.j[0] != 0.0 || M.j[1] != 0.0 || M.j[2] != 0.0) ? 1 : 0;
+    const double bj = M.P * MUB / (QE * Ms * (1.0 + M.xi * M.xi));
+    for (int a = 0; a < 3; ++a)
+        p.cj[a] = (p.stt && ext[a] > 1) ? (float)(bj * M.j[a] / (2.0 * c->cell[a] * g0 * Ms)) : 0.f;
+    const double cad = M.stt_literal_eq7 ? 1.0 : 1.0 + M.alpha * M.xi;
+    p.c_ad = (float)(cad / (1.0 + M.alpha * M.alpha));
+    p.c_nad = (float)((M.xi - M.alpha) / (1.0 + M.alpha * M.alpha));
+}
+
+template <typename K>
+mm_status set_smem(mm_ctx* c, K kern)
+{
+    CUDA_TRY(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
+    return MM_OK;
+}
+
+// ---- one evaluation: the five passes, the last one carrying the epilogue `ep` ----
+mm_status launch_eval_generic(mm_ctx* c, const EpiParams& ep)
+{
+    const Geom& g = c->g;
+    cudaStream_t st = c->stream;
+    size_t bytes;
+    if (ep.demag) {
+        {   // a1
+            const int tx = pick_tx(g.Px, 2, 1, &bytes);
+            if (!tx) return fail(c, MM_EUNSUPPORTED, "x line too long for the shared-memory tile");
+            const int npair = 3 * g.Nz * ((g.Ny + 1) / 2);
+            k_gen_fwd_x<<<(npair + tx - 1) / tx, 256, bytes, st>>>(g, c->plan[0], ep.m_in, c->specA, tx);
+            c->launches++;
+        }
+        if (g.Pz > 1) {
+            {   // a2
+                const int tx = pick_tx(g.Py, 2, 1, &bytes);
+                if (!tx) return fail(c, MM_EUNSUPPORTED, "y line too long for the shared-memory tile");
+                dim3 grid((g.Cx + tx - 1) / tx, 3 * g.Nz);
+                k_gen_y<-1><<<grid, 256, bytes, st>>>(g, c->plan[1], c->specA, c->specB, tx);
+                c->launches++;
+            }
+            {   // a3
+                const int tx = pick_tx(g.Pz, 4, 1, &bytes);
+                if (!tx) return fail(c, MM_EUNSUPPORTED, "z line too long for the shared-memory tile");
+                dim3 grid((g.Cx + tx - 1) / tx, g.Py);
+                k_gen_mid<<<grid, 256, bytes, st>>>(g, c->plan[2], c->specB, c->khat, 2, tx);
+                c->launches++;
+            }
+            {   // a4
+                const int tx = pick_tx(g.Py, 2, 1, &bytes);
+                dim3 grid((g.Cx + tx - 1) / tx, 3 * g.Nz);
+                k_gen_y<1><<<grid, 256, bytes, st>>>(g, c->plan[1], c->specB, c->specA, tx);
+                c->launches++;
+            }
+        } else if (g.Py > 1) {   // 2D: y forward, multiply, y inverse in one kernel
+            const int tx = pick_tx(g.Py, 4, 1, &bytes);
+            if (!tx) return fail(c, MM_EUNSUPPORTED, "y line too long for the shared-memory tile");
+            dim3 grid((g.Cx + tx - 1) / tx, 1);
+            k_gen_mid<<<grid, 256, bytes, st>>>(g, c->plan[1], c->specA, c->khat, 1, tx);
+            c->launches++;
+        } else {
+            k_gen_mul1d<<<(g.Cx + 127) / 128, 128, 0, st>>>(g, c->specA, c->khat);
+            c->launches++;
+        }
+    }
+    {   // a5-a10
+        const int tx = pick_tx(g.Px, 2, 3, &bytes);
+        if (!tx) return fail(c, MM_EUNSUPPORTED, "x line too long for the shared-memory tile");
+        const int npy = (g.Ny + 1) / 2;
+        dim3 grid((npy + tx - 1) / tx, g.Nz);
+        k_gen_inv_x<<<grid, 256, bytes, st>>>(g, c->plan[0], c->specA, ep, tx);
+        c->launches++;
+    }
+    CUDA_TRY(c, cudaGetLastError());
+    return MM_OK;
+}
+
+mm_status launch_eval(mm_ctx* c, const EpiParams& ep)
+{
+    if (c->fast && c->fp.usable) return launch_eval_fast(c->fp, c->g, c->stream, c->specA, c->specB, c->khat, ep,
+                                                          &c->launches)
+                                            ? MM_OK
+                                            : fail(c, MM_ECUDA, std::string("fast path launch: ") +
+                                                                    cudaGetErrorString(cudaGetLastError()));
+    return launch_eval_generic(c, ep);
+}
+
+mm_status check_ready(mm_ctx* c)
+{
+    if (!c) return MM_EINVAL;
+    if (!c->has_mat) return fail(c, MM_ESTATE, "mm_set_material has not been called");
+    if (!c->has_demag) return fail(c, MM_ESTATE, "mm_demag_init has not been called");
+    return MM_OK;
+}
+
+double gamma0_of(const mm_ctx* c) { return c->mat.gamma0 > 0 ? c->mat.gamma0 : GAMMA0_DEFAULT; }
+
+// m_out = [normalise](m_n + sum_j a_j k_j): used when an evaluation is skipped (FSAL reuse).
+__global__ void k_combine(size_t n, const float* __restrict__ m_n, float* __restrict__ m_out, int na,
+                          float a0, float a1, const float* __restrict__ k0, const float* __restrict__ k1)
+{
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < 3 * n;
+         i += (size_t)gridDim.x * blockDim.x) {
+        float v = m_n[i] + a0 * k0[i];
+        if (na > 1) v += a1 * k1[i];
+        m_out[i] = v;
+    }
+}
+
+__global__ void k_copy4(const float4* __restrict__ src, float4* __restrict__ dst, size_t n4)
+{
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n4; i += (size_t)gridDim.x * blockDim.x)
+        dst[i] = src[i];
+}
+
+// One stage of `tab` (0-based s).  Enqueues only.
+mm_status run_stage(mm_ctx* c, float* m_dev, const Tableau& tab, int s, double dt, uint64_t step,
+                    bool adaptive_target)
+{
+    const int S = tab.S;
+    const double dtr = dt * gamma0_of(c) * c->mat.Ms;
+    EpiParams ep;
+    std::memset(&ep, 0, sizeof(ep));
+    fill_material(c, ep, step, dt);
+    ep.mode = EPI_STAGE;
+    ep.m_in = s == 0 ? m_dev : c->ms[(s - 1) & 1];
+    ep.m_n = m_dev;
+    ep.maxbits = c->maxbits;
+    const bool last = s == S - 1;
+    // k_s must be stored if a later stage row, the final combination or the FSAL hand-over reads it
+    bool store_k = false;
+    for (int r = s + 2; r < S; ++r) store_k |= tab.A[r][s] != 0.0;
+    if (!last) {
+        if (!tab.fsal) store_k |= tab.b[s] != 0.0;                       // read by the final combine
+        if (tab.embedded) store_k |= (tab.b[s] - tab.bs[s]) != 0.0;      // read by the error estimate
+    }
+    if (tab.fsal && last) store_k = true;                                // handed to the next step
+    ep.k_out = store_k ? c->kb[s] : nullptr;
+    const double* row = nullptr;     // coefficients of the state this stage produces
+    if (!last) row = tab.A[s + 1];
+    else if (!tab.fsal) row = tab.b;
+    if (row) {
+        ep.a_self = (float)(dtr * row[s]);
+        for (int j = 0; j < s; ++j)
+            if (row[j] != 0.0) {
+                ep.a[ep.na] = (float)(dtr * row[j]);
+                ep.ka[ep.na] = c->kb[j];
+                ep.na++;
+            }
+        const bool is_new_state = last || (tab.fsal && s == S - 2);
+        ep.normalise = is_new_state ? 1 : 0;
+        if (last) ep.m_out = (S > 1 && !adaptive_target) ? m_dev : c->mtmp;
+        else ep.m_out = c->ms[s & 1];
+    }
+    if (last) {
+        ep.do_err = 1;
+        if (tab.embedded) {
+            ep.e_self = (float)(dtr * (tab.b[s] - tab.bs[s]));
+            for (int j = 0; j < s; ++j) {
+                const double d = tab.b[j] - tab.bs[j];
+                if (d != 0.0) {
+                    ep.e[ep.ne] = (float)(dtr * d);
+                    ep.ke[ep.ne] = c->kb[j];
+                    ep.ne++;
+                }
+            }
+        } else {
+            ep.e_self = (float)dtr;   // max |dm| of the last stage: NaN sentinel and diagnostics
+        }
+    }
+    return launch_eval(c, ep);
+}
+
+// One trial step; enqueues everything, no synchronisation.  After it, maxbits holds the error
+// estimate and the new state is in *newstate (m_dev itself when written in place).
+mm_status enqueue_step(mm_ctx* c, float* m_dev, mm_method method, const Tableau& tab, double dt,
+                       bool adaptive_target, float** newstate)
+{
+    const int S = tab.S;
+    const size_t n = ncell(c->g);
+    CUDA_TRY(c, cudaMemsetAsync(c->maxbits, 0, sizeof(unsigned int), c->stream));
+    const uint64_t step = c->step_index;
+    int s0 = 0;
+    if (tab.fsal && c->k0_valid && c->k0_method == (int)method) {
+        // k_1 of this step is the last stage of the previous accepted step: skip the evaluation
+        const double dtr = dt * gamma0_of(c) * c->mat.Ms;
+        k_combine<<<148 * 8, 256, 0, c->stream>>>(n, m_dev, c->ms[0], 1, (float)(dtr * tab.A[1][0]), 0.f,
+                                                  c->kb[0], c->kb[0]);
+        c->launches++;
+        s0 = 1;
+    }
+    for (int s = s0; s < S; ++s) {
+        mm_status st = run_stage(c, m_dev, tab, s, dt, step, adaptive_target);
+        if (st != MM_OK) return st;
+    }
+    if (tab.fsal) *newstate = c->ms[(S - 2) & 1];
+    else *newstate = (S > 1 && !adaptive_target) ? m_dev : c->mtmp;
+    return MM_OK;
+}
+
+mm_status commit_step(mm_ctx* c, float* m_dev, mm_method method, const Tableau& tab, float* newstate)
+{
+    const size_t n = ncell(c->g);
+    if (newstate != m_dev)
+        CUDA_TRY(c, cudaMemcpyAsync(m_dev, newstate, 3 * n * sizeof(float), cudaMemcpyDeviceToDevice, c->stream));
+    if (tab.fsal) {
+        std::swap(c->kb[0], c->kb[tab.S - 1]);
+        c->k0_valid = true;
+        c->k0_method = (int)method;
+    }
+    c->step_index++;
+    return MM_OK;
+}
+
+}  // namespace
+
+// ==================================================================================================
+extern "C" {
+
+mm_status mm_create(mm_ctx** out, const int grid[3], const double cellsize[3], const int pbc[3],
+                    void* cuda_stream)
+{
+    if (!out || !grid || !cellsize || !pbc) return fail(nullptr, MM_EINVAL, "NULL argument");
+    *out = nullptr;
+    for (int a = 0; a < 3; ++a) {
+        if (grid[a] < 1) return fail(nullptr, MM_EINVAL, "grid sizes must be >= 1");
+        if (!(cellsize[a] > 0)) return fail(nullptr, MM_EINVAL, "cell sizes must be > 0");
+        if (pbc[a] < 0) return fail(nullptr, MM_EINVAL, "pbc must be >= 0");
+    }
+    int P[3];
+    for (int a = 0; a < 3; ++a) {
+        P[a] = pbc[a] > 0 ? grid[a] : (grid[a] > 1 ? 2 * grid[a] : 1);
+        if (!smooth235(P[a]))
+            return fail(nullptr, MM_EUNSUPPORTED, "padded size has a prime factor other than 2, 3, 5");
+    }
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) {
+        cudaGetLastError();
+        return fail(nullptr, MM_ECUDA, "no CUDA device: this library has no CPU fallback");
+    }
+    mm_ctx* c = new (std::nothrow) mm_ctx();
+    if (!c) return fail(nullptr, MM_ENOMEM, "host allocation failed");
+    Geom& g = c->g;
+    g.Nx = grid[0]; g.Ny = grid[1]; g.Nz = grid[2];
+    g.Px = P[0]; g.Py = P[1]; g.Pz = P[2];
+    g.Cx = P[0] / 2 + 1; g.Cy = P[1] / 2 + 1; g.Cz = P[2] / 2 + 1;
+    g.CxS = (g.Cx + 3) & ~3;     // rows start on 32-byte boundaries
+    g.perx = pbc[0] > 0; g.pery = pbc[1] > 0; g.perz = pbc[2] > 0;
+    for (int a = 0; a < 3; ++a) { c->cell[a] = cellsize[a]; c->pbc[a] = pbc[a]; }
+    c->stream = (cudaStream_t)cuda_stream;
+    c->has_mat = c->has_demag = false;
+    c->launches = 0;
+    c->fast = 1;
+    c->khat = nullptr; c->specA = c->specB = nullptr;
+    for (int a = 0; a < 3; ++a) c->tw[a] = nullptr;
+    for (int i = 0; i < 7; ++i) c->kb[i] = nullptr;
+    c->ms[0] = c->ms[1] = c->mtmp = nullptr;
+    c->maxbits = nullptr;
+    c->step_index = 0;
+    c->k0_valid = false;
+    c->k0_method = -1;
+    std::memset(&c->fp, 0, sizeof(c->fp));
+    *out = c;
+    return MM_OK;
+}
+
+mm_status mm_set_material(mm_ctx* c, const mm_material* mat)
+{
+    if (!c || !mat) return MM_EINVAL;
+    if (!(mat->Ms > 0)) return fail(c, MM_EINVAL, "Ms must be > 0");
+    if (mat->Aex < 0 || mat->alpha < 0 || mat->T < 0) return fail(c, MM_EINVAL, "Aex, alpha, T must be >= 0");
+    if (mat->Ku != 0.0 && mat->anis_u[0] == 0.0 && mat->anis_u[1] == 0.0 && mat->anis_u[2] == 0.0)
+        return fail(c, MM_EINVAL, "anisotropy axis is zero");
+    c->mat = *mat;
+    c->has_mat = true;
+    c->k0_valid = false;
+    return MM_OK;
+}
+
+mm_status mm_demag_init(mm_ctx* c)
+{
+    if (!c) return MM_EINVAL;
+    if (c->has_demag) return MM_OK;
+    const Geom& g = c->g;
+    const int grid[3] = { g.Nx, g.Ny, g.Nz };
+    const size_t nC = (size_t)g.Cx * g.Cy * g.Cz;
+    std::vector<float> kh;
+    try {
+        kh.resize(6 * nC);
+    } catch (const std::bad_alloc&) {
+        return fail(c, MM_ENOMEM, "host allocation of K-hat failed");
+    }
+    std::string err;
+    const int rc = mmh::build_khat(c->cell, grid, c->pbc, kh.data(), &err);
+    if (rc != 0) return fail(c, (mm_status)rc, err);
+    CUDA_TRY(c, cudaMalloc(&c->khat, 6 * nC * sizeof(float)));
+    CUDA_TRY(c, cudaMemcpy(c->khat, kh.data(), 6 * nC * sizeof(float), cudaMemcpyHostToDevice));
+    const size_t nA = (size_t)3 * g.Nz * g.Ny * g.CxS;
+    CUDA_TRY(c, cudaMalloc(&c->specA, nA * sizeof(float2)));
+    CUDA_TRY(c, cudaMemset(c->specA, 0, nA * sizeof(float2)));
+    if (g.Pz > 1) {
+        const size_t nB = (size_t)3 * g.Nz * g.Py * g.CxS;
+        CUDA_TRY(c, cudaMalloc(&c->specB, nB * sizeof(float2)));
+        CUDA_TRY(c, cudaMemset(c->specB, 0, nB * sizeof(float2)));
+    }
+    const int P[3] = { g.Px, g.Py, g.Pz };
+    for (int a = 0; a < 3; ++a) {
+        make_plan(c->plan[a], P[a]);
+        std::vector<float2> tw(P[a]);
+        for (int q = 0; q < P[a]; ++q) {
+            const long double ang = -2.0L * 3.14159265358979323846264338327950288L * q / P[a];
+            tw[q] = make_float2((float)cosl(ang), (float)sinl(ang));
+        }
+        CUDA_TRY(c, cudaMalloc(&c->tw[a], P[a] * sizeof(float2)));
+        CUDA_TRY(c, cudaMemcpy(c->tw[a], tw.data(), P[a] * sizeof(float2), cudaMemcpyHostToDevice));
+        c->plan[a].tw = c->tw[a];
+    }
+    const size_t fb = 3 * ncell(g) * sizeof(float);
+    for (int i = 0; i < 7; ++i) CUDA_TRY(c, cudaMalloc(&c->kb[i], fb));
+    for (int i = 0; i < 2; ++i) CUDA_TRY(c, cudaMalloc(&c->ms[i], fb));
+    CUDA_TRY(c, cudaMalloc(&c->mtmp, fb));
+    CUDA_TRY(c, cudaMalloc(&c->maxbits, sizeof(unsigned int)));
+    CUDA_TRY(c, cudaMemset(c->maxbits, 0, sizeof(unsigned int)));
+    mm_status s;
+    if ((s = set_smem(c, k_gen_fwd_x)) != MM_OK) return s;
+    if ((s = set_smem(c, k_gen_y<-1>)) != MM_OK) return s;
+    if ((s = set_smem(c, k_gen_y<1>)) != MM_OK) return s;
+    if ((s = set_smem(c, k_gen_mid)) != MM_OK) return s;
+    if ((s = set_smem(c, k_gen_inv_x)) != MM_OK) return s;
+    std::string ferr;
+    if (!fast_plan_init(c->fp, g, &ferr)) return fail(c, MM_ECUDA, ferr);
+    c->has_demag = true;
+    return MM_OK;
+}
+
+static mm_status eval_to(mm_ctx* c, const float* m_dev, float* out, int mode, uint64_t step, double dt_th)
+{
+    mm_status s = check_ready(c);
+    if (s != MM_OK) return s;
+    if (!m_dev || !out) return fail(c, MM_EINVAL, "NULL device pointer");
+    EpiParams ep;
+    std::memset(&ep, 0, sizeof(ep));
+    fill_material(c, ep, step, dt_th);
+    ep.mode = mode;
+    ep.m_in = m_dev;
+    ep.out = out;
+    ep.out_scale = mode == EPI_TORQUE ? (float)(gamma0_of(c) * c->mat.Ms) : (float)c->mat.Ms;
+    if (mode == EPI_HMS) ep.demag = 1;
+    return launch_eval(c, ep);
+}
+
+mm_status mm_heff(mm_ctx* c, const float* m_dev, float* H_dev, double t, uint64_t step, double dt_th)
+{
+    (void)t;
+    return eval_to(c, m_dev, H_dev, EPI_HEFF, step, dt_th);
+}
+
+mm_status mm_torque(mm_ctx* c, const float* m_dev, float* dmdt_dev, double t, uint64_t step, double dt_th)
+{
+    (void)t;
+    return eval_to(c, m_dev, dmdt_dev, EPI_TORQUE, step, dt_th);
+}
+
+mm_status mm_demag_field(mm_ctx* c, const float* m_dev, float* H_dev)
+{
+    return eval_to(c, m_dev, H_dev, EPI_HMS, 0, 0.0);
+}
+
+mm_status mm_step(mm_ctx* c, float* m_dev, mm_method method, double* dt_inout, double tol, double* t_inout,
+                  double* err_out, int* accepted_out)
+{
+    mm_status s = check_ready(c);
+    if (s != MM_OK) return s;
+    if (!m_dev || !dt_inout || !(*dt_inout > 0)) return fail(c, MM_EINVAL, "bad m_dev / dt");
+    const Tableau tab = make_tableau(method);
+    if (tab.S == 0) return fail(c, MM_EINVAL, "unknown method");
+    if (tab.embedded && c->mat.T > 0)
+        return fail(c, MM_EUNSUPPORTED, "thermal field needs a fixed-step method (reading A6)");
+    if (tab.embedded && !(tol > 0)) return fail(c, MM_EINVAL, "tol must be > 0");
+    const double dt = *dt_inout;
+    float* newstate = nullptr;
+    s = enqueue_step(c, m_dev, method, tab, dt, tab.embedded, &newstate);
+    if (s != MM_OK) return s;
+    unsigned int bits = 0;
+    CUDA_TRY(c, cudaMemcpyAsync(&bits, c->maxbits, sizeof(bits), cudaMemcpyDeviceToHost, c->stream));
+    CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+    float errf;
+    std::memcpy(&errf, &bits, sizeof(errf));
+    if (!std::isfinite(errf)) {
+        c->k0_valid = false;
+        return fail(c, MM_ENUMERIC, "non-finite value met by the max-norm reduction");
+    }
+    int accept = 1;
+    double err = 0.0;
+    if (tab.embedded) {
+        // reading A10: accept iff err <= tol; dt <- dt clamp(0.8 (tol/err)^(1/order), 0.2, 2)
+        err = (double)errf;
+        accept = err <= tol;
+        const double order = method == MM_RKDP ? 5.0 : (method == MM_RK23 ? 3.0 : 2.0);
+        const double fac = err == 0.0 ? 2.0 : std::fmin(2.0, std::fmax(0.2, 0.8 * std::pow(tol / err, 1.0 / order)));
+        *dt_inout = dt * fac;
+    }
+    if (accept) {
+        s = commit_step(c, m_dev, method, tab, newstate);
+        if (s != MM_OK) return s;
+        CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+        if (t_inout) *t_inout += dt;
+    }
+    // on a rejected FSAL step k_1 = f(m_n) in kb[0] is still valid: keep it
+    if (tab.fsal && !accept && !c->k0_valid) {
+        c->k0_valid = true;
+        c->k0_method = (int)method;
+    }
+    if (err_out) *err_out = err;
+    if (accepted_out) *accepted_out = accept;
+    return MM_OK;
+}
+
+mm_status mm_steps_fixed(mm_ctx* c, float* m_dev, mm_method method, double dt, int n, double* t_inout,
+                         double* max_err_out)
+{
+    mm_status s = check_ready(c);
+    if (s != MM_OK) return s;
+    if (!m_dev || !(dt > 0) || n < 0) return fail(c, MM_EINVAL, "bad m_dev / dt / n");
+    const Tableau tab = make_tableau(method);
+    if (tab.S == 0) return fail(c, MM_EINVAL, "unknown method");
+    std::vector<unsigned int> bits((size_t)n, 0u);
+    unsigned int* dbits = nullptr;
+    if (n > 0) CUDA_TRY(c, cudaMalloc(&dbits, (size_t)n * sizeof(unsigned int)));
+    for (int i = 0; i < n; ++i) {
+        float* newstate = nullptr;
+        s = enqueue_step(c, m_dev, method, tab, dt, false, &newstate);
+        if (s == MM_OK) s = commit_step(c, m_dev, method, tab, newstate);
+        if (s != MM_OK) { cudaFree(dbits); return s; }
+        cudaMemcpyAsync(dbits + i, c->maxbits, sizeof(unsigned int), cudaMemcpyDeviceToDevice, c->stream);
+    }
+    if (n > 0) {
+        cudaMemcpyAsync(bits.data(), dbits, (size_t)n * sizeof(unsigned int), cudaMemcpyDeviceToHost, c->stream);
+        cudaError_t e = cudaStreamSynchronize(c->stream);
+        cudaFree(dbits);
+        if (e != cudaSuccess) return fail(c, MM_ECUDA, cudaGetErrorString(e));
+    }
+    double maxerr = 0.0;
+    for (int i = 0; i < n; ++i) {
+        float f;
+        std::memcpy(&f, &bits[i], sizeof(f));
+        if (!std::isfinite(f)) {
+            c->k0_valid = false;
+            return fail(c, MM_ENUMERIC, "non-finite value met by the max-norm reduction");
+        }
+        if (tab.embedded && f > maxerr) maxerr = f;
+    }
+    if (t_inout) *t_inout += dt * n;
+    if (max_err_out) *max_err_out = maxerr;
+    return MM_OK;
+}
+
+mm_status mm_fused_eval(mm_ctx* c, float* m_dev, mm_method method, int stage, double dt, uint64_t step)
+{
+    mm_status s = check_ready(c);
+    if (s != MM_OK) return s;
+    const Tableau tab = make_tableau(method);
+    if (tab.S == 0 || stage < 0 || stage >= tab.S || !m_dev || !(dt > 0))
+        return fail(c, MM_EINVAL, "bad method / stage / dt");
+    c->k0_valid = false;
+    return run_stage(c, m_dev, tab, stage, dt, step, false);
+}
+
+mm_status mm_reset_stepper(mm_ctx* c, uint64_t step_index)
+{
+    if (!c) return MM_EINVAL;
+    c->step_index = step_index;
+    c->k0_valid = false;
+    return MM_OK;
+}
+
+mm_status mm_get_demag_kernel(mm_ctx* c, int comp, float* host_out, size_t n)
+{
+    if (!c || !host_out || comp < 0 || comp > 5) return MM_EINVAL;
+    if (!c->has_demag) return fail(c, MM_ESTATE, "mm_demag_init has not been called");
+    const size_t nC = (size_t)c->g.Cx * c->g.Cy * c->g.Cz;
+    if (n < nC) return fail(c, MM_EINVAL, "host_out too small");
+    CUDA_TRY(c, cudaMemcpy(host_out, c->khat + comp * nC, nC * sizeof(float), cudaMemcpyDeviceToHost));
+    return MM_OK;
+}
+
+mm_status mm_demag_tensor_host(const double cellsize[3], const int grid[3], const int pbc[3], size_t n,
+                               const long* off_host, double* out_host)
+{
+    if (!cellsize || !grid || !pbc || (n && (!off_host || !out_host))) return MM_EINVAL;
+    mmh::tensor_at(cellsize, grid, pbc, n, off_host, out_host);
+    return MM_OK;
+}
+
+mm_status mm_demag_khat_host(const double cellsize[3], const int grid[3], const int pbc[3], float* out_host,
+                             size_t n)
+{
+    if (!cellsize || !grid || !pbc || !out_host) return MM_EINVAL;
+    size_t nC = 1;
+    for (int a = 0; a < 3; ++a) {
+        const int P = pbc[a] > 0 ? grid[a] : (grid[a] > 1 ? 2 * grid[a] : 1);
+        nC *= (size_t)(P / 2 + 1);
+    }
+    if (n < 6 * nC) return MM_EINVAL;
+    std::string err;
+    return (mm_status)mmh::build_khat(cellsize, grid, pbc, out_host, &err);
+}
+
+mm_status mm_padded_size(const mm_ctx* c, int P_out[3], int C_out[3])
+{
+    if (!c) return MM_EINVAL;
+    if (P_out) { P_out[0] = c->g.Px; P_out[1] = c->g.Py; P_out[2] = c->g.Pz; }
+    if (C_out) { C_out[0] = c->g.Cx; C_out[1] = c->g.Cy; C_out[2] = c->g.Cz; }
+    return MM_OK;
+}
+
+uint64_t mm_launch_count(const mm_ctx* c) { return c ? c->launches : 0; }
+
+mm_status mm_set_fast_path(mm_ctx* c, int enable)
+{
+    if (!c) return MM_EINVAL;
+    c->fast = enable ? 1 : 0;
+    return MM_OK;
+}
+
+mm_status mm_copy_bandwidth(mm_ctx* c, const void* src_dev, void* dst_dev, size_t nbytes, int reps,
+                            double* sec_out)
+{
+    if (!c || !src_dev || !dst_dev || nbytes < 16 || reps < 1 || !sec_out) return MM_EINVAL;
+    cudaEvent_t e0, e1;
+    CUDA_TRY(c, cudaEventCreate(&e0));
+    CUDA_TRY(c, cudaEventCreate(&e1));
+    const size_t n4 = nbytes / 16;
+    k_copy4<<<148 * 16, 512, 0, c->stream>>>((const float4*)src_dev, (float4*)dst_dev, n4);
+    CUDA_TRY(c, cudaEventRecord(e0, c->stream));
+    for (int i = 0; i < reps; ++i)
+        k_copy4<<<148 * 16, 512, 0, c->stream>>>((const float4*)src_dev, (float4*)dst_dev, n4);
+    CUDA_TRY(c, cudaEventRecord(e1, c->stream));
+    CUDA_TRY(c, cudaEventSynchronize(e1));
+    float ms = 0.f;
+    CUDA_TRY(c, cudaEventElapsedTime(&ms, e0, e1));
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    c->launches += reps + 1;
+    *sec_out = (double)ms * 1e-3 / reps;
+    return MM_OK;
+}
+
+const char* mm_last_error(const mm_ctx* c) { return c ? c->err.c_str() : g_create_error.c_str(); }
+
+void mm_destroy(mm_ctx* c)
+{
+    if (!c) return;
+    cudaFree(c->khat);
+    cudaFree(c->specA);
+    cudaFree(c->specB);
+    for (int a = 0; a < 3; ++a) cudaFree(c->tw[a]);
+    for (int i = 0; i < 7; ++i) cudaFree(c->kb[i]);
+    cudaFree(c->ms[0]);
+    cudaFree(c->ms[1]);
+    cudaFree(c->mtmp);
+    cudaFree(c->maxbits);
+    fast_plan_destroy(c->fp);
+    delete c;
+}
+
+}  // extern "C"

@@ -1,0 +1,80 @@
+// mm_common.cuh -- shared device-side types of the hot path.
+//
+// Product code.  Nothing here is shared with oracle/.
+//
+// Layouts (x fastest everywhere):
+//   field      float  [3][Nz][Ny][Nx]                      m, H, k_s, caller or context owned
+//   specA      float2 [3][Nz][Ny][CxS]                     after the x pass   (CxS >= Cx = Px/2+1)
+//   specB      float2 [3][Nz][Py][CxS]                     after the y pass   (3D only)
+//   khat       float  [6][Cz][Cy][Cx]  (xx,yy,zz,xy,xz,yz) one octant, includes -1/(Px Py Pz)
+// Units on the device (section 3.3): fields in units of Ms, time in 1/(gamma0 Ms).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace mm {
+
+struct Geom {
+    int Nx, Ny, Nz;      // cells
+    int Px, Py, Pz;      // padded transform sizes (reading A9)
+    int Cx, Cy, Cz;      // P/2 + 1
+    int CxS;             // row stride of the spectra, in complex elements
+    int perx, pery, perz;
+};
+
+enum EpiMode { EPI_HMS = 0, EPI_HEFF = 1, EPI_TORQUE = 2, EPI_STAGE = 3 };
+
+#define MM_MAXK 8
+
+// Everything the fused epilogue needs (steps a6-a10), passed by value.
+struct EpiParams {
+    const float* m_in;   // state this evaluation acts on
+    float* out;          // EPI_HMS / EPI_HEFF / EPI_TORQUE: output field
+    int mode;
+    int demag;           // 0: H_ms taken as zero
+    float out_scale;     // Ms (A/m) for fields, gamma0 Ms (1/s) for the torque
+    // local field terms, reduced units
+    float wex[3];        // 2A/(mu0 Ms^2 d_a^2); 0 for a one-cell axis           Eq. (3)
+    float kan, u[3];     // 2Ku/(mu0 Ms^2), axis                                  Eq. (4)
+    float hext[3];       // B/(mu0 Ms)
+    int thermal;         // Eq. (6)
+    float sig_th;        // sqrt(2 alpha kB T/(gamma0 mu0 Ms V dt)) / Ms
+    uint32_t key0, key1, step0, step1;
+    // torque
+    float alpha, inv1pa2;   // Eq. (1)
+    int stt;                // Eq. (7)-(8)
+    float cj[3];            // b_j j_a / (2 d_a gamma0 Ms)
+    float c_ad, c_nad;      // (1 + alpha xi | 1)/(1+alpha^2), (xi - alpha)/(1+alpha^2)
+    // Runge-Kutta stage combine (EPI_STAGE)
+    const float* m_n;    // state at the start of the step
+    float* m_out;        // next stage input / new state (may be NULL)
+    float* k_out;        // where k_s is stored (may be NULL)
+    int normalise;
+    float a_self;        // dt * a_{s+1,s}
+    int na;
+    float a[MM_MAXK];
+    const float* ka[MM_MAXK];
+    int do_err;          // error / max-norm reduction
+    float e_self;
+    int ne;
+    float e[MM_MAXK];
+    const float* ke[MM_MAXK];
+    unsigned int* maxbits;   // atomicMax target (bit pattern of a non-negative float)
+};
+
+__device__ __forceinline__ float2 cadd(float2 a, float2 b) { return make_float2(a.x + b.x, a.y + b.y); }
+__device__ __forceinline__ float2 csub(float2 a, float2 b) { return make_float2(a.x - b.x, a.y - b.y); }
+__device__ __forceinline__ float2 cmul(float2 a, float2 b)
+{
+    return make_float2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x);
+}
+__device__ __forceinline__ float2 cconj(float2 a) { return make_float2(a.x, -a.y); }
+__device__ __forceinline__ float2 cscale(float2 a, float s) { return make_float2(a.x * s, a.y * s); }
+// multiply by SGN * i  (SGN = -1: forward transform convention exp(-i ...))
+template <int SGN>
+__device__ __forceinline__ float2 cmuli(float2 a)
+{
+    return SGN < 0 ? make_float2(a.y, -a.x) : make_float2(-a.y, a.x);
+}
+
+}  // namespace mm

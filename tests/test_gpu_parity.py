@@ -1,0 +1,242 @@
+"""GPU parity: the CUDA path (through the C-ABI) against the fp64 oracle, element by element.
+
+Tolerances (BASELINE.json north_star): per H_eff evaluation 2e-5 of max|H| (fp32 against fp64); after
+100 fixed-step RK4 steps 1e-4 in m.  Reading A12: the magnetostatic field is also checked on its own
+scale so that a demag error cannot hide under the exchange field.
+"""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+from oracle import mm_oracle as orc                      # noqa: E402
+from paper_1102_3069_b200 import workloads as wlm        # noqa: E402
+from tests import util                                   # noqa: E402
+
+TOL_H = 2e-5
+TOL_M = 1e-4
+
+GRIDS = [
+    # grid, cell, pbc                       what it exercises
+    ((32, 32, 1), (4e-9, 4e-9, 4e-9), (0, 0, 0)),        # config 1 shape
+    ((24, 10, 6), (3e-9, 4e-9, 5e-9), (0, 0, 0)),        # radix 3 and 5 (48, 20, 12)
+    ((15, 9, 5), (3e-9, 3e-9, 3e-9), (0, 0, 0)),         # odd sizes, ragged pair tail (30, 18, 10)
+    ((40, 6, 3), (2e-9, 2e-9, 4e-9), (0, 0, 0)),         # 80 = 16 * 5
+    ((16, 12, 1), (4e-9, 4e-9, 2e-9), (2, 2, 0)),        # periodic film, no padding in x, y
+    ((8, 6, 4), (4e-9, 3e-9, 2e-9), (0, 1, 2)),          # mixed periodic / open 3D
+    ((16, 1, 1), (2e-9, 3e-9, 4e-9), (0, 0, 0)),         # 1D chain: multiply without y / z pass
+    ((1, 1, 1), (5e-9, 5e-9, 5e-9), (0, 0, 0)),          # macrospin
+    ((1, 8, 2), (5e-9, 4e-9, 3e-9), (0, 0, 0)),          # one cell along x
+    ((64, 48, 2), (3e-9, 3e-9, 3e-9), (0, 0, 0)),        # several tiles per pass
+]
+
+
+def _cmp(a_gpu, b_ref, tol, scale=None):
+    a = a_gpu.double().cpu().numpy()
+    s = np.abs(b_ref).max() if scale is None else scale
+    err = np.abs(a - b_ref).max()
+    assert err <= tol * s, f"max err {err:.3e} > {tol:.1e} * {s:.3e}"
+    return err / s if s > 0 else 0.0
+
+
+@pytest.mark.parametrize("fast", [False, True])
+@pytest.mark.parametrize("grid,cell,pbc", GRIDS)
+def test_demag_field_matches_direct_pair_sum(grid, cell, pbc, fast):
+    wl = util.small(grid, cell, pbc)
+    m = wlm.initial_m(wl)
+    sim = util.gpu_sim(wl, fast=fast)
+    H = sim.demag_field(util.to_dev(m))
+    ncell = grid[0] * grid[1] * grid[2]
+    if ncell <= 2048:
+        ref = orc.demag_field_direct(m.astype(np.float64), wl.mat["Ms"], grid, cell, pbc)
+    else:
+        ref = util.oracle_problem(wl).demag_field(m.astype(np.float64))
+    _cmp(H, ref, TOL_H, scale=max(np.abs(ref).max(), 1e-3 * wl.mat["Ms"]))
+    sim.close()
+
+
+@pytest.mark.parametrize("fast", [False, True])
+@pytest.mark.parametrize("grid,cell,pbc", GRIDS)
+def test_heff_and_torque_match_oracle(grid, cell, pbc, fast):
+    wl = util.small(grid, cell, pbc, T=300.0, seed=12345678901234, j=(1e12, -5e11, 2e11), P=0.5, xi=0.04)
+    m = wlm.initial_m(wl)
+    pb = util.oracle_problem(wl)
+    sim = util.gpu_sim(wl, fast=fast)
+    md = util.to_dev(m)
+    m64 = m.astype(np.float64)
+    step, dt = (1 << 33) + 5, 5e-14
+    Href = pb.heff(m64, step, dt)
+    _cmp(sim.heff(md, step=step, dt_thermal=dt), Href, TOL_H)
+    Tref = pb.torque(m64, step, dt)
+    _cmp(sim.torque(md, step=step, dt_thermal=dt), Tref, TOL_H)
+    # without the thermal field (which dominates the scale at these cell sizes)
+    wl2 = util.small(grid, cell, pbc, j=(1e12, -5e11, 2e11), P=0.5, xi=0.04)
+    pb2 = util.oracle_problem(wl2)
+    sim.set_material(wl2.mat)
+    _cmp(sim.heff(md), pb2.heff(m64), TOL_H)
+    _cmp(sim.torque(md), pb2.torque(m64), TOL_H)
+    sim.close()
+
+
+def test_local_terms_alone_demag_off():
+    wl = util.small((24, 10, 6), Aex=1.3e-11)
+    m = wlm.initial_m(wl)
+    pb = util.oracle_problem(wl, demag="none")
+    sim = util.gpu_sim(wl, demag=False)
+    _cmp(sim.heff(util.to_dev(m)), pb.heff(m.astype(np.float64)), 2e-6)
+    sim.close()
+
+
+def test_config1_heff_then_100_rk4_steps():
+    """BASELINE.json configs[0]: 32x32x1, one H_eff against the direct O(N^2) sum, then 100 RK4 steps."""
+    wl = wlm.config(0)
+    m = wlm.initial_m(wl)
+    m64 = m.astype(np.float64)
+    sim = util.gpu_sim(wl)
+    md = util.to_dev(m)
+    pb1 = util.oracle_problem(wl, demag="direct")
+    _cmp(sim.heff(md), pb1.heff(m64), TOL_H)
+    pb = util.oracle_problem(wl)
+    mo = m64.copy()
+    for _ in range(wl.steps):
+        mo = orc.rk4_step(pb.torque, mo, wl.dt)
+    t, _ = sim.steps_fixed(md, "rk4", wl.dt, wl.steps)
+    assert abs(t - wl.steps * wl.dt) < 1e-20
+    err = np.abs(md.double().cpu().numpy() - mo).max()
+    assert err <= TOL_M, err
+    # same through mm_step, one call per step
+    md2 = util.to_dev(m)
+    sim.reset_stepper(0)
+    for _ in range(wl.steps):
+        acc, _, dtn, _ = sim.step(md2, "rk4", wl.dt)
+        assert acc and dtn == wl.dt
+    assert np.abs(md2.double().cpu().numpy() - mo).max() <= TOL_M
+    sim.close()
+
+
+@pytest.mark.parametrize("grid,cell,pbc", [((24, 10, 6), (3e-9, 4e-9, 5e-9), (0, 0, 0)),
+                                           ((16, 12, 1), (4e-9, 4e-9, 2e-9), (2, 2, 0))])
+def test_rk4_with_thermal_and_stt_trajectory(grid, cell, pbc):
+    wl = util.small(grid, cell, pbc, init="xnoise", alpha=0.1, T=300.0, seed=3, j=(1e12, 0, 0), P=0.5,
+                    xi=0.04)
+    m = wlm.initial_m(wl)
+    pb = util.oracle_problem(wl)
+    dt, n = 5e-14, 10
+    mo = m.astype(np.float64)
+    for s in range(n):
+        mo = orc.rk4_step(lambda x: pb.torque(x, s, dt), mo, dt)
+    sim = util.gpu_sim(wl)
+    md = util.to_dev(m)
+    sim.steps_fixed(md, "rk4", dt, n)
+    assert np.abs(md.double().cpu().numpy() - mo).max() <= TOL_M
+    sim.close()
+
+
+def test_rk1_steps():
+    wl = util.small((15, 9, 5), alpha=0.5)
+    m = wlm.initial_m(wl)
+    pb = util.oracle_problem(wl)
+    mo = m.astype(np.float64)
+    for _ in range(20):
+        mo = orc.rk1_step(pb.torque, mo, 2e-14)
+    sim = util.gpu_sim(wl)
+    md = util.to_dev(m)
+    sim.steps_fixed(md, "rk1", 2e-14, 20)
+    assert np.abs(md.double().cpu().numpy() - mo).max() <= TOL_M
+    sim.close()
+
+
+def test_rkdp_replay_of_oracle_step_sequence_and_free_run():
+    """Reading A10: adaptive runs are compared by replaying the oracle's accepted dt sequence."""
+    wl = util.small((24, 10, 6), init="tilted", alpha=0.02, Bext=(-0.0246, 0.0043, 0.0), Ku=0.0)
+    m = wlm.initial_m(wl)
+    pb = util.oracle_problem(wl)
+    tol, dt = 1e-5, 1e-13
+    mo = m.astype(np.float64)
+    k1, seq, errs, trials = None, [], [], 0
+    while len(seq) < 30:
+        mn, err, k7 = orc.rkdp_step(pb.torque, mo, dt, k1)
+        ok, dtn = orc.rkdp_controller(dt, err, tol)
+        trials += 1
+        if ok:
+            seq.append(dt); errs.append(err); mo, k1 = mn, k7
+        dt = dtn
+    sim = util.gpu_sim(wl)
+    md = util.to_dev(m)
+    for d, e in zip(seq, errs):
+        _, ge = sim.steps_fixed(md, "rkdp", d, 1)
+        assert abs(ge - e) <= 0.02 * e + 1e-9, (ge, e)
+    assert np.abs(md.double().cpu().numpy() - mo).max() <= TOL_M
+    # free run with the library's own controller: same number of trials, same end time (to a few %)
+    md = util.to_dev(m)
+    sim.reset_stepper(0)
+    dt, t, nacc, ntr = 1e-13, 0.0, 0, 0
+    while nacc < 30:
+        acc, err, dt, t = sim.step(md, "rkdp", dt, tol, t)
+        ntr += 1
+        nacc += int(acc)
+    assert abs(ntr - trials) <= 2
+    assert abs(t - sum(seq)) <= 0.05 * sum(seq)
+    assert np.abs(md.double().cpu().numpy() - mo).max() <= 1e-3
+    sim.close()
+
+
+def test_thermal_with_adaptive_method_is_refused():
+    import paper_1102_3069_b200 as mm
+    wl = util.small((8, 6, 4), T=300.0)
+    sim = util.gpu_sim(wl)
+    md = util.to_dev(wlm.initial_m(wl))
+    with pytest.raises(mm.MMError) as e:
+        sim.step(md, "rkdp", 1e-13)
+    assert e.value.status == 5
+    sim.close()
+
+
+def test_call_order_and_nan_are_reported():
+    import paper_1102_3069_b200 as mm
+    wl = util.small((8, 6, 4))
+    sim = mm.Sim(wl.grid, wl.cell, wl.pbc, None, demag_init=False)
+    md = util.to_dev(wlm.initial_m(wl))
+    with pytest.raises(mm.MMError) as e:
+        sim.heff(md)
+    assert e.value.status == 4
+    sim.set_material(wl.mat)
+    with pytest.raises(mm.MMError) as e:
+        sim.heff(md)
+    assert e.value.status == 4
+    sim.demag_init()
+    sim.heff(md)
+    md[0, 1, 2, 3] = float("nan")
+    with pytest.raises(mm.MMError) as e:
+        sim.step(md, "rk4", 1e-13)
+    assert e.value.status == 6
+    sim.close()
+
+
+def test_uniform_state_mean_field_is_sample_demag_factor():
+    """Pin P7 on the GPU alone: mean of H_a/Ms over a uniformly magnetised sample = -N_aa of one cell
+    the size of the sample (coarse-graining identity); the latter comes from the oracle tensor."""
+    grid, cell = (32, 32, 1), (4e-9, 4e-9, 4e-9)
+    for a in range(3):
+        d = [0.0, 0.0, 0.0]; d[a] = 1.0
+        wl = wlm.Workload("u", grid, cell, (0, 0, 0), wlm._mat(), "uniform", 0, extra={"dir": d})
+        sim = util.gpu_sim(wl)
+        H = sim.demag_field(util.to_dev(wlm.initial_m(wl))).double().cpu().numpy()
+        big = orc.tensor_at([[0, 0, 0]], tuple(c * n for c, n in zip(cell, grid)))[0]
+        assert abs(H[a].mean() / wl.mat["Ms"] + big[a]) <= 2e-6
+        sim.close()
+
+
+def test_reciprocity_and_positive_energy_on_gpu():
+    """Pin P18: sum m1.H[m2] = sum m2.H[m1]; demag energy >= 0."""
+    wl = util.small((64, 48, 2), (3e-9, 3e-9, 3e-9))
+    sim = util.gpu_sim(wl)
+    m1 = util.to_dev(wlm.initial_m(wl))
+    wl.seed = 99
+    m2 = util.to_dev(wlm.initial_m(wl))
+    H1 = sim.demag_field(m1).double()
+    H2 = sim.demag_field(m2).double()
+    a = float((m1.double() * H2).sum()); b = float((m2.double() * H1).sum())
+    assert abs(a - b) <= 1e-5 * max(abs(a), abs(b))
+    assert float((m1.double() * H1).sum()) < 0.0
+    sim.close()
