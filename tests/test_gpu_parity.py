@@ -11,7 +11,7 @@ pytestmark = pytest.mark.gpu
 
 from oracle import mm_oracle as orc                      # noqa: E402
 from paper_1102_3069_b200 import workloads as wlm        # noqa: E402
-from tests import util                                   # noqa: E402
+import mmtest_util as util                               # noqa: E402
 
 TOL_H = 2e-5
 TOL_M = 1e-4
