@@ -207,7 +207,7 @@ void fill_material(const mm_ctx* c, EpiParams& p, uint64_t step, double dt_therm
 template <typename K>
 mm_status set_smem(mm_ctx* c, K kern)
 {
-    CUDA_TRY(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
+    CUDA_TRY(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 224 * 1024));
     return MM_OK;
 }
 
