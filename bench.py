@@ -1,0 +1,319 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the hot path (one effective-field evaluation + LL torque per RK stage).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--config NAME]
+
+One "step" is one classical RK4 time step = 4 fused evaluations (FFT convolution, local field terms,
+torque, stage combine, max-norm reduction: every row of the hot-path table in DESIGN.md) on the
+headline grid 512x512x64 (the grid BASELINE.json's metric is quoted on).  `value` = evaluations per
+second with the state resident in HBM; `e2e` = the same through mm_steps_fixed_host with the state in
+pinned HOST memory, host<->device copies inside the timed region.  The working set (> 2 GB) is far
+larger than L2 (126 MB), so no explicit L2 flush is needed between iterations.
+
+N > 1: the path does not shard without a global transpose (replicas only), so
+each rank runs an independent replica of the same problem; value = all ranks' evaluations / max time.
+
+--impl reference times the CPU oracle (test infrastructure, fp64, numpy FFT) on a bounded sample.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "H_eff+torque evaluations per second at 512x512x64 (RK4 stages)"
+UNIT = "evals/s"
+
+
+def load_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+def workload(name):
+    from paper_1102_3069_b200 import workloads as wlm
+    if name == "headline":
+        return wlm.config(5)
+    if name.startswith("cfg"):
+        return wlm.config(int(name[3:]))
+    g = tuple(int(v) for v in name.split("x"))
+    return wlm.scaled(wlm.config(5), g)
+
+
+def algorithmic_bytes(wl, method="rk4"):
+    """per-pass bytes of one evaluation (averaged over the RK4 stages for
+    the last pass), live data only, K-hat octant read once."""
+    Nx, Ny, Nz = wl.grid
+    P = [n if p > 0 else (2 * n if n > 1 else 1) for n, p in zip(wl.grid, wl.pbc)]
+    Cx, Cy, Cz = P[0] // 2 + 1, P[1] // 2 + 1, P[2] // 2 + 1
+    N = Nx * Ny * Nz
+    sA = 8 * Cx * Ny * Nz * 3
+    sB = 8 * Cx * P[1] * Nz * 3
+    ncomp = 6 if Nz > 1 else 4
+    khat = 4 * ncomp * Cx * Cy * Cz
+    b = {}
+    b["fwd_x"] = 12 * N + sA
+    if P[2] > 1:
+        b["fwd_y"] = sA + sB
+        b["mid"] = 2 * sB + khat
+        b["inv_y"] = sA + sB
+    else:
+        b["fwd_y"] = 0
+        b["mid"] = 2 * sA + khat
+        b["inv_y"] = 0
+    # RK4 stage combine: (k1, m2) (m_n, k2, m3) (m_n, k3, m4) (m_n, k1..k3, m) = 24+36+36+60 over 4 stages
+    comb = (24 + 36 + 36 + 60) / 4.0
+    b["inv_x"] = sA + 12 * N + comb * N
+    b["total"] = sum(b.values())
+    return b
+
+
+class ClockSampler(threading.Thread):
+    def __init__(self, index):
+        super().__init__(daemon=True)
+        self.cmd = ["nvidia-smi", "-i", str(index),
+                    "--query-gpu=clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,"
+                    "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+                    "clocks_event_reasons.sw_power_cap", "--format=csv,noheader,nounits", "-lms", "100"]
+        self.rows, self.proc = [], None
+
+    def run(self):
+        try:
+            self.proc = subprocess.Popen(self.cmd, stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            for line in self.proc.stdout:
+                self.rows.append(line.strip())
+        except Exception:
+            pass
+
+    def stop(self):
+        if self.proc is not None:
+            self.proc.terminate()
+        self.join(timeout=2)
+        sm, mx, reasons = [], 0.0, set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            f = [x.strip() for x in r.split(",")]
+            try:
+                sm.append(float(f[0])); mx = max(mx, float(f[1]))
+            except Exception:
+                continue
+            for n, v in zip(names, f[2:6]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        sm.sort()
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": mx or None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def oracle_sample_eval(sample_grid, nevals):
+    """Time the oracle (as it stands) on a sub-grid of the headline workload; returns (sec per eval, cells)."""
+    import numpy as np
+    from oracle import mm_oracle as orc
+    from paper_1102_3069_b200 import workloads as wlm
+    wl = wlm.scaled(wlm.config(5), sample_grid)
+    d = wl.mat
+    mat = orc.Material(Ms=d["Ms"], Aex=d["Aex"], alpha=d["alpha"], gamma0=d["gamma0"], Ku=d["Ku"],
+                       anis_u=tuple(d["anis_u"]), Bext=tuple(d["Bext"]))
+    pb = orc.Problem(wl.grid, wl.cell, wl.pbc, mat)
+    m = wlm.initial_m(wl).astype(np.float64)
+    pb.torque(m)                               # warm-up
+    ts = []
+    for _ in range(nevals):
+        t0 = time.perf_counter()
+        pb.torque(m)
+        ts.append(time.perf_counter() - t0)
+    ts.sort()
+    return ts[len(ts) // 2], wl.grid[0] * wl.grid[1] * wl.grid[2]
+
+
+def host_threads():
+    try:
+        return len(os.sched_getaffinity(0))
+    except Exception:
+        return os.cpu_count() or 1
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    sample = (128, 128, 64)
+    full = 512 * 512 * 64
+    # one "step" = 4 evaluations (one RK4 step's worth) of the sample
+    t0 = time.perf_counter()
+    sec, cells = oracle_sample_eval(sample, 4 * max(1, args.steps))
+    frac = cells / full
+    evals_per_s = (1.0 / sec) * frac        # scaled to the full grid by cell count
+    out = {"impl": "reference", "metric": METRIC, "value": evals_per_s, "unit": UNIT, "n_gpus": args.gpus,
+           "steps": args.steps, "warmup": args.warmup, "ms_per_step": 4 * sec / frac * 1e3,
+           "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+           "data": "synthetic", "config": {"workload": "headline 512x512x64 vortex state (bounded sample)",
+                                           "sample": "x".join(map(str, sample))},
+           "cpu_baseline": {"value": evals_per_s, "unit": UNIT, "cores": host_threads(), "kind": "oracle",
+                            "sample": f"{sample[0]}x{sample[1]}x{sample[2]} sub-grid of the headline workload "
+                                      f"(1/{round(1 / frac)} of its cells), median eval time scaled by cell count"},
+           "e2e": {"value": evals_per_s, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+           "wall_s": time.perf_counter() - t0}
+    print(json.dumps(out))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours")
+    ap.add_argument("--config", default="headline")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--generic", action="store_true", help="force the generic shared-memory FFT kernels")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+
+    import numpy as np
+    import torch
+    import paper_1102_3069_b200 as mm
+    from paper_1102_3069_b200 import workloads as wlm
+
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    wl = workload(args.config)
+    N = wl.grid[0] * wl.grid[1] * wl.grid[2]
+    m0 = torch.from_numpy(wlm.initial_m(wl))
+    t0 = time.perf_counter()
+    sim = mm.Sim(wl.grid, wl.cell, wl.pbc, wl.mat)
+    setup_s = time.perf_counter() - t0
+    if args.generic:
+        sim.set_fast_path(False)
+    md = m0.cuda()
+    dt = wl.dt if wl.method == "rk4" else 5e-14
+    method = "rk4"
+    stages = 4
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- device-resident timing ----
+    sim.steps_fixed(md, method, dt, max(3, args.warmup))
+    barrier()
+    sampler = ClockSampler(local)
+    sampler.start()
+    sim.kernel_timing(True)
+    l0 = sim.launch_count()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    e0.record()
+    sim.steps_fixed(md, method, dt, args.steps)
+    e1.record()
+    barrier()
+    sec = e0.elapsed_time(e1) * 1e-3
+    launches = sim.launch_count() - l0
+    kt = sim.kernel_times()
+    sim.kernel_timing(False)
+    clocks = sampler.stop()
+    if dist is not None:
+        t = torch.tensor([sec], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        sec = float(t.item())
+    evals = stages * args.steps
+    value = world * evals / sec
+    assert torch.isfinite(md).all()
+
+    # ---- end to end: state in pinned host memory, copies inside the timed region ----
+    e2e = None
+    if not args.no_e2e:
+        mh = m0.clone().pin_memory()
+        sim.steps_fixed_host(mh, method, dt, 1)
+        barrier()
+        t0 = time.perf_counter()
+        e0.record()
+        for _ in range(args.steps):
+            sim.steps_fixed_host(mh, method, dt, 1)
+        e1.record()
+        barrier()
+        sec2 = e0.elapsed_time(e1) * 1e-3
+        if dist is not None:
+            t = torch.tensor([sec2], device="cuda", dtype=torch.float64)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            sec2 = float(t.item())
+        nb = mh.numel() * 4
+        e2e = {"value": world * evals / sec2, "unit": UNIT, "h2d_bytes_per_step": nb, "d2h_bytes_per_step": nb,
+               "ms_per_step": sec2 / args.steps * 1e3}
+
+    if rank != 0:
+        return
+
+    # ---- roofline of the dominant kernel ----
+    peak, peak_src = load_peaks()
+    ab = algorithmic_bytes(wl)
+    dom = max((k for k in kt if k != "other" and kt[k][1] > 0), key=lambda k: kt[k][0])
+    dsec, dcnt = kt[dom]
+    ach = ab[dom] / (dsec / dcnt) / 1e9
+    per_pass = {k: {"ms": kt[k][0] / kt[k][1] * 1e3, "alg_GB": ab.get(k, 0) / 1e9,
+                    "GBps": ab.get(k, 0) / (kt[k][0] / kt[k][1]) / 1e9} for k in kt if kt[k][1] > 0}
+    # own float4 copy kernel as a cross-check of the denominator
+    nb = 1 << 30
+    src = torch.empty(nb // 4, dtype=torch.float32, device="cuda").normal_()
+    dst = torch.empty_like(src)
+    csec = sim.copy_bandwidth(src, dst, reps=10)
+    copy_gbs = 2 * nb / csec / 1e9
+    del src, dst
+    t_eval = sec / evals
+    whole = ab["total"] / t_eval / 1e9
+
+    cpu = None
+    if world == 1 and not args.no_cpu_baseline:
+        sample = (128, 128, 64)
+        s_eval, cells = oracle_sample_eval(sample, 5)
+        frac = cells / N
+        cpu = {"value": (1.0 / s_eval) * frac, "unit": UNIT, "cores": host_threads(), "kind": "oracle",
+               "sample": f"{sample[0]}x{sample[1]}x{sample[2]} sub-grid of the workload (1/{round(1 / frac)} of "
+                         f"its cells), median of 5 oracle H_eff+torque evaluations ({s_eval:.2f} s each), scaled "
+                         f"by cell count"}
+
+    out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+           "warmup": max(3, args.warmup), "ms_per_step": sec / args.steps * 1e3, "higher_is_better": True,
+           "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+           "config": {"workload": f"{wl.name}: {wl.grid[0]}x{wl.grid[1]}x{wl.grid[2]} cells, open boundaries, "
+                                  f"vortex + noise state, RK4 dt={dt:g} s, 1 step = 4 fused evaluations",
+                      "l2": "working set > 2 GB >> 126 MB L2 (inputs larger than L2, no flush)",
+                      "parallelism": "replicas" if world > 1 else "single GPU",
+                      "path": "generic" if args.generic else "fast"},
+           "ns_per_cell_per_stage": t_eval / N * 1e9, "ms_per_eval": t_eval * 1e3,
+           "gpu_launches": launches, "clocks": clocks, "setup_s": setup_s,
+           "roofline": {"bound": "hbm", "kernel": dom, "achieved": ach, "peak": peak, "unit": "GB/s",
+                        "frac": ach / peak, "traffic": None, "peak_source": peak_src,
+                        "alg_bytes_per_launch": ab[dom], "launch_ms": dsec / dcnt * 1e3},
+           "whole_eval": {"alg_bytes": ab["total"], "GBps": whole, "frac_of_peak": whole / peak,
+                          "frac_of_8TBps_nominal": whole / 8000.0},
+           "per_pass": per_pass, "own_copy_kernel_GBps": copy_gbs}
+    if e2e is not None:
+        out["e2e"] = e2e
+    if cpu is not None:
+        out["cpu_baseline"] = cpu
+    print(json.dumps(out))
+    sim.close()
+
+
+if __name__ == "__main__":
+    main()

@@ -140,6 +140,12 @@ mm_status mm_step(mm_ctx* ctx, float* m_dev, mm_method method, double* dt_inout,
 mm_status mm_steps_fixed(mm_ctx* ctx, float* m_dev, mm_method method, double dt, int n,
                          double* t_inout, double* max_err_out);
 
+/* mm_steps_fixed_host -- the same as mm_steps_fixed for a state held in HOST memory (pinned memory
+ * gives the full PCIe rate): m_host is copied to the device, advanced n steps and copied back, all on
+ * the context's stream; returns after the copy back.  This is the end-to-end call bench.py times. */
+mm_status mm_steps_fixed_host(mm_ctx* ctx, float* m_host, mm_method method, double dt, int n,
+                              double* t_inout, double* max_err_out);
+
 /* mm_fused_eval -- the unit the throughput metric counts: ONE fused evaluation = demag convolution +
  * local field terms + torque + an RK4-shaped stage combine + max-norm reduction, i.e. stage `stage`
  * (0-based) of `method` applied to m_dev with step dt, writing the stage derivative and the next stage
@@ -178,6 +184,14 @@ mm_status mm_padded_size(const mm_ctx* ctx, int P_out[3], int C_out[3]);
 
 /* mm_launch_count -- number of kernels this context has launched so far (bench.py "gpu_launches"). */
 uint64_t mm_launch_count(const mm_ctx* ctx);
+
+/* mm_kernel_timing / mm_kernel_times -- optional per-pass timing with CUDA events recorded on the
+ * context's stream around every launch (bench.py "roofline").  mm_kernel_timing(ctx, 1) switches it on
+ * and clears the counters; mm_kernel_times synchronises the stream and returns, per pass category
+ * (0 forward x, 1 forward y, 2 last axis + K-hat multiply, 3 inverse y, 4 inverse x + epilogue,
+ * 5 other), the summed device seconds and the number of launches since the last call. */
+mm_status mm_kernel_timing(mm_ctx* ctx, int enable);
+mm_status mm_kernel_times(mm_ctx* ctx, double sec_out[6], uint64_t count_out[6]);
 
 /* mm_set_fast_path -- 1 (default): use the size-specialised register FFT kernels when the grid
  * allows; 0: force the generic shared-memory radix-2/3/4/5 kernels (tests compare the two). */

@@ -12,6 +12,6 @@ struct FastPlan {
 inline bool fast_plan_init(FastPlan& fp, const Geom&, std::string*) { fp.usable = false; return true; }
 inline void fast_plan_destroy(FastPlan&) {}
 inline bool launch_eval_fast(FastPlan&, const Geom&, cudaStream_t, float2*, float2*, const float*,
-                             const EpiParams&, uint64_t*) { return false; }
+                             const EpiParams&, KTimer&) { return false; }
 
 }  // namespace mm

@@ -104,7 +104,7 @@ struct mm_ctx {
     bool has_mat, has_demag;
     mm_material mat;
     std::string err;
-    uint64_t launches;
+    KTimer kt;
     int fast;
     // device
     float* khat;
@@ -114,6 +114,7 @@ struct mm_ctx {
     float* kb[7];
     float* ms[2];
     float* mtmp;
+    float* mhost;     // device copy of a caller's host state (mm_steps_fixed_host)
     unsigned int* maxbits;
     // stepper state
     uint64_t step_index;
@@ -222,39 +223,45 @@ mm_status launch_eval_generic(mm_ctx* c, const EpiParams& ep)
             const int tx = pick_tx(g.Px, 2, 1, &bytes);
             if (!tx) return fail(c, MM_EUNSUPPORTED, "x line too long for the shared-memory tile");
             const int npair = 3 * g.Nz * ((g.Ny + 1) / 2);
+            c->kt.begin(KT_FWD_X);
             k_gen_fwd_x<<<(npair + tx - 1) / tx, 256, bytes, st>>>(g, c->plan[0], ep.m_in, c->specA, tx);
-            c->launches++;
+            c->kt.end(KT_FWD_X);
         }
         if (g.Pz > 1) {
             {   // a2
                 const int tx = pick_tx(g.Py, 2, 1, &bytes);
                 if (!tx) return fail(c, MM_EUNSUPPORTED, "y line too long for the shared-memory tile");
                 dim3 grid((g.Cx + tx - 1) / tx, 3 * g.Nz);
+                c->kt.begin(KT_FWD_Y);
                 k_gen_y<-1><<<grid, 256, bytes, st>>>(g, c->plan[1], c->specA, c->specB, tx);
-                c->launches++;
+                c->kt.end(KT_FWD_Y);
             }
             {   // a3
                 const int tx = pick_tx(g.Pz, 4, 1, &bytes);
                 if (!tx) return fail(c, MM_EUNSUPPORTED, "z line too long for the shared-memory tile");
                 dim3 grid((g.Cx + tx - 1) / tx, g.Py);
+                c->kt.begin(KT_MID);
                 k_gen_mid<<<grid, 256, bytes, st>>>(g, c->plan[2], c->specB, c->khat, 2, tx);
-                c->launches++;
+                c->kt.end(KT_MID);
             }
             {   // a4
                 const int tx = pick_tx(g.Py, 2, 1, &bytes);
                 dim3 grid((g.Cx + tx - 1) / tx, 3 * g.Nz);
+                c->kt.begin(KT_INV_Y);
                 k_gen_y<1><<<grid, 256, bytes, st>>>(g, c->plan[1], c->specB, c->specA, tx);
-                c->launches++;
+                c->kt.end(KT_INV_Y);
             }
         } else if (g.Py > 1) {   // 2D: y forward, multiply, y inverse in one kernel
             const int tx = pick_tx(g.Py, 4, 1, &bytes);
             if (!tx) return fail(c, MM_EUNSUPPORTED, "y line too long for the shared-memory tile");
             dim3 grid((g.Cx + tx - 1) / tx, 1);
+            c->kt.begin(KT_MID);
             k_gen_mid<<<grid, 256, bytes, st>>>(g, c->plan[1], c->specA, c->khat, 1, tx);
-            c->launches++;
+            c->kt.end(KT_MID);
         } else {
+            c->kt.begin(KT_MID);
             k_gen_mul1d<<<(g.Cx + 127) / 128, 128, 0, st>>>(g, c->specA, c->khat);
-            c->launches++;
+            c->kt.end(KT_MID);
         }
     }
     {   // a5-a10
@@ -262,8 +269,9 @@ mm_status launch_eval_generic(mm_ctx* c, const EpiParams& ep)
         if (!tx) return fail(c, MM_EUNSUPPORTED, "x line too long for the shared-memory tile");
         const int npy = (g.Ny + 1) / 2;
         dim3 grid((npy + tx - 1) / tx, g.Nz);
+        c->kt.begin(KT_INV_X);
         k_gen_inv_x<<<grid, 256, bytes, st>>>(g, c->plan[0], c->specA, ep, tx);
-        c->launches++;
+        c->kt.end(KT_INV_X);
     }
     CUDA_TRY(c, cudaGetLastError());
     return MM_OK;
@@ -272,7 +280,7 @@ mm_status launch_eval_generic(mm_ctx* c, const EpiParams& ep)
 mm_status launch_eval(mm_ctx* c, const EpiParams& ep)
 {
     if (c->fast && c->fp.usable) return launch_eval_fast(c->fp, c->g, c->stream, c->specA, c->specB, c->khat, ep,
-                                                          &c->launches)
+                                                          c->kt)
                                             ? MM_OK
                                             : fail(c, MM_ECUDA, std::string("fast path launch: ") +
                                                                     cudaGetErrorString(cudaGetLastError()));
@@ -378,9 +386,10 @@ mm_status enqueue_step(mm_ctx* c, float* m_dev, mm_method method, const Tableau&
     if (tab.fsal && c->k0_valid && c->k0_method == (int)method) {
         // k_1 of this step is the last stage of the previous accepted step: skip the evaluation
         const double dtr = dt * gamma0_of(c) * c->mat.Ms;
+        c->kt.begin(KT_OTHER);
         k_combine<<<148 * 8, 256, 0, c->stream>>>(n, m_dev, c->ms[0], 1, (float)(dtr * tab.A[1][0]), 0.f,
                                                   c->kb[0], c->kb[0]);
-        c->launches++;
+        c->kt.end(KT_OTHER);
         s0 = 1;
     }
     for (int s = s0; s < S; ++s) {
@@ -443,7 +452,9 @@ mm_status mm_create(mm_ctx** out, const int grid[3], const double cellsize[3], c
     for (int a = 0; a < 3; ++a) { c->cell[a] = cellsize[a]; c->pbc[a] = pbc[a]; }
     c->stream = (cudaStream_t)cuda_stream;
     c->has_mat = c->has_demag = false;
-    c->launches = 0;
+    std::memset(&c->kt, 0, sizeof(c->kt));
+    c->kt.stream = c->stream;
+    c->mhost = nullptr;
     c->fast = 1;
     c->khat = nullptr; c->specA = c->specB = nullptr;
     for (int a = 0; a < 3; ++a) c->tw[a] = nullptr;
@@ -513,6 +524,7 @@ mm_status mm_demag_init(mm_ctx* c)
     for (int i = 0; i < 7; ++i) CUDA_TRY(c, cudaMalloc(&c->kb[i], fb));
     for (int i = 0; i < 2; ++i) CUDA_TRY(c, cudaMalloc(&c->ms[i], fb));
     CUDA_TRY(c, cudaMalloc(&c->mtmp, fb));
+    CUDA_TRY(c, cudaMalloc(&c->mhost, fb));
     CUDA_TRY(c, cudaMalloc(&c->maxbits, sizeof(unsigned int)));
     CUDA_TRY(c, cudaMemset(c->maxbits, 0, sizeof(unsigned int)));
     mm_status s;
@@ -649,6 +661,49 @@ mm_status mm_steps_fixed(mm_ctx* c, float* m_dev, mm_method method, double dt, i
     return MM_OK;
 }
 
+mm_status mm_steps_fixed_host(mm_ctx* c, float* m_host, mm_method method, double dt, int n, double* t_inout,
+                              double* max_err_out)
+{
+    mm_status s = check_ready(c);
+    if (s != MM_OK) return s;
+    if (!m_host) return fail(c, MM_EINVAL, "NULL host pointer");
+    const size_t fb = 3 * ncell(c->g) * sizeof(float);
+    CUDA_TRY(c, cudaMemcpyAsync(c->mhost, m_host, fb, cudaMemcpyHostToDevice, c->stream));
+    c->k0_valid = false;
+    s = mm_steps_fixed(c, c->mhost, method, dt, n, t_inout, max_err_out);
+    if (s != MM_OK) return s;
+    CUDA_TRY(c, cudaMemcpyAsync(m_host, c->mhost, fb, cudaMemcpyDeviceToHost, c->stream));
+    CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+    return MM_OK;
+}
+
+mm_status mm_kernel_timing(mm_ctx* c, int enable)
+{
+    if (!c) return MM_EINVAL;
+    cudaStreamSynchronize(c->stream);
+    c->kt.on = enable != 0;
+    for (int k = 0; k < KT_N; ++k) c->kt.nev[k] = 0;
+    return MM_OK;
+}
+
+mm_status mm_kernel_times(mm_ctx* c, double sec_out[6], uint64_t count_out[6])
+{
+    if (!c || !sec_out || !count_out) return MM_EINVAL;
+    CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+    for (int k = 0; k < KT_N; ++k) {
+        double tot = 0.0;
+        for (int i = 0; i + 1 < c->kt.nev[k]; i += 2) {
+            float ms = 0.f;
+            CUDA_TRY(c, cudaEventElapsedTime(&ms, c->kt.ev[k][i], c->kt.ev[k][i + 1]));
+            tot += ms * 1e-3;
+        }
+        sec_out[k] = tot;
+        count_out[k] = (uint64_t)(c->kt.nev[k] / 2);
+        c->kt.nev[k] = 0;
+    }
+    return MM_OK;
+}
+
 mm_status mm_fused_eval(mm_ctx* c, float* m_dev, mm_method method, int stage, double dt, uint64_t step)
 {
     mm_status s = check_ready(c);
@@ -708,7 +763,7 @@ mm_status mm_padded_size(const mm_ctx* c, int P_out[3], int C_out[3])
     return MM_OK;
 }
 
-uint64_t mm_launch_count(const mm_ctx* c) { return c ? c->launches : 0; }
+uint64_t mm_launch_count(const mm_ctx* c) { return c ? c->kt.launches : 0; }
 
 mm_status mm_set_fast_path(mm_ctx* c, int enable)
 {
@@ -735,7 +790,7 @@ mm_status mm_copy_bandwidth(mm_ctx* c, const void* src_dev, void* dst_dev, size_
     CUDA_TRY(c, cudaEventElapsedTime(&ms, e0, e1));
     cudaEventDestroy(e0);
     cudaEventDestroy(e1);
-    c->launches += reps + 1;
+    c->kt.launches += reps + 1;
     *sec_out = (double)ms * 1e-3 / reps;
     return MM_OK;
 }
@@ -753,6 +808,11 @@ void mm_destroy(mm_ctx* c)
     cudaFree(c->ms[0]);
     cudaFree(c->ms[1]);
     cudaFree(c->mtmp);
+    cudaFree(c->mhost);
+    for (int k = 0; k < KT_N; ++k) {
+        for (int i = 0; i < c->kt.cap[k]; ++i) cudaEventDestroy(c->kt.ev[k][i]);
+        delete[] c->kt.ev[k];
+    }
     cudaFree(c->maxbits);
     fast_plan_destroy(c->fp);
     delete c;

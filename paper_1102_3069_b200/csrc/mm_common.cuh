@@ -77,4 +77,30 @@ __device__ __forceinline__ float2 cmuli(float2 a)
     return SGN < 0 ? make_float2(a.y, -a.x) : make_float2(-a.y, a.x);
 }
 
+// ---- optional per-pass timing with CUDA events on the launching stream (bench.py "roofline") ----
+enum KernelCat { KT_FWD_X = 0, KT_FWD_Y = 1, KT_MID = 2, KT_INV_Y = 3, KT_INV_X = 4, KT_OTHER = 5, KT_N = 6 };
+
+struct KTimer {
+    bool on;
+    cudaStream_t stream;
+    uint64_t launches;
+    cudaEvent_t* ev[KT_N];      // start/stop pairs
+    int nev[KT_N], cap[KT_N];
+    void begin(int cat) { if (on) rec(cat); }
+    void end(int cat) { launches++; if (on) rec(cat); }
+    void rec(int cat)
+    {
+        if (nev[cat] == cap[cat]) {
+            const int ncap = cap[cat] ? 2 * cap[cat] : 256;
+            cudaEvent_t* e = new cudaEvent_t[ncap];
+            for (int i = 0; i < nev[cat]; ++i) e[i] = ev[cat][i];
+            for (int i = nev[cat]; i < ncap; ++i) cudaEventCreate(&e[i]);
+            delete[] ev[cat];
+            ev[cat] = e;
+            cap[cat] = ncap;
+        }
+        cudaEventRecord(ev[cat][nev[cat]++], stream);
+    }
+};
+
 }  // namespace mm

@@ -67,6 +67,9 @@ def lib():
             f.argtypes = [vp, vp, vp, C.c_double, C.c_uint64, C.c_double]
         L.mm_step.argtypes = [vp, vp, C.c_int, d3, C.c_double, d3, d3, i3]
         L.mm_steps_fixed.argtypes = [vp, vp, C.c_int, C.c_double, C.c_int, d3, d3]
+        L.mm_steps_fixed_host.argtypes = [vp, vp, C.c_int, C.c_double, C.c_int, d3, d3]
+        L.mm_kernel_timing.argtypes = [vp, C.c_int]
+        L.mm_kernel_times.argtypes = [vp, d3, C.POINTER(C.c_uint64)]
         L.mm_fused_eval.argtypes = [vp, vp, C.c_int, C.c_int, C.c_double, C.c_uint64]
         L.mm_reset_stepper.argtypes = [vp, C.c_uint64]
         L.mm_demag_field.argtypes = [vp, vp, vp]
@@ -185,6 +188,24 @@ class Sim:
         self._chk(self.L.mm_steps_fixed(self.ctx, self._dev(m), METHODS[method], dt, n, C.byref(tv),
                                         C.byref(err)))
         return tv.value, err.value
+
+    def steps_fixed_host(self, m_host, method, dt, n, t=0.0):
+        """m_host: CPU float32 tensor (pinned for full PCIe rate), updated in place."""
+        assert (not m_host.is_cuda) and m_host.dtype == self.torch.float32 and m_host.is_contiguous()
+        assert tuple(m_host.shape) == self.shape
+        tv, err = C.c_double(t), C.c_double(0.0)
+        self._chk(self.L.mm_steps_fixed_host(self.ctx, C.c_void_p(m_host.data_ptr()), METHODS[method], dt, n,
+                                             C.byref(tv), C.byref(err)))
+        return tv.value, err.value
+
+    def kernel_timing(self, enable=True):
+        self._chk(self.L.mm_kernel_timing(self.ctx, int(enable)))
+
+    def kernel_times(self):
+        sec, cnt = (C.c_double * 6)(), (C.c_uint64 * 6)()
+        self._chk(self.L.mm_kernel_times(self.ctx, sec, cnt))
+        names = ("fwd_x", "fwd_y", "mid", "inv_y", "inv_x", "other")
+        return {n: (sec[i], int(cnt[i])) for i, n in enumerate(names)}
 
     def fused_eval(self, m, method, stage, dt, step=0):
         self._chk(self.L.mm_fused_eval(self.ctx, self._dev(m), METHODS[method], stage, dt, step))
