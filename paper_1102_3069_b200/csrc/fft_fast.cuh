@@ -1,17 +1,157 @@
-// fft_fast.cuh -- size-specialised register FFT passes (placeholder: not built yet, generic path only).
+// fft_fast.cuh -- size-specialised register FFT passes for padded lengths 64..1024 (powers of two).
+//
+// Every line transform of length L = T * E is done by T threads that hold E complex values each
+// ("standard form": thread t holds elements t + T j in register j), as two register FFTs (length E,
+// then length T) with ONE exchange through shared memory in between ("1D FFT sets per
+// axis"; the zero-padded half is never loaded and the cropped half never stored).
+// Layouts are those of mm_common.cuh, so each fast pass is interchangeable with its generic
+// counterpart of fft_generic.cuh (mm_set_fast_path takes a bit mask).
+//
+// Product code; shares nothing with oracle/.
 #pragma once
 #include <string>
+#include <vector>
 #include "mm_common.cuh"
+#include "epilogue.cuh"
 
 namespace mm {
+namespace ff {
 
-struct FastPlan {
-    bool usable;
-};
+// cos(2 pi j / 32) and sin(2 pi j / 32) as compile-time constants
+__host__ __device__ constexpr float cos32(int j)
+{
+    j &= 31;
+    if (j > 16) j = 32 - j;
+    bool neg = false;
+    if (j > 8) { j = 16 - j; neg = true; }
+    const float t[9] = { 1.0f, 0.98078528040323044913f, 0.92387953251128675613f, 0.83146961230254523708f,
+                         0.70710678118654752440f, 0.55557023301960222474f, 0.38268343236508977173f,
+                         0.19509032201612826785f, 0.0f };
+    return neg ? -t[j] : t[j];
+}
+__host__ __device__ constexpr float sin32(int j) { return cos32(j - 8); }
 
-inline bool fast_plan_init(FastPlan& fp, const Geom&, std::string*) { fp.usable = false; return true; }
-inline void fast_plan_destroy(FastPlan&) {}
-inline bool launch_eval_fast(FastPlan&, const Geom&, cudaStream_t, float2*, float2*, const float*,
-                             const EpiParams&, KTimer&) { return false; }
+template <int N, int SGN>
+__device__ __forceinline__ void fft_reg(float2 (&v)[N]);
 
+// last level of the decimation-in-time recursion: v[K] = e[K] + w^K o[K], v[K + N/2] = e[K] - w^K o[K]
+template <int N, int SGN, int K>
+__device__ __forceinline__ void dit_combine(float2 (&v)[N], const float2 (&e)[N / 2], const float2 (&o)[N / 2])
+{
+    if constexpr (K < N / 2) {
+        if constexpr (K == 0) {
+            v[0] = cadd(e[0], o[0]);
+            v[N / 2] = csub(e[0], o[0]);
+        } else if constexpr (4 * K == N) {
+            const float2 t = cmuli<SGN>(o[K]);
+            v[K] = cadd(e[K], t);
+            v[K + N / 2] = csub(e[K], t);
+        } else {
+            constexpr float c = cos32(K * (32 / N));
+            constexpr float s = SGN * sin32(K * (32 / N));      // w^K = (c, s)
+            float2 a;
+            a.x = fmaf(c, o[K].x, e[K].x);
+            a.x = fmaf(-s, o[K].y, a.x);
+            a.y = fmaf(c, o[K].y, e[K].y);
+            a.y = fmaf(s, o[K].x, a.y);
+            v[K] = a;
+            v[K + N / 2] = make_float2(fmaf(2.0f, e[K].x, -a.x), fmaf(2.0f, e[K].y, -a.y));
+        }
+        dit_combine<N, SGN, K + 1>(v, e, o);
+    }
+}
+
+// in-place DFT of N = 2, 4, 8, 16, 32 register values, natural order in and out
+template <int N, int SGN>
+__device__ __forceinline__ void fft_reg(float2 (&v)[N])
+{
+    static_assert(N == 2 || N == 4 || N == 8 || N == 16 || N == 32, "register FFT size");
+    if constexpr (N == 2) {
+        const float2 a = v[0], b = v[1];
+        v[0] = cadd(a, b);
+        v[1] = csub(a, b);
+    } else if constexpr (N == 4) {
+        const float2 a = cadd(v[0], v[2]), b = csub(v[0], v[2]);
+        const float2 c = cadd(v[1], v[3]), d = cmuli<SGN>(csub(v[1], v[3]));
+        v[0] = cadd(a, c);
+        v[1] = cadd(b, d);
+        v[2] = csub(a, c);
+        v[3] = csub(b, d);
+    } else {
+        float2 e[N / 2], o[N / 2];
+#pragma unroll
+        for (int i = 0; i < N / 2; ++i) { e[i] = v[2 * i]; o[i] = v[2 * i + 1]; }
+        fft_reg<N / 2, SGN>(e);
+        fft_reg<N / 2, SGN>(o);
+        dit_combine<N, SGN, 0>(v, e, o);
+    }
+}
+
+template <int N, int SGN, int K>
+__device__ __forceinline__ void half_twiddle(float2 (&b)[N / 2])
+{
+    if constexpr (K < N / 2) {
+        if constexpr (4 * K == N) {
+            b[K] = cmuli<SGN>(b[K]);
+        } else if constexpr (K > 0) {
+            constexpr float c = cos32(K * (32 / N));
+            constexpr float s = SGN * sin32(K * (32 / N));
+            const float2 x = b[K];
+            b[K] = make_float2(fmaf(c, x.x, -s * x.y), fmaf(c, x.y, s * x.x));
+        }
+        half_twiddle<N, SGN, K + 1>(b);
+    }
+}
+
+// DFT of N values of which v[N/2..N-1] are zero (not read): one decimation-in-frequency level,
+// X[2k] = FFT_{N/2}(x)[k], X[2k+1] = FFT_{N/2}(x w^n)[k]
+template <int N, int SGN>
+__device__ __forceinline__ void fft_reg_half(float2 (&v)[N])
+{
+    float2 a[N / 2], b[N / 2];
+#pragma unroll
+    for (int i = 0; i < N / 2; ++i) { a[i] = v[i]; b[i] = v[i]; }
+    half_twiddle<N, SGN, 0>(b);
+    fft_reg<N / 2, SGN>(a);
+    fft_reg<N / 2, SGN>(b);
+#pragma unroll
+    for (int i = 0; i < N / 2; ++i) { v[2 * i] = a[i]; v[2 * i + 1] = b[i]; }
+}
+
+struct SyncWarp { __device__ __forceinline__ void operator()() const { __syncwarp(); } };
+struct SyncBlock { __device__ __forceinline__ void operator()() const { __syncthreads(); } };
+
+// Length T*E transform of one line in standard form.  sb: this line's exchange buffer, already
+// offset by the column; element `slot` lives at sb[slot * CS], slot = n1 (E + 1) + k2.
+// tw[k2 * T + t] = exp(-2 pi i t k2 / (T E)).
+template <int T, int E, int SGN, bool IN_HALF, class Sync>
+__device__ __forceinline__ void fft_line(float2 (&v)[E], float2* sb, const int CS, const int t,
+                                         const float2* __restrict__ tw, Sync sync)
+{
+    static_assert(E % T == 0, "E must be a multiple of T");
+    if constexpr (IN_HALF) fft_reg_half<E, SGN>(v);
+    else fft_reg<E, SGN>(v);
+#pragma unroll
+    for (int k2 = 1; k2 < E; ++k2) {
+        float2 w = __ldg(tw + k2 * T + t);
+        if (SGN > 0) w.y = -w.y;
+        v[k2] = cmul(v[k2], w);
+    }
+#pragma unroll
+    for (int k2 = 0; k2 < E; ++k2) sb[(t * (E + 1) + k2) * CS] = v[k2];
+    sync();
+#pragma unroll
+    for (int q = 0; q < E / T; ++q) {
+        float2 u[T];
+#pragma unroll
+        for (int n1 = 0; n1 < T; ++n1) u[n1] = sb[(n1 * (E + 1) + t + T * q) * CS];
+        fft_reg<T, SGN>(u);
+#pragma unroll
+        for (int k1 = 0; k1 < T; ++k1) v[q + (E / T) * k1] = u[k1];
+    }
+}
+
+}  // namespace ff
 }  // namespace mm
+
+#include "fft_fast_kernels.cuh"
