@@ -193,8 +193,10 @@ uint64_t mm_launch_count(const mm_ctx* ctx);
 mm_status mm_kernel_timing(mm_ctx* ctx, int enable);
 mm_status mm_kernel_times(mm_ctx* ctx, double sec_out[6], uint64_t count_out[6]);
 
-/* mm_set_fast_path -- 1 (default): use the size-specialised register FFT kernels when the grid
- * allows; 0: force the generic shared-memory radix-2/3/4/5 kernels (tests compare the two). */
+/* mm_set_fast_path -- bit mask of the passes that may use the size-specialised register FFT kernels
+ * when the grid allows (1 forward x, 2 the y passes, 4 last axis + K-hat multiply, 8 inverse x +
+ * epilogue); a negative value (and the default) enables all, 0 forces the generic shared-memory
+ * radix-2/3/4/5 kernels.  Both families use the same layouts, so tests compare them pass by pass. */
 mm_status mm_set_fast_path(mm_ctx* ctx, int enable);
 
 /* mm_copy_bandwidth -- the library's own float4 grid-stride copy kernel, used by bench.py as the

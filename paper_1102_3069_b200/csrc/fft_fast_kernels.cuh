@@ -1,0 +1,276 @@
+// fft_fast_kernels.cuh -- the five passes of one evaluation built on ff::fft_line (steps a1-a10).
+// Included by fft_fast.cuh.  Product code; shares nothing with oracle/.
+#pragma once
+
+namespace mm {
+namespace ff {
+
+extern __shared__ float2 ff_smem[];
+
+// ---------------------------------------------------------------------------------------------
+// a1: forward x pass, real -> complex.  T threads own one pair of rows (y0, y0+1) packed as
+// real/imaginary part of one complex line; the two spectra are separated with the Hermitian
+// partner k <-> L-k, which in standard form lives in thread T-t, register E-1-j (shuffle).
+// PER = periodic x axis (no zero padding: Nx == L); otherwise Nx == L/2.
+// block = 128 threads = 128/T line slots; persistent grid-stride loop over row pairs.
+// ---------------------------------------------------------------------------------------------
+template <int T, int E, bool PER>
+__global__ void __launch_bounds__(128)
+k_fwd_x(Geom g, const float* __restrict__ m, float2* __restrict__ specA, const float2* __restrict__ tw)
+{
+    constexpr int L = T * E;
+    constexpr int LB = T * (E + 1);            // exchange buffer of one line, float2
+    constexpr int NIN = PER ? E : E / 2;
+    const int t = threadIdx.x % T;
+    const int slot = threadIdx.x / T;
+    const int nslot = 128 / T;
+    float2* sb = ff_smem + slot * LB;
+    const int npy = (g.Ny + 1) >> 1;
+    const int npair = 3 * g.Nz * npy;
+    const unsigned lane = threadIdx.x & 31;
+    const unsigned lbase = lane - t;           // first lane of this line's thread group
+    // the trip count is uniform over the block (full-mask shuffles); an idle slot redoes the last pair
+    for (int pb = blockIdx.x * nslot; pb < npair; pb += gridDim.x * nslot) {
+        const bool act = pb + slot < npair;
+        const int pp = act ? pb + slot : npair - 1;
+        const int cz = pp / npy, y0 = 2 * (pp - cz * npy);
+        const bool two = y0 + 1 < g.Ny;
+        const float* __restrict__ r0 = m + ((size_t)cz * g.Ny + y0) * g.Nx;
+        float2 v[E];
+#pragma unroll
+        for (int j = 0; j < NIN; ++j) {
+            v[j].x = r0[t + T * j];
+            v[j].y = two ? r0[g.Nx + t + T * j] : 0.f;
+        }
+        __syncwarp();                           // previous iteration's reads of sb are done
+        fft_line<T, E, -1, !PER>(v, sb, 1, t, tw, SyncWarp());
+        // separate: A[k] = (Z[k] + conj Z[L-k]) / 2,  B[k] = (Z[k] - conj Z[L-k]) / (2i)
+        float2* __restrict__ o0 = specA + ((size_t)cz * g.Ny + y0) * g.CxS;
+        float2* __restrict__ o1 = o0 + g.CxS;
+        const unsigned src = lbase + ((T - t) % T);
+#pragma unroll
+        for (int j = 0; j < E / 2; ++j) {
+            float2 p;
+            p.x = __shfl_sync(0xffffffffu, v[E - 1 - j].x, src);
+            p.y = __shfl_sync(0xffffffffu, v[E - 1 - j].y, src);
+            if (t == 0) p = v[(E - j) % E];
+            const float2 z = v[j];
+            if (act) o0[t + T * j] = make_float2(0.5f * (z.x + p.x), 0.5f * (z.y - p.y));
+            if (act && two) o1[t + T * j] = make_float2(0.5f * (z.y + p.y), 0.5f * (p.x - z.x));
+        }
+        if (t == 0 && act) {                    // k = L/2 is its own partner
+            o0[L / 2] = make_float2(v[E / 2].x, 0.f);
+            if (two) o1[L / 2] = make_float2(v[E / 2].y, 0.f);
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// a2 / a4: y pass on a tile of 8 adjacent kx columns of one (component, z) plane.
+// forward (SGN = -1): src rows y < Ny (PER: all) -> dst rows ky < Py.  inverse: dst rows y < Ny.
+// thread = (column c = tid & 7, t = tid >> 3); block = 8 T threads; grid = (ceil(Cx/8), 3 Nz).
+// ---------------------------------------------------------------------------------------------
+template <int T, int E, int SGN, bool PER>
+__global__ void __launch_bounds__(8 * T)
+k_y(Geom g, const float2* __restrict__ src, float2* __restrict__ dst, const float2* __restrict__ tw)
+{
+    constexpr bool FWD = SGN < 0;
+    constexpr int NIN = (FWD && !PER) ? E / 2 : E;
+    constexpr int NOUT = (!FWD && !PER) ? E / 2 : E;
+    const int c = threadIdx.x & 7, t = threadIdx.x >> 3;
+    const int kx = blockIdx.x * 8 + c;
+    const bool valid = kx < g.Cx;
+    const int cz = blockIdx.y;
+    const int nin = FWD ? g.Ny : g.Py, nout = FWD ? g.Py : g.Ny;
+    const float2* __restrict__ sp = src + (size_t)cz * nin * g.CxS + kx;
+    float2* __restrict__ dp = dst + (size_t)cz * nout * g.CxS + kx;
+    float2 v[E];
+    if (valid) {
+#pragma unroll
+        for (int j = 0; j < NIN; ++j) v[j] = sp[(size_t)(t + T * j) * g.CxS];
+    } else {
+#pragma unroll
+        for (int j = 0; j < NIN; ++j) v[j] = make_float2(0.f, 0.f);
+    }
+    fft_line<T, E, SGN, (FWD && !PER)>(v, ff_smem + c, 8, t, tw, SyncBlock());
+    if (valid) {
+#pragma unroll
+        for (int j = 0; j < NOUT; ++j) dp[(size_t)(t + T * j) * g.CxS] = v[j];
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// a3: last-axis pass: forward transform of the three components, H^ = K^ M^ with the real
+// symmetric kernel from its octant, inverse transform, crop; in place.
+// Each thread carries one line of all three components (3 E registers), so the 3x3 product
+// needs no exchange.  A block handles 16 kx columns of one line set; when PAIR, blockIdx.y = 2 p + h
+// and the blocks h = 0, 1 take the lines `other` = p and P_other - p, which share the same K^
+// octant entries: they are adjacent in launch order, so the second fetch hits L2.
+//   3D: axis z (stride sz = Py CxS), other = ky.     2D (Nz = 1): axis y, PAIR = false.
+// thread = (c = tid & 15, t = tid >> 4); block = 16 T.
+// ---------------------------------------------------------------------------------------------
+template <int T, int E, bool PER, bool PAIR>
+__global__ void __launch_bounds__(16 * T, (T * E <= 128) ? 3 : 1)
+k_mid(Geom g, float2* __restrict__ spec, const float* __restrict__ khat, const float2* __restrict__ tw,
+      int axis)
+{
+    constexpr int L = T * E;
+    constexpr int LB = T * (E + 1) * 16;       // one component's exchange tile, float2
+    constexpr int NIO = PER ? E : E / 2;
+    const int c = threadIdx.x & 15, t = threadIdx.x >> 4;
+    const int h = PAIR ? (blockIdx.y & 1) : 0;
+    const int kx = blockIdx.x * 16 + c;
+    const bool valid = kx < g.Cx;
+    // line geometry
+    const int Pother = axis == 2 ? g.Py : 1;
+    const int oth_oct = PAIR ? (blockIdx.y >> 1) : blockIdx.y;     // 0 .. Pother/2
+    int other = oth_oct;
+    float so = 1.f;                             // sign of the components odd in `other`
+    if (PAIR && h == 1) {
+        other = (Pother - oth_oct) % Pother;
+        if (other == oth_oct) return;           // self-paired line: done by the h = 0 block
+        so = -1.f;
+    }
+    const bool store = valid;
+    const size_t rstride = axis == 2 ? (size_t)g.Py * g.CxS : (size_t)g.CxS;
+    const size_t cstride = (size_t)g.Nz * (axis == 2 ? g.Py : g.Ny) * g.CxS;
+    float2* __restrict__ base = spec + (axis == 2 ? (size_t)other * g.CxS : 0) + kx;
+    float2 v[3][E];
+#pragma unroll
+    for (int comp = 0; comp < 3; ++comp) {
+        if (valid) {
+#pragma unroll
+            for (int j = 0; j < NIO; ++j) v[comp][j] = base[comp * cstride + (size_t)(t + T * j) * rstride];
+        } else {
+#pragma unroll
+            for (int j = 0; j < NIO; ++j) v[comp][j] = make_float2(0.f, 0.f);
+        }
+    }
+#pragma unroll
+    for (int comp = 0; comp < 3; ++comp)
+        fft_line<T, E, -1, !PER>(v[comp], ff_smem + comp * LB + c, 16, t, tw, SyncBlock());
+    // ---- multiply: the octant index of (k_axis, other) and the signs of the odd components ----
+    {
+        const size_t nC = (size_t)g.Cx * g.Cy * g.Cz;
+        const int kxc = valid ? kx : 0;
+#pragma unroll
+        for (int j = 0; j < E; ++j) {
+            int ka = t + T * j;
+            float sa = 1.f;
+            if (2 * ka > L) { ka = L - ka; sa = -1.f; }
+            const size_t ko = axis == 2 ? ((size_t)ka * g.Cy + oth_oct) * g.Cx + kxc
+                                        : ((size_t)ka) * g.Cx + kxc;
+            const float sy = axis == 2 ? so : sa;
+            const float sz = axis == 2 ? sa : 1.f;
+            const float kxx = __ldg(khat + ko), kyy = __ldg(khat + ko + nC), kzz = __ldg(khat + ko + 2 * nC);
+            const float kxy = sy * __ldg(khat + ko + 3 * nC);
+            const float kxz = sz * __ldg(khat + ko + 4 * nC);
+            const float kyz = sy * sz * __ldg(khat + ko + 5 * nC);
+            const float2 mx = v[0][j], my = v[1][j], mz = v[2][j];
+            v[0][j] = make_float2(kxx * mx.x + kxy * my.x + kxz * mz.x, kxx * mx.y + kxy * my.y + kxz * mz.y);
+            v[1][j] = make_float2(kxy * mx.x + kyy * my.x + kyz * mz.x, kxy * mx.y + kyy * my.y + kyz * mz.y);
+            v[2][j] = make_float2(kxz * mx.x + kyz * my.x + kzz * mz.x, kxz * mx.y + kyz * my.y + kzz * mz.y);
+        }
+    }
+    __syncthreads();                            // all reads of the forward exchange are done
+#pragma unroll
+    for (int comp = 0; comp < 3; ++comp)
+        fft_line<T, E, 1, false>(v[comp], ff_smem + comp * LB + c, 16, t, tw, SyncBlock());
+    if (store) {
+#pragma unroll
+        for (int comp = 0; comp < 3; ++comp)
+#pragma unroll
+            for (int j = 0; j < NIO; ++j) base[comp * cstride + (size_t)(t + T * j) * rstride] = v[comp][j];
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// a5-a10: inverse x pass, complex -> real, and the fused epilogue.  T threads own one pair of rows
+// (y0, y0+1) of one z plane and run the three components one after the other; the magnetostatic
+// field of the pair goes to shared memory as float2 (row y0, row y0+1) per x, and the same threads
+// then do the per-cell tail (exchange, anisotropy, Zeeman, thermal, torque, RK combine, max-norm).
+// ---------------------------------------------------------------------------------------------
+template <int T, int E, bool PER>
+__global__ void __launch_bounds__(128)
+k_inv_x(Geom g, const float2* __restrict__ specA, const float2* __restrict__ tw, EpiParams ep)
+{
+    constexpr int L = T * E;
+    constexpr int LB = T * (E + 1);
+    constexpr int NX = PER ? L : L / 2;        // == g.Nx
+    constexpr int NOUT = PER ? E : E / 2;
+    const int t = threadIdx.x % T;
+    const int slot = threadIdx.x / T;
+    const int nslot = 128 / T;
+    float2* sb = ff_smem + slot * (LB + 3 * NX);
+    float2* hb = sb + LB;                       // [3][NX] float2
+    const int npy = (g.Ny + 1) >> 1;
+    const int npair = g.Nz * npy;
+    const unsigned lane = threadIdx.x & 31;
+    const unsigned lbase = lane - t;
+    const unsigned srcl = lbase + ((T - t) % T);
+    unsigned int red = 0u;
+    for (int pb = blockIdx.x * nslot; pb < npair; pb += gridDim.x * nslot) {
+        const bool act = pb + slot < npair;
+        const int pp = act ? pb + slot : npair - 1;
+        const int z = pp / npy, y0 = 2 * (pp - z * npy);
+        const bool two = y0 + 1 < g.Ny;
+#pragma unroll 1
+        for (int comp = 0; comp < 3; ++comp) {
+            const float2* __restrict__ a0 = specA + (((size_t)comp * g.Nz + z) * g.Ny + y0) * g.CxS;
+            const float2* __restrict__ a1 = a0 + g.CxS;
+            float2 v[E];
+            // Z[k] = A[k] + i B[k] (k <= L/2),  Z[L-k] = conj A[k] + i conj B[k]
+#pragma unroll
+            for (int j = 0; j < E / 2; ++j) {
+                const float2 A = a0[t + T * j];
+                const float2 B = two ? a1[t + T * j] : make_float2(0.f, 0.f);
+                v[j] = make_float2(A.x - B.y, A.y + B.x);
+                v[E - 1 - j] = make_float2(A.x + B.y, B.x - A.y);      // belongs to thread T-t
+            }
+            float2 nyq = make_float2(0.f, 0.f);
+            if (t == 0) {
+                const float2 A = a0[L / 2];
+                const float2 B = two ? a1[L / 2] : make_float2(0.f, 0.f);
+                nyq = make_float2(A.x - B.y, A.y + B.x);
+            }
+            // thread 0 keeps its own mirrored values (k = T j' <-> L - T j' = T (E - j')), shifted by one
+            // register; every other thread takes register E-1-j from thread T-t
+            float2 own[E / 2];
+#pragma unroll
+            for (int j = 0; j < E / 2; ++j) own[j] = v[E - 1 - j];    // own[j] = Zrev of register j
+#pragma unroll
+            for (int j = E / 2; j < E; ++j) {
+                float2 p;
+                p.x = __shfl_sync(0xffffffffu, v[j].x, srcl);
+                p.y = __shfl_sync(0xffffffffu, v[j].y, srcl);
+                v[j] = p;
+            }
+            if (t == 0) {
+                v[E / 2] = nyq;
+#pragma unroll
+                for (int j = E / 2 + 1; j < E; ++j) v[j] = own[E - j];
+            }
+            __syncwarp();
+            fft_line<T, E, 1, false>(v, sb, 1, t, tw, SyncWarp());
+#pragma unroll
+            for (int j = 0; j < NOUT; ++j) hb[comp * NX + t + T * j] = v[j];
+        }
+        __syncwarp();
+        if (act)
+#pragma unroll 2
+        for (int j = 0; j < NOUT; ++j) {
+            const int x = t + T * j;
+            const float2 hx = hb[x], hy = hb[NX + x], hz = hb[2 * NX + x];
+            red = max(red, __float_as_uint(epilogue_cell(g, ep, x, y0, z, hx.x, hy.x, hz.x)) & 0x7fffffffu);
+            if (two)
+                red = max(red, __float_as_uint(epilogue_cell(g, ep, x, y0 + 1, z, hx.y, hy.y, hz.y)) & 0x7fffffffu);
+        }
+        __syncwarp();
+    }
+    if (ep.do_err) block_max_atomic(red, ep.maxbits);
+}
+
+}  // namespace ff
+}  // namespace mm
+
+#include "fft_fast_plan.cuh"

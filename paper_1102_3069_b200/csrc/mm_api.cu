@@ -212,52 +212,77 @@ mm_status set_smem(mm_ctx* c, K kern)
     return MM_OK;
 }
 
-// ---- one evaluation: the five passes, the last one carrying the epilogue `ep` ----
-mm_status launch_eval_generic(mm_ctx* c, const EpiParams& ep)
+// ---- one evaluation: the five passes, the last one carrying the epilogue `ep`.  Each pass runs its
+// size-specialised kernel (fft_fast*.cuh) when one exists for the grid and the bit of c->fast is set,
+// else the generic shared-memory kernel; both use the same layouts. ----
+mm_status launch_eval(mm_ctx* c, const EpiParams& ep)
 {
     const Geom& g = c->g;
     cudaStream_t st = c->stream;
+    const FastPlan& fp = c->fp;
     size_t bytes;
     if (ep.demag) {
         {   // a1
-            const int tx = pick_tx(g.Px, 2, 1, &bytes);
-            if (!tx) return fail(c, MM_EUNSUPPORTED, "x line too long for the shared-memory tile");
-            const int npair = 3 * g.Nz * ((g.Ny + 1) / 2);
             c->kt.begin(KT_FWD_X);
-            k_gen_fwd_x<<<(npair + tx - 1) / tx, 256, bytes, st>>>(g, c->plan[0], ep.m_in, c->specA, tx);
+            if (!((c->fast & FAST_FWD_X) && fast_fwd_x(fp, g, st, ep.m_in, c->specA))) {
+                const int tx = pick_tx(g.Px, 2, 1, &bytes);
+                if (!tx) return fail(c, MM_EUNSUPPORTED, "x line too long for the shared-memory tile");
+                const int npair = 3 * g.Nz * ((g.Ny + 1) / 2);
+                k_gen_fwd_x<<<(npair + tx - 1) / tx, 256, bytes, st>>>(g, c->plan[0], ep.m_in, c->specA, tx);
+            }
             c->kt.end(KT_FWD_X);
         }
         if (g.Pz > 1) {
             {   // a2
-                const int tx = pick_tx(g.Py, 2, 1, &bytes);
-                if (!tx) return fail(c, MM_EUNSUPPORTED, "y line too long for the shared-memory tile");
-                dim3 grid((g.Cx + tx - 1) / tx, 3 * g.Nz);
                 c->kt.begin(KT_FWD_Y);
-                k_gen_y<-1><<<grid, 256, bytes, st>>>(g, c->plan[1], c->specA, c->specB, tx);
+                if (!((c->fast & FAST_Y) && fast_y(fp, g, st, -1, c->specA, c->specB))) {
+                    const int tx = pick_tx(g.Py, 2, 1, &bytes);
+                    if (!tx) return fail(c, MM_EUNSUPPORTED, "y line too long for the shared-memory tile");
+                    dim3 grid((g.Cx + tx - 1) / tx, 3 * g.Nz);
+                    k_gen_y<-1><<<grid, 256, bytes, st>>>(g, c->plan[1], c->specA, c->specB, tx);
+                }
                 c->kt.end(KT_FWD_Y);
             }
             {   // a3
-                const int tx = pick_tx(g.Pz, 4, 1, &bytes);
-                if (!tx) return fail(c, MM_EUNSUPPORTED, "z line too long for the shared-memory tile");
-                dim3 grid((g.Cx + tx - 1) / tx, g.Py);
                 c->kt.begin(KT_MID);
-                k_gen_mid<<<grid, 256, bytes, st>>>(g, c->plan[2], c->specB, c->khat, 2, tx);
+                if (!((c->fast & FAST_MID) && fast_mid3(fp, g, st, c->specB, c->khat))) {
+                    const int tx = pick_tx(g.Pz, 4, 1, &bytes);
+                    if (!tx) return fail(c, MM_EUNSUPPORTED, "z line too long for the shared-memory tile");
+                    dim3 grid((g.Cx + tx - 1) / tx, g.Py);
+                    k_gen_mid<<<grid, 256, bytes, st>>>(g, c->plan[2], c->specB, c->khat, 2, tx);
+                }
                 c->kt.end(KT_MID);
             }
             {   // a4
-                const int tx = pick_tx(g.Py, 2, 1, &bytes);
-                dim3 grid((g.Cx + tx - 1) / tx, 3 * g.Nz);
                 c->kt.begin(KT_INV_Y);
-                k_gen_y<1><<<grid, 256, bytes, st>>>(g, c->plan[1], c->specB, c->specA, tx);
+                if (!((c->fast & FAST_Y) && fast_y(fp, g, st, 1, c->specB, c->specA))) {
+                    const int tx = pick_tx(g.Py, 2, 1, &bytes);
+                    dim3 grid((g.Cx + tx - 1) / tx, 3 * g.Nz);
+                    k_gen_y<1><<<grid, 256, bytes, st>>>(g, c->plan[1], c->specB, c->specA, tx);
+                }
                 c->kt.end(KT_INV_Y);
             }
-        } else if (g.Py > 1) {   // 2D: y forward, multiply, y inverse in one kernel
-            const int tx = pick_tx(g.Py, 4, 1, &bytes);
-            if (!tx) return fail(c, MM_EUNSUPPORTED, "y line too long for the shared-memory tile");
-            dim3 grid((g.Cx + tx - 1) / tx, 1);
-            c->kt.begin(KT_MID);
-            k_gen_mid<<<grid, 256, bytes, st>>>(g, c->plan[1], c->specA, c->khat, 1, tx);
-            c->kt.end(KT_MID);
+        } else if (g.Py > 1) {
+            if ((c->fast & FAST_MID) && fp.ok_mul2) {
+                // 2D: y forward, k-space multiply, y inverse as three launches (the spectra of a 2D grid
+                // are L2-resident, so the extra round trip does not reach HBM)
+                c->kt.begin(KT_FWD_Y);
+                fast_y(fp, g, st, -1, c->specA, c->specB);
+                c->kt.end(KT_FWD_Y);
+                c->kt.begin(KT_MID);
+                fast_mul2(fp, g, st, c->specB, c->khat);
+                c->kt.end(KT_MID);
+                c->kt.begin(KT_INV_Y);
+                fast_y(fp, g, st, 1, c->specB, c->specA);
+                c->kt.end(KT_INV_Y);
+            } else {   // generic: y forward, multiply, y inverse in one kernel
+                const int tx = pick_tx(g.Py, 4, 1, &bytes);
+                if (!tx) return fail(c, MM_EUNSUPPORTED, "y line too long for the shared-memory tile");
+                dim3 grid((g.Cx + tx - 1) / tx, 1);
+                c->kt.begin(KT_MID);
+                k_gen_mid<<<grid, 256, bytes, st>>>(g, c->plan[1], c->specA, c->khat, 1, tx);
+                c->kt.end(KT_MID);
+            }
         } else {
             c->kt.begin(KT_MID);
             k_gen_mul1d<<<(g.Cx + 127) / 128, 128, 0, st>>>(g, c->specA, c->khat);
@@ -265,26 +290,18 @@ mm_status launch_eval_generic(mm_ctx* c, const EpiParams& ep)
         }
     }
     {   // a5-a10
-        const int tx = pick_tx(g.Px, 2, 3, &bytes);
-        if (!tx) return fail(c, MM_EUNSUPPORTED, "x line too long for the shared-memory tile");
-        const int npy = (g.Ny + 1) / 2;
-        dim3 grid((npy + tx - 1) / tx, g.Nz);
         c->kt.begin(KT_INV_X);
-        k_gen_inv_x<<<grid, 256, bytes, st>>>(g, c->plan[0], c->specA, ep, tx);
+        if (!(ep.demag && (c->fast & FAST_INV_X) && fast_inv_x(fp, g, st, c->specA, ep))) {
+            const int tx = pick_tx(g.Px, 2, 3, &bytes);
+            if (!tx) return fail(c, MM_EUNSUPPORTED, "x line too long for the shared-memory tile");
+            const int npy = (g.Ny + 1) / 2;
+            dim3 grid((npy + tx - 1) / tx, g.Nz);
+            k_gen_inv_x<<<grid, 256, bytes, st>>>(g, c->plan[0], c->specA, ep, tx);
+        }
         c->kt.end(KT_INV_X);
     }
     CUDA_TRY(c, cudaGetLastError());
     return MM_OK;
-}
-
-mm_status launch_eval(mm_ctx* c, const EpiParams& ep)
-{
-    if (c->fast && c->fp.usable) return launch_eval_fast(c->fp, c->g, c->stream, c->specA, c->specB, c->khat, ep,
-                                                          c->kt)
-                                            ? MM_OK
-                                            : fail(c, MM_ECUDA, std::string("fast path launch: ") +
-                                                                    cudaGetErrorString(cudaGetLastError()));
-    return launch_eval_generic(c, ep);
 }
 
 mm_status check_ready(mm_ctx* c)
@@ -447,7 +464,7 @@ mm_status mm_create(mm_ctx** out, const int grid[3], const double cellsize[3], c
     g.Nx = grid[0]; g.Ny = grid[1]; g.Nz = grid[2];
     g.Px = P[0]; g.Py = P[1]; g.Pz = P[2];
     g.Cx = P[0] / 2 + 1; g.Cy = P[1] / 2 + 1; g.Cz = P[2] / 2 + 1;
-    g.CxS = (g.Cx + 3) & ~3;     // rows start on 32-byte boundaries
+    g.CxS = (g.Cx + 7) & ~7;     // rows start on 64-byte boundaries
     g.perx = pbc[0] > 0; g.pery = pbc[1] > 0; g.perz = pbc[2] > 0;
     for (int a = 0; a < 3; ++a) { c->cell[a] = cellsize[a]; c->pbc[a] = pbc[a]; }
     c->stream = (cudaStream_t)cuda_stream;
@@ -455,7 +472,7 @@ mm_status mm_create(mm_ctx** out, const int grid[3], const double cellsize[3], c
     std::memset(&c->kt, 0, sizeof(c->kt));
     c->kt.stream = c->stream;
     c->mhost = nullptr;
-    c->fast = 1;
+    c->fast = FAST_ALL;
     c->khat = nullptr; c->specA = c->specB = nullptr;
     for (int a = 0; a < 3; ++a) c->tw[a] = nullptr;
     for (int i = 0; i < 7; ++i) c->kb[i] = nullptr;
@@ -503,7 +520,7 @@ mm_status mm_demag_init(mm_ctx* c)
     const size_t nA = (size_t)3 * g.Nz * g.Ny * g.CxS;
     CUDA_TRY(c, cudaMalloc(&c->specA, nA * sizeof(float2)));
     CUDA_TRY(c, cudaMemset(c->specA, 0, nA * sizeof(float2)));
-    if (g.Pz > 1) {
+    if (g.Py > 1) {
         const size_t nB = (size_t)3 * g.Nz * g.Py * g.CxS;
         CUDA_TRY(c, cudaMalloc(&c->specB, nB * sizeof(float2)));
         CUDA_TRY(c, cudaMemset(c->specB, 0, nB * sizeof(float2)));
@@ -768,7 +785,7 @@ uint64_t mm_launch_count(const mm_ctx* c) { return c ? c->kt.launches : 0; }
 mm_status mm_set_fast_path(mm_ctx* c, int enable)
 {
     if (!c) return MM_EINVAL;
-    c->fast = enable ? 1 : 0;
+    c->fast = enable < 0 ? FAST_ALL : (enable & FAST_ALL);
     return MM_OK;
 }
 

@@ -228,7 +228,7 @@ class Sim:
         return int(self.L.mm_launch_count(self.ctx))
 
     def set_fast_path(self, enable):
-        self._chk(self.L.mm_set_fast_path(self.ctx, int(enable)))
+        self._chk(self.L.mm_set_fast_path(self.ctx, -1 if enable is True else int(enable)))
 
     def copy_bandwidth(self, src, dst, reps=10):
         sec = C.c_double(0.0)

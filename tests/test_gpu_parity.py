@@ -240,3 +240,66 @@ def test_reciprocity_and_positive_energy_on_gpu():
     assert abs(a - b) <= 1e-5 * max(abs(a), abs(b))
     assert float((m1.double() * H1).sum()) < 0.0
     sim.close()
+
+
+# ---- size-specialised register FFT passes (fft_fast*.cuh): padded lengths 64..1024 ----
+FAST_GRIDS = [
+    # grid, cell, pbc                                     padded          passes with a fast kernel
+    ((32, 32, 32), (3e-9, 3e-9, 3e-9), (0, 0, 0)),      # 64^3            all
+    ((64, 32, 64), (3e-9, 4e-9, 2e-9), (0, 0, 0)),      # 128 x 64 x 128  all
+    ((128, 64, 6), (3e-9, 3e-9, 3e-9), (0, 0, 0)),      # 256 x 128 x 12  x, y fast; z generic
+    ((256, 64, 1), (3.90625e-9, 3.90625e-9, 4e-9), (0, 0, 0)),   # config 2 shape: 512 x 128, 2D
+    ((512, 45, 3), (3e-9, 3e-9, 3e-9), (0, 0, 0)),      # 1024 along x, odd Ny (ragged pair), generic y/z
+    ((16, 512, 1), (3e-9, 3e-9, 3e-9), (0, 0, 0)),      # 1024 along y, 2D
+    ((64, 128, 1), (4e-9, 4e-9, 2e-9), (2, 2, 0)),      # periodic film: no padding in x, y
+    ((64, 32, 64), (3e-9, 3e-9, 3e-9), (1, 0, 1)),      # periodic x, z; open y
+    ((36, 32, 128), (3e-9, 3e-9, 3e-9), (0, 0, 0)),     # x generic (72), y 64, z 256; ragged kx tiles
+]
+
+
+@pytest.mark.parametrize("grid,cell,pbc", FAST_GRIDS)
+def test_fast_passes_match_generic_pass_by_pass(grid, cell, pbc):
+    """Both kernel families use the same layouts: switch the fast kernels on one pass at a time."""
+    wl = util.small(grid, cell, pbc, j=(1e12, -5e11, 2e11), P=0.5, xi=0.04)
+    m = wlm.initial_m(wl)
+    sim = util.gpu_sim(wl, fast=0)
+    md = util.to_dev(m)
+    Hg = sim.demag_field(md).double()
+    Tg = sim.torque(md).double()
+    sH, sT = float(Hg.abs().max()), float(Tg.abs().max())
+    for mask in (1, 2, 4, 8, 15):
+        sim.set_fast_path(mask)
+        eh = float((sim.demag_field(md).double() - Hg).abs().max()) / sH
+        et = float((sim.torque(md).double() - Tg).abs().max()) / sT
+        assert eh <= 2e-6 and et <= 2e-6, (mask, eh, et)
+    sim.close()
+
+
+@pytest.mark.parametrize("grid,cell,pbc", FAST_GRIDS[:4] + FAST_GRIDS[6:8])
+def test_fast_path_matches_oracle(grid, cell, pbc):
+    wl = util.small(grid, cell, pbc, T=300.0, seed=77, j=(1e12, -5e11, 2e11), P=0.5, xi=0.04)
+    m = wlm.initial_m(wl)
+    m64 = m.astype(np.float64)
+    pb = util.oracle_problem(wl)
+    sim = util.gpu_sim(wl)
+    md = util.to_dev(m)
+    ref = pb.demag_field(m64)
+    _cmp(sim.demag_field(md), ref, TOL_H)
+    _cmp(sim.heff(md, step=3, dt_thermal=5e-14), pb.heff(m64, 3, 5e-14), TOL_H)
+    _cmp(sim.torque(md, step=3, dt_thermal=5e-14), pb.torque(m64, 3, 5e-14), TOL_H)
+    sim.close()
+
+
+def test_fast_path_rk4_and_rkdp_steps_match_generic():
+    wl = util.small((64, 32, 64), (3e-9, 3e-9, 3e-9), init="xnoise", alpha=0.1)
+    m = wlm.initial_m(wl)
+    out = {}
+    for fast in (0, 15):
+        sim = util.gpu_sim(wl, fast=fast)
+        md = util.to_dev(m)
+        sim.steps_fixed(md, "rk4", 5e-14, 5)
+        _, err = sim.steps_fixed(md, "rkdp", 5e-14, 3)
+        out[fast] = (md.double().cpu().numpy(), err)
+        sim.close()
+    assert np.abs(out[0][0] - out[15][0]).max() <= 1e-5
+    assert abs(out[0][1] - out[15][1]) <= 0.02 * out[0][1] + 1e-9
