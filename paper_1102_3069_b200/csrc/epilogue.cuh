@@ -61,8 +61,88 @@ __device__ __forceinline__ void cross3(const float a[3], const float b[3], float
     c[2] = a[0] * b[1] - a[1] * b[0];
 }
 
-// One cell.  hms = magnetostatic field in units of Ms.  Returns the value to be max-reduced
-// (error norm or |dm/dtau|), 0 when no reduction is asked for.
+// Tail of one cell once its neighbours are known: m = the cell, h = H_ms + H_ex (units of Ms),
+// D = (b_j j.grad) m in reduced units.  Adds anisotropy, Zeeman and thermal fields, forms the torque,
+// does the Runge-Kutta stage combine.  All loads come before all stores.  Returns the value to be
+// max-reduced (error norm or |dm/dtau|), 0 when no reduction is asked for.
+__device__ __forceinline__ float epilogue_finish(const EpiParams& p, size_t idx, size_t n, const float (&m)[3],
+                                                 float (&h)[3], const float (&D)[3])
+{
+    // ---- anisotropy (Eq. (4), reading A5), Zeeman ----
+    {
+        const float mu = m[0] * p.u[0] + m[1] * p.u[1] + m[2] * p.u[2];
+        const float s = p.kan * mu;
+#pragma unroll
+        for (int c = 0; c < 3; ++c) h[c] += s * p.u[c] + p.hext[c];
+    }
+    // ---- thermal field (Eq. (6), reading A6) ----
+    if (p.thermal) {
+        float eta[3];
+        thermal_eta(p, (uint64_t)idx, eta);
+#pragma unroll
+        for (int c = 0; c < 3; ++c) h[c] += p.sig_th * eta[c];
+    }
+    if (p.mode == EPI_HEFF) {
+#pragma unroll
+        for (int c = 0; c < 3; ++c) p.out[idx + c * n] = p.out_scale * h[c];
+        return 0.f;
+    }
+    // ---- torque, Eq. (1): dm/dtau = -1/(1+alpha^2) [ m x h + alpha m x (m x h) ] ----
+    float mxh[3], mxmxh[3], k[3];
+    cross3(m, h, mxh);
+    cross3(m, mxh, mxmxh);
+#pragma unroll
+    for (int c = 0; c < 3; ++c) k[c] = -p.inv1pa2 * (mxh[c] + p.alpha * mxmxh[c]);
+    if (p.stt) {   // Eq. (7): - c_ad m x (m x D) - c_nad m x D
+        float mxD[3], mxmxD[3];
+        cross3(m, D, mxD);
+        cross3(m, mxD, mxmxD);
+#pragma unroll
+        for (int c = 0; c < 3; ++c) k[c] -= p.c_ad * mxmxD[c] + p.c_nad * mxD[c];
+    }
+    if (p.mode == EPI_TORQUE) {
+#pragma unroll
+        for (int c = 0; c < 3; ++c) p.out[idx + c * n] = p.out_scale * k[c];
+        return 0.f;
+    }
+    // ---- Runge-Kutta stage combine (PAPER.md:123-141) ----
+    float r[3] = { 0.f, 0.f, 0.f };
+    if (p.m_out) {
+        float acc[3] = { p.a_self * k[0], p.a_self * k[1], p.a_self * k[2] };
+        for (int j = 0; j < p.na; ++j) {
+            const float* __restrict__ kj = p.ka[j];
+#pragma unroll
+            for (int c = 0; c < 3; ++c) acc[c] += p.a[j] * kj[idx + c * n];
+        }
+        const float* __restrict__ mn = p.m_n;
+        r[0] = mn[idx] + acc[0]; r[1] = mn[idx + n] + acc[1]; r[2] = mn[idx + 2 * n] + acc[2];
+        if (p.normalise) {
+            const float s = rsqrtf(r[0] * r[0] + r[1] * r[1] + r[2] * r[2]);
+            r[0] *= s; r[1] *= s; r[2] *= s;
+        }
+    }
+    float red = 0.f;
+    if (p.do_err) {
+        float e[3] = { p.e_self * k[0], p.e_self * k[1], p.e_self * k[2] };
+        for (int j = 0; j < p.ne; ++j) {
+            const float* __restrict__ kj = p.ke[j];
+#pragma unroll
+            for (int c = 0; c < 3; ++c) e[c] += p.e[j] * kj[idx + c * n];
+        }
+        red = sqrtf(e[0] * e[0] + e[1] * e[1] + e[2] * e[2]);
+    }
+    if (p.k_out) {
+#pragma unroll
+        for (int c = 0; c < 3; ++c) p.k_out[idx + c * n] = k[c];
+    }
+    if (p.m_out) {
+#pragma unroll
+        for (int c = 0; c < 3; ++c) p.m_out[idx + c * n] = r[c];
+    }
+    return red;
+}
+
+// One cell.  hms = magnetostatic field in units of Ms.  Returns the value to be max-reduced.
 __device__ __forceinline__ float epilogue_cell(const Geom& g, const EpiParams& p, int x, int y, int z,
                                                float hx, float hy, float hz)
 {
@@ -105,75 +185,97 @@ __device__ __forceinline__ float epilogue_cell(const Geom& g, const EpiParams& p
             }
         }
     }
-    // ---- anisotropy (Eq. (4), reading A5), Zeeman ----
-    {
-        const float mu = m[0] * p.u[0] + m[1] * p.u[1] + m[2] * p.u[2];
-        const float s = p.kan * mu;
+    return epilogue_finish(p, idx, n, m, h, D);
+}
+
+// ---- two vertically adjacent cells (x, y0) and (x, y0 + 1) at once: the inverse x pass owns row
+// pairs.  PairNbr holds every m value the two cells need (12 positions x 3 components); it is loaded
+// one x ahead of its use so that the loads of the next pair are in flight during the arithmetic
+// and stores of the current one. ----
+struct PairNbr {
+    float col[4][3];     // rows y0-1, y0, y0+1, y0+2 at x (missing row -> the cell's own row)
+    float xm[2][3], xp[2][3], zm[2][3], zp[2][3];
+};
+
+struct PairGeom {        // per row pair, uniform over x
+    size_t n;            // cells per component
+    size_t row[4];       // start of rows y0-1 .. y0+2 in plane z (clamped / wrapped)
+    size_t rzm[2], rzp[2];   // start of rows y0, y0+1 in planes z-1, z+1 (clamped / wrapped)
+};
+
+__device__ __forceinline__ PairGeom pair_geom(const Geom& g, int y0, int z, bool two)
+{
+    PairGeom q;
+    const size_t plane = (size_t)g.Ny * g.Nx;
+    q.n = plane * g.Nz;
+    const int y1 = two ? y0 + 1 : y0;
+    const int ym = y0 > 0 ? y0 - 1 : (g.pery ? g.Ny - 1 : y0);
+    int yA = y0 + 1, yB = y0 + 2;                 // + neighbours of the two cells
+    if (yA >= g.Ny) yA = g.pery ? yA - g.Ny : y0;
+    if (yB >= g.Ny) yB = g.pery ? yB - g.Ny : y1;
+    const int zm = z > 0 ? z - 1 : (g.perz ? g.Nz - 1 : z);
+    const int zp = z + 1 < g.Nz ? z + 1 : (g.perz ? 0 : z);
+    const size_t zb = (size_t)z * plane;
+    q.row[0] = zb + (size_t)ym * g.Nx;
+    q.row[1] = zb + (size_t)y0 * g.Nx;
+    q.row[2] = zb + (size_t)yA * g.Nx;            // == row y0+1 when it exists
+    q.row[3] = zb + (size_t)yB * g.Nx;
+    q.rzm[0] = (size_t)zm * plane + (size_t)y0 * g.Nx;
+    q.rzm[1] = (size_t)zm * plane + (size_t)y1 * g.Nx;
+    q.rzp[0] = (size_t)zp * plane + (size_t)y0 * g.Nx;
+    q.rzp[1] = (size_t)zp * plane + (size_t)y1 * g.Nx;
+    return q;
+}
+
+__device__ __forceinline__ void pair_load(const Geom& g, const float* __restrict__ mi, const PairGeom& q, int x,
+                                          bool two, PairNbr& v)
+{
+    const int xl = x > 0 ? x - 1 : (g.perx ? g.Nx - 1 : x);
+    const int xr = x + 1 < g.Nx ? x + 1 : (g.perx ? 0 : x);
+    const size_t r1 = two ? q.row[1] + g.Nx : q.row[1];     // the pair's second row (or the first again)
 #pragma unroll
-        for (int c = 0; c < 3; ++c) h[c] += s * p.u[c] + p.hext[c];
+    for (int c = 0; c < 3; ++c) {
+        const float* __restrict__ mc = mi + c * q.n;
+        v.col[0][c] = mc[q.row[0] + x];
+        v.col[1][c] = mc[q.row[1] + x];
+        v.col[2][c] = mc[q.row[2] + x];
+        v.col[3][c] = mc[q.row[3] + x];
+        v.xm[0][c] = mc[q.row[1] + xl];
+        v.xp[0][c] = mc[q.row[1] + xr];
+        v.xm[1][c] = mc[r1 + xl];
+        v.xp[1][c] = mc[r1 + xr];
+        v.zm[0][c] = mc[q.rzm[0] + x];
+        v.zm[1][c] = mc[q.rzm[1] + x];
+        v.zp[0][c] = mc[q.rzp[0] + x];
+        v.zp[1][c] = mc[q.rzp[1] + x];
     }
-    // ---- thermal field (Eq. (6), reading A6) ----
-    if (p.thermal) {
-        float eta[3];
-        thermal_eta(p, (uint64_t)idx, eta);
+}
+
+// which = 0: cell (x, y0); which = 1: cell (x, y0 + 1).  hms = magnetostatic field in units of Ms.
+__device__ __forceinline__ float pair_cell(const EpiParams& p, const PairGeom& q, const PairNbr& v, int which,
+                                           int x, int Nx, float hx, float hy, float hz)
+{
+    const size_t idx = (which ? q.row[1] + Nx : q.row[1]) + x;
+    float h[3] = { hx, hy, hz };
+    if (p.mode == EPI_HMS) {
 #pragma unroll
-        for (int c = 0; c < 3; ++c) h[c] += p.sig_th * eta[c];
-    }
-    if (p.mode == EPI_HEFF) {
-#pragma unroll
-        for (int c = 0; c < 3; ++c) p.out[idx + c * n] = p.out_scale * h[c];
+        for (int c = 0; c < 3; ++c) p.out[idx + c * q.n] = p.out_scale * h[c];
         return 0.f;
     }
-    // ---- torque, Eq. (1): dm/dtau = -1/(1+alpha^2) [ m x h + alpha m x (m x h) ] ----
-    float mxh[3], mxmxh[3], k[3];
-    cross3(m, h, mxh);
-    cross3(m, mxh, mxmxh);
+    float m[3], D[3];
 #pragma unroll
-    for (int c = 0; c < 3; ++c) k[c] = -p.inv1pa2 * (mxh[c] + p.alpha * mxmxh[c]);
-    if (p.stt) {   // Eq. (7): - c_ad m x (m x D) - c_nad m x D
-        float mxD[3], mxmxD[3];
-        cross3(m, D, mxD);
-        cross3(m, mxD, mxmxD);
-#pragma unroll
-        for (int c = 0; c < 3; ++c) k[c] -= p.c_ad * mxmxD[c] + p.c_nad * mxD[c];
+    for (int c = 0; c < 3; ++c) {
+        const float mc = v.col[1 + which][c];
+        m[c] = mc;
+        const float xp = v.xp[which][c], xm = v.xm[which][c];
+        const float yp = v.col[2 + which][c], ym = v.col[which][c];
+        const float zp = v.zp[which][c], zm = v.zm[which][c];
+        h[c] += p.wex[0] * ((xp - mc) + (xm - mc));
+        h[c] += p.wex[1] * ((yp - mc) + (ym - mc));
+        h[c] += p.wex[2] * ((zp - mc) + (zm - mc));
+        D[c] = p.cj[0] * (xp - xm) + p.cj[1] * (yp - ym) + p.cj[2] * (zp - zm);
     }
-    if (p.mode == EPI_TORQUE) {
-#pragma unroll
-        for (int c = 0; c < 3; ++c) p.out[idx + c * n] = p.out_scale * k[c];
-        return 0.f;
-    }
-    // ---- Runge-Kutta stage combine (PAPER.md:123-141) ----
-    if (p.k_out) {
-#pragma unroll
-        for (int c = 0; c < 3; ++c) p.k_out[idx + c * n] = k[c];
-    }
-    if (p.m_out) {
-        float acc[3] = { p.a_self * k[0], p.a_self * k[1], p.a_self * k[2] };
-        for (int j = 0; j < p.na; ++j) {
-            const float* __restrict__ kj = p.ka[j];
-#pragma unroll
-            for (int c = 0; c < 3; ++c) acc[c] += p.a[j] * kj[idx + c * n];
-        }
-        const float* __restrict__ mn = p.m_n;
-        float r[3] = { mn[idx] + acc[0], mn[idx + n] + acc[1], mn[idx + 2 * n] + acc[2] };
-        if (p.normalise) {
-            const float s = rsqrtf(r[0] * r[0] + r[1] * r[1] + r[2] * r[2]);
-            r[0] *= s; r[1] *= s; r[2] *= s;
-        }
-#pragma unroll
-        for (int c = 0; c < 3; ++c) p.m_out[idx + c * n] = r[c];
-    }
-    float red = 0.f;
-    if (p.do_err) {
-        float e[3] = { p.e_self * k[0], p.e_self * k[1], p.e_self * k[2] };
-        for (int j = 0; j < p.ne; ++j) {
-            const float* __restrict__ kj = p.ke[j];
-#pragma unroll
-            for (int c = 0; c < 3; ++c) e[c] += p.e[j] * kj[idx + c * n];
-        }
-        red = sqrtf(e[0] * e[0] + e[1] * e[1] + e[2] * e[2]);
-    }
-    return red;
+    return epilogue_finish(p, idx, q.n, m, h, D);
 }
 
 // Block-wide max of non-negative floats (NaN wins), one atomicMax per block (step a10).

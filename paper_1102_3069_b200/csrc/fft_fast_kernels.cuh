@@ -201,8 +201,8 @@ k_inv_x(Geom g, const float2* __restrict__ specA, const float2* __restrict__ tw,
     const int t = threadIdx.x % T;
     const int slot = threadIdx.x / T;
     const int nslot = 128 / T;
-    float2* sb = ff_smem + slot * (LB + 3 * NX);
-    float2* hb = sb + LB;                       // [3][NX] float2
+    float2* sb = ff_smem + slot * (LB + 2 * NX);
+    float2* hb = sb + LB;                       // [2][NX] float2: components x, y (z reuses sb)
     const int npy = (g.Ny + 1) >> 1;
     const int npair = g.Nz * npy;
     const unsigned lane = threadIdx.x & 31;
@@ -252,18 +252,40 @@ k_inv_x(Geom g, const float2* __restrict__ specA, const float2* __restrict__ tw,
             }
             __syncwarp();
             fft_line<T, E, 1, false>(v, sb, 1, t, tw, SyncWarp());
+            if (comp < 2) {
 #pragma unroll
-            for (int j = 0; j < NOUT; ++j) hb[comp * NX + t + T * j] = v[j];
+                for (int j = 0; j < NOUT; ++j) hb[comp * NX + t + T * j] = v[j];
+            } else {
+                __syncwarp();                   // the exchange buffer is free: it takes the z component
+#pragma unroll
+                for (int j = 0; j < NOUT; ++j) sb[t + T * j] = v[j];
+            }
         }
         __syncwarp();
-        if (act)
-#pragma unroll 2
-        for (int j = 0; j < NOUT; ++j) {
-            const int x = t + T * j;
-            const float2 hx = hb[x], hy = hb[NX + x], hz = hb[2 * NX + x];
-            red = max(red, __float_as_uint(epilogue_cell(g, ep, x, y0, z, hx.x, hy.x, hz.x)) & 0x7fffffffu);
-            if (two)
-                red = max(red, __float_as_uint(epilogue_cell(g, ep, x, y0 + 1, z, hx.y, hy.y, hz.y)) & 0x7fffffffu);
+        if (act) {
+            // per-cell tail, software-pipelined: the neighbour loads of x + T are issued before the
+            // arithmetic and stores of x
+            const PairGeom q = pair_geom(g, y0, z, two);
+            PairNbr na, nb;
+            pair_load(g, ep.m_in, q, t, two, na);
+#pragma unroll 1
+            for (int j = 0; j < NOUT; j += 2) {
+                const int x0 = t + T * j, x1 = x0 + T;
+                pair_load(g, ep.m_in, q, x1, two, nb);
+                {
+                    const float2 hx = hb[x0], hy = hb[NX + x0], hz = sb[x0];
+                    red = max(red, __float_as_uint(pair_cell(ep, q, na, 0, x0, g.Nx, hx.x, hy.x, hz.x)) & 0x7fffffffu);
+                    if (two)
+                        red = max(red, __float_as_uint(pair_cell(ep, q, na, 1, x0, g.Nx, hx.y, hy.y, hz.y)) & 0x7fffffffu);
+                }
+                if (j + 2 < NOUT) pair_load(g, ep.m_in, q, x1 + T, two, na);
+                {
+                    const float2 hx = hb[x1], hy = hb[NX + x1], hz = sb[x1];
+                    red = max(red, __float_as_uint(pair_cell(ep, q, nb, 0, x1, g.Nx, hx.x, hy.x, hz.x)) & 0x7fffffffu);
+                    if (two)
+                        red = max(red, __float_as_uint(pair_cell(ep, q, nb, 1, x1, g.Nx, hx.y, hy.y, hz.y)) & 0x7fffffffu);
+                }
+            }
         }
         __syncwarp();
     }

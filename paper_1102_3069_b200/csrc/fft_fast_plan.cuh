@@ -74,7 +74,7 @@ template <int T, int E, bool PER>
 bool launch_inv_x(const FastPlan& fp, const Geom& g, cudaStream_t st, const float2* specA, const EpiParams& ep)
 {
     constexpr int NX = PER ? T * E : T * E / 2;
-    const size_t bytes = (size_t)(128 / T) * (T * (E + 1) + 3 * NX) * sizeof(float2);
+    const size_t bytes = (size_t)(128 / T) * (T * (E + 1) + 2 * NX) * sizeof(float2);
     static bool once = ensure_smem(k_inv_x<T, E, PER>, bytes);
     if (!once) return false;
     const int nslot = 128 / T;
