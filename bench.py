@@ -177,6 +177,7 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--generic", action="store_true", help="force the generic shared-memory FFT kernels")
+    ap.add_argument("--fast", type=int, default=-1, help="bit mask for mm_set_fast_path (default: all)")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
@@ -202,7 +203,9 @@ def main():
     sim = mm.Sim(wl.grid, wl.cell, wl.pbc, wl.mat)
     setup_s = time.perf_counter() - t0
     if args.generic:
-        sim.set_fast_path(False)
+        sim.set_fast_path(0)
+    elif args.fast >= 0:
+        sim.set_fast_path(args.fast)
     md = m0.cuda()
     dt = wl.dt if wl.method == "rk4" else 5e-14
     method = "rk4"

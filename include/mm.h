@@ -188,14 +188,16 @@ uint64_t mm_launch_count(const mm_ctx* ctx);
 /* mm_kernel_timing / mm_kernel_times -- optional per-pass timing with CUDA events recorded on the
  * context's stream around every launch (bench.py "roofline").  mm_kernel_timing(ctx, 1) switches it on
  * and clears the counters; mm_kernel_times synchronises the stream and returns, per pass category
- * (0 forward x, 1 forward y, 2 last axis + K-hat multiply, 3 inverse y, 4 inverse x + epilogue,
- * 5 other), the summed device seconds and the number of launches since the last call. */
+ * (0 forward x, 1 forward y, 2 last axis + K-hat multiply, 3 inverse y, 4 inverse x (+ epilogue when
+ * fused), 5 other, 6 the per-cell epilogue kernel of the split last pass), the summed device seconds
+ * and the number of launches since the last call. */
 mm_status mm_kernel_timing(mm_ctx* ctx, int enable);
-mm_status mm_kernel_times(mm_ctx* ctx, double sec_out[6], uint64_t count_out[6]);
+mm_status mm_kernel_times(mm_ctx* ctx, double sec_out[7], uint64_t count_out[7]);
 
 /* mm_set_fast_path -- bit mask of the passes that may use the size-specialised register FFT kernels
  * when the grid allows (1 forward x, 2 the y passes, 4 last axis + K-hat multiply, 8 inverse x +
- * epilogue); a negative value (and the default) enables all, 0 forces the generic shared-memory
+ * fused epilogue, 16 the split last pass: inverse x to an H_ms field, then a streaming per-cell
+ * kernel; 16 wins over 8); a negative value (and the default) enables all, 0 forces the generic shared-memory
  * radix-2/3/4/5 kernels.  Both families use the same layouts, so tests compare them pass by pass. */
 mm_status mm_set_fast_path(mm_ctx* ctx, int enable);
 

@@ -61,85 +61,173 @@ __device__ __forceinline__ void cross3(const float a[3], const float b[3], float
     c[2] = a[0] * b[1] - a[1] * b[0];
 }
 
-// Tail of one cell once its neighbours are known: m = the cell, h = H_ms + H_ex (units of Ms),
-// D = (b_j j.grad) m in reduced units.  Adds anisotropy, Zeeman and thermal fields, forms the torque,
-// does the Runge-Kutta stage combine.  All loads come before all stores.  Returns the value to be
-// max-reduced (error norm or |dm/dtau|), 0 when no reduction is asked for.
-__device__ __forceinline__ float epilogue_finish(const EpiParams& p, size_t idx, size_t n, const float (&m)[3],
-                                                 float (&h)[3], const float (&D)[3])
+// V consecutive floats (V = 1 or 4; the address is 16-byte aligned when V = 4)
+template <int V>
+__device__ __forceinline__ void ldv(const float* __restrict__ p, float (&v)[V])
+{
+    if constexpr (V == 4) {
+        const float4 t = *reinterpret_cast<const float4*>(p);
+        v[0] = t.x; v[1] = t.y; v[2] = t.z; v[3] = t.w;
+    } else {
+#pragma unroll
+        for (int u = 0; u < V; ++u) v[u] = p[u];
+    }
+}
+template <int V>
+__device__ __forceinline__ void stv(float* __restrict__ p, const float (&v)[V])
+{
+    if constexpr (V == 4) {
+        *reinterpret_cast<float4*>(p) = make_float4(v[0], v[1], v[2], v[3]);
+    } else {
+#pragma unroll
+        for (int u = 0; u < V; ++u) p[u] = v[u];
+    }
+}
+
+// Tail of V consecutive cells (along x, first index idx) once their neighbours are known:
+// m = the cells, h = H_ms + H_ex (units of Ms), D = (b_j j.grad) m in reduced units, all [3][V].
+// Adds anisotropy, Zeeman and thermal fields, forms the torque, does the Runge-Kutta stage combine.
+// All loads come before all stores.  Returns the value to be max-reduced (error norm or
+// |dm/dtau|), 0 when no reduction is asked for.
+template <int V>
+__device__ __forceinline__ float epilogue_finish_v(const EpiParams& p, size_t idx, size_t n, const float (&m)[3][V],
+                                                   float (&h)[3][V], const float (&D)[3][V])
 {
     // ---- anisotropy (Eq. (4), reading A5), Zeeman ----
-    {
-        const float mu = m[0] * p.u[0] + m[1] * p.u[1] + m[2] * p.u[2];
+#pragma unroll
+    for (int u = 0; u < V; ++u) {
+        const float mu = m[0][u] * p.u[0] + m[1][u] * p.u[1] + m[2][u] * p.u[2];
         const float s = p.kan * mu;
 #pragma unroll
-        for (int c = 0; c < 3; ++c) h[c] += s * p.u[c] + p.hext[c];
+        for (int c = 0; c < 3; ++c) h[c][u] += s * p.u[c] + p.hext[c];
     }
     // ---- thermal field (Eq. (6), reading A6) ----
     if (p.thermal) {
-        float eta[3];
-        thermal_eta(p, (uint64_t)idx, eta);
 #pragma unroll
-        for (int c = 0; c < 3; ++c) h[c] += p.sig_th * eta[c];
+        for (int u = 0; u < V; ++u) {
+            float eta[3];
+            thermal_eta(p, (uint64_t)(idx + u), eta);
+#pragma unroll
+            for (int c = 0; c < 3; ++c) h[c][u] += p.sig_th * eta[c];
+        }
     }
     if (p.mode == EPI_HEFF) {
 #pragma unroll
-        for (int c = 0; c < 3; ++c) p.out[idx + c * n] = p.out_scale * h[c];
+        for (int c = 0; c < 3; ++c) {
+            float o[V];
+#pragma unroll
+            for (int u = 0; u < V; ++u) o[u] = p.out_scale * h[c][u];
+            stv<V>(p.out + idx + c * n, o);
+        }
         return 0.f;
     }
     // ---- torque, Eq. (1): dm/dtau = -1/(1+alpha^2) [ m x h + alpha m x (m x h) ] ----
-    float mxh[3], mxmxh[3], k[3];
-    cross3(m, h, mxh);
-    cross3(m, mxh, mxmxh);
+    float k[3][V];
 #pragma unroll
-    for (int c = 0; c < 3; ++c) k[c] = -p.inv1pa2 * (mxh[c] + p.alpha * mxmxh[c]);
-    if (p.stt) {   // Eq. (7): - c_ad m x (m x D) - c_nad m x D
-        float mxD[3], mxmxD[3];
-        cross3(m, D, mxD);
-        cross3(m, mxD, mxmxD);
+    for (int u = 0; u < V; ++u) {
+        const float mm_[3] = { m[0][u], m[1][u], m[2][u] };
+        const float hh[3] = { h[0][u], h[1][u], h[2][u] };
+        float mxh[3], mxmxh[3];
+        cross3(mm_, hh, mxh);
+        cross3(mm_, mxh, mxmxh);
 #pragma unroll
-        for (int c = 0; c < 3; ++c) k[c] -= p.c_ad * mxmxD[c] + p.c_nad * mxD[c];
+        for (int c = 0; c < 3; ++c) k[c][u] = -p.inv1pa2 * (mxh[c] + p.alpha * mxmxh[c]);
+        if (p.stt) {   // Eq. (7): - c_ad m x (m x D) - c_nad m x D
+            const float DD[3] = { D[0][u], D[1][u], D[2][u] };
+            float mxD[3], mxmxD[3];
+            cross3(mm_, DD, mxD);
+            cross3(mm_, mxD, mxmxD);
+#pragma unroll
+            for (int c = 0; c < 3; ++c) k[c][u] -= p.c_ad * mxmxD[c] + p.c_nad * mxD[c];
+        }
     }
     if (p.mode == EPI_TORQUE) {
 #pragma unroll
-        for (int c = 0; c < 3; ++c) p.out[idx + c * n] = p.out_scale * k[c];
+        for (int c = 0; c < 3; ++c) {
+            float o[V];
+#pragma unroll
+            for (int u = 0; u < V; ++u) o[u] = p.out_scale * k[c][u];
+            stv<V>(p.out + idx + c * n, o);
+        }
         return 0.f;
     }
     // ---- Runge-Kutta stage combine ----
-    float r[3] = { 0.f, 0.f, 0.f };
+    float r[3][V];
     if (p.m_out) {
-        float acc[3] = { p.a_self * k[0], p.a_self * k[1], p.a_self * k[2] };
+        float acc[3][V];
+#pragma unroll
+        for (int c = 0; c < 3; ++c)
+#pragma unroll
+            for (int u = 0; u < V; ++u) acc[c][u] = p.a_self * k[c][u];
         for (int j = 0; j < p.na; ++j) {
             const float* __restrict__ kj = p.ka[j];
+            const float aj = p.a[j];
 #pragma unroll
-            for (int c = 0; c < 3; ++c) acc[c] += p.a[j] * kj[idx + c * n];
+            for (int c = 0; c < 3; ++c) {
+                float t[V];
+                ldv<V>(kj + idx + c * n, t);
+#pragma unroll
+                for (int u = 0; u < V; ++u) acc[c][u] += aj * t[u];
+            }
         }
-        const float* __restrict__ mn = p.m_n;
-        r[0] = mn[idx] + acc[0]; r[1] = mn[idx + n] + acc[1]; r[2] = mn[idx + 2 * n] + acc[2];
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            float t[V];
+            ldv<V>(p.m_n + idx + c * n, t);
+#pragma unroll
+            for (int u = 0; u < V; ++u) r[c][u] = t[u] + acc[c][u];
+        }
         if (p.normalise) {
-            const float s = rsqrtf(r[0] * r[0] + r[1] * r[1] + r[2] * r[2]);
-            r[0] *= s; r[1] *= s; r[2] *= s;
+#pragma unroll
+            for (int u = 0; u < V; ++u) {
+                const float s = rsqrtf(r[0][u] * r[0][u] + r[1][u] * r[1][u] + r[2][u] * r[2][u]);
+                r[0][u] *= s; r[1][u] *= s; r[2][u] *= s;
+            }
         }
     }
     float red = 0.f;
     if (p.do_err) {
-        float e[3] = { p.e_self * k[0], p.e_self * k[1], p.e_self * k[2] };
+        float e[3][V];
+#pragma unroll
+        for (int c = 0; c < 3; ++c)
+#pragma unroll
+            for (int u = 0; u < V; ++u) e[c][u] = p.e_self * k[c][u];
         for (int j = 0; j < p.ne; ++j) {
             const float* __restrict__ kj = p.ke[j];
+            const float ej = p.e[j];
 #pragma unroll
-            for (int c = 0; c < 3; ++c) e[c] += p.e[j] * kj[idx + c * n];
+            for (int c = 0; c < 3; ++c) {
+                float t[V];
+                ldv<V>(kj + idx + c * n, t);
+#pragma unroll
+                for (int u = 0; u < V; ++u) e[c][u] += ej * t[u];
+            }
         }
-        red = sqrtf(e[0] * e[0] + e[1] * e[1] + e[2] * e[2]);
+#pragma unroll
+        for (int u = 0; u < V; ++u) {
+            const float q = sqrtf(e[0][u] * e[0][u] + e[1][u] * e[1][u] + e[2][u] * e[2][u]);
+            // NaN must win the reduction: compare bit patterns of |q|
+            red = __uint_as_float(max(__float_as_uint(red), __float_as_uint(q) & 0x7fffffffu));
+        }
     }
     if (p.k_out) {
 #pragma unroll
-        for (int c = 0; c < 3; ++c) p.k_out[idx + c * n] = k[c];
+        for (int c = 0; c < 3; ++c) stv<V>(p.k_out + idx + c * n, k[c]);
     }
     if (p.m_out) {
 #pragma unroll
-        for (int c = 0; c < 3; ++c) p.m_out[idx + c * n] = r[c];
+        for (int c = 0; c < 3; ++c) stv<V>(p.m_out + idx + c * n, r[c]);
     }
     return red;
+}
+
+__device__ __forceinline__ float epilogue_finish(const EpiParams& p, size_t idx, size_t n, const float (&m)[3],
+                                                 float (&h)[3], const float (&D)[3])
+{
+    const float m1[3][1] = { { m[0] }, { m[1] }, { m[2] } };
+    float h1[3][1] = { { h[0] }, { h[1] }, { h[2] } };
+    const float D1[3][1] = { { D[0] }, { D[1] }, { D[2] } };
+    return epilogue_finish_v<1>(p, idx, n, m1, h1, D1);
 }
 
 // One cell.  hms = magnetostatic field in units of Ms.  Returns the value to be max-reduced.
@@ -295,6 +383,79 @@ __device__ __forceinline__ void block_max_atomic(unsigned int b, unsigned int* t
         for (int o = 16; o > 0; o >>= 1) b = max(b, __shfl_xor_sync(0xffffffffu, b, o));
         if (lane == 0 && b != 0u) atomicMax(target, b);
     }
+}
+
+// ---------------------------------------------------------------------------------------------
+// a6-a10 as a streaming kernel of their own (the "split" variant of the last pass): the inverse x
+// pass has left H_ms (units of Ms) in `hms`, laid out like a field; each thread owns 4 consecutive
+// cells along x (float4 traffic), takes its x neighbours from the adjacent lanes and the y / z
+// neighbours from the rows above and below.  Needs Nx % 4 == 0.  One quad per thread.
+// ---------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256)
+k_epi4(Geom g, const float* __restrict__ hms, EpiParams ep)
+{
+    const int nx4 = g.Nx >> 2;
+    const size_t total = (size_t)nx4 * g.Ny * g.Nz;
+    size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const bool active = i < total;
+    if (!active) i = total - 1;
+    const int x4 = (int)(i % nx4);
+    const size_t yz = i / nx4;
+    const int y = (int)(yz % g.Ny), z = (int)(yz / g.Ny);
+    const int x = x4 << 2;
+    const size_t plane = (size_t)g.Ny * g.Nx;
+    const size_t n = plane * g.Nz;
+    const size_t rowc = (size_t)z * plane + (size_t)y * g.Nx;
+    const size_t idx = rowc + x;
+    const float* __restrict__ mi = ep.m_in;
+    const unsigned lane = threadIdx.x & 31;
+    float m[3][4], h[3][4], D[3][4];
+#pragma unroll
+    for (int c = 0; c < 3; ++c) ldv<4>(mi + idx + c * n, m[c]);
+    // x neighbours of the quad's end cells: adjacent lanes hold them unless the lane is at a warp or row end
+    float xl[3], xr[3];
+    {
+        const bool lsh = lane > 0 && x4 > 0, rsh = lane < 31 && x4 + 1 < nx4;
+        const int xli = x > 0 ? x - 1 : (g.perx ? g.Nx - 1 : x);
+        const int xri = x + 4 < g.Nx ? x + 4 : (g.perx ? 0 : x + 3);
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            const float up = __shfl_up_sync(0xffffffffu, m[c][3], 1);
+            const float dn = __shfl_down_sync(0xffffffffu, m[c][0], 1);
+            xl[c] = lsh ? up : mi[rowc + xli + c * n];
+            xr[c] = rsh ? dn : mi[rowc + xri + c * n];
+        }
+    }
+    unsigned int red = 0u;
+    if (active) {
+        const int ym = y > 0 ? y - 1 : (g.pery ? g.Ny - 1 : y);
+        const int yp = y + 1 < g.Ny ? y + 1 : (g.pery ? 0 : y);
+        const int zm = z > 0 ? z - 1 : (g.perz ? g.Nz - 1 : z);
+        const int zp = z + 1 < g.Nz ? z + 1 : (g.perz ? 0 : z);
+        const size_t iym = (size_t)z * plane + (size_t)ym * g.Nx + x, iyp = (size_t)z * plane + (size_t)yp * g.Nx + x;
+        const size_t izm = (size_t)zm * plane + (size_t)y * g.Nx + x, izp = (size_t)zp * plane + (size_t)y * g.Nx + x;
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            float a[4], b[4], d[4], e[4];
+            ldv<4>(hms + idx + c * n, h[c]);
+            ldv<4>(mi + iym + c * n, a);
+            ldv<4>(mi + iyp + c * n, b);
+            ldv<4>(mi + izm + c * n, d);
+            ldv<4>(mi + izp + c * n, e);
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                const float mc = m[c][u];
+                const float xm = u > 0 ? m[c][u > 0 ? u - 1 : 0] : xl[c];
+                const float xp = u < 3 ? m[c][u < 3 ? u + 1 : 3] : xr[c];
+                h[c][u] += ep.wex[0] * ((xp - mc) + (xm - mc));
+                h[c][u] += ep.wex[1] * ((b[u] - mc) + (a[u] - mc));
+                h[c][u] += ep.wex[2] * ((e[u] - mc) + (d[u] - mc));
+                D[c][u] = ep.cj[0] * (xp - xm) + ep.cj[1] * (b[u] - a[u]) + ep.cj[2] * (e[u] - d[u]);
+            }
+        }
+        red = __float_as_uint(epilogue_finish_v<4>(ep, idx, n, m, h, D)) & 0x7fffffffu;
+    }
+    if (ep.do_err) block_max_atomic(red, ep.maxbits);
 }
 
 }  // namespace mm

@@ -292,6 +292,77 @@ k_inv_x(Geom g, const float2* __restrict__ specA, const float2* __restrict__ tw,
     if (ep.do_err) block_max_atomic(red, ep.maxbits);
 }
 
+// ---------------------------------------------------------------------------------------------
+// a5 on its own (the "split" variant of the last pass): inverse x pass, complex -> real, cropped,
+// scaled, written as a field [3][Nz][Ny][Nx]; k_epi4 then does the per-cell tail.  Same thread
+// layout as k_fwd_x: T threads own one pair of rows of one (component, z).
+// ---------------------------------------------------------------------------------------------
+template <int T, int E, bool PER>
+__global__ void __launch_bounds__(128)
+k_inv_x_h(Geom g, const float2* __restrict__ specA, const float2* __restrict__ tw, float* __restrict__ out,
+          float scale)
+{
+    constexpr int L = T * E;
+    constexpr int LB = T * (E + 1);
+    constexpr int NOUT = PER ? E : E / 2;
+    const int t = threadIdx.x % T;
+    const int slot = threadIdx.x / T;
+    const int nslot = 128 / T;
+    float2* sb = ff_smem + slot * LB;
+    const int npy = (g.Ny + 1) >> 1;
+    const int npair = 3 * g.Nz * npy;
+    const unsigned lane = threadIdx.x & 31;
+    const unsigned lbase = lane - t;
+    const unsigned srcl = lbase + ((T - t) % T);
+    for (int pb = blockIdx.x * nslot; pb < npair; pb += gridDim.x * nslot) {
+        const bool act = pb + slot < npair;
+        const int pp = act ? pb + slot : npair - 1;
+        const int cz = pp / npy, y0 = 2 * (pp - cz * npy);
+        const bool two = y0 + 1 < g.Ny;
+        const float2* __restrict__ a0 = specA + ((size_t)cz * g.Ny + y0) * g.CxS;
+        const float2* __restrict__ a1 = a0 + g.CxS;
+        float2 v[E];
+#pragma unroll
+        for (int j = 0; j < E / 2; ++j) {
+            const float2 A = a0[t + T * j];
+            const float2 B = two ? a1[t + T * j] : make_float2(0.f, 0.f);
+            v[j] = make_float2(A.x - B.y, A.y + B.x);
+            v[E - 1 - j] = make_float2(A.x + B.y, B.x - A.y);
+        }
+        float2 nyq = make_float2(0.f, 0.f);
+        if (t == 0) {
+            const float2 A = a0[L / 2];
+            const float2 B = two ? a1[L / 2] : make_float2(0.f, 0.f);
+            nyq = make_float2(A.x - B.y, A.y + B.x);
+        }
+        float2 own[E / 2];
+#pragma unroll
+        for (int j = 0; j < E / 2; ++j) own[j] = v[E - 1 - j];
+#pragma unroll
+        for (int j = E / 2; j < E; ++j) {
+            float2 p;
+            p.x = __shfl_sync(0xffffffffu, v[j].x, srcl);
+            p.y = __shfl_sync(0xffffffffu, v[j].y, srcl);
+            v[j] = p;
+        }
+        if (t == 0) {
+            v[E / 2] = nyq;
+#pragma unroll
+            for (int j = E / 2 + 1; j < E; ++j) v[j] = own[E - j];
+        }
+        __syncwarp();
+        fft_line<T, E, 1, false>(v, sb, 1, t, tw, SyncWarp());
+        float* __restrict__ o0 = out + ((size_t)cz * g.Ny + y0) * g.Nx;
+        if (act) {
+#pragma unroll
+            for (int j = 0; j < NOUT; ++j) {
+                o0[t + T * j] = scale * v[j].x;
+                if (two) o0[g.Nx + t + T * j] = scale * v[j].y;
+            }
+        }
+    }
+}
+
 }  // namespace ff
 }  // namespace mm
 

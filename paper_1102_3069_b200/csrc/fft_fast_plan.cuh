@@ -4,7 +4,7 @@
 
 namespace mm {
 
-enum FastBits { FAST_FWD_X = 1, FAST_Y = 2, FAST_MID = 4, FAST_INV_X = 8, FAST_ALL = 15 };
+enum FastBits { FAST_FWD_X = 1, FAST_Y = 2, FAST_MID = 4, FAST_INV_X = 8, FAST_SPLIT = 16, FAST_ALL = 31 };
 
 struct FastPlan {
     bool ok_x, ok_y, ok_mid3, ok_mul2;   // which passes have a size-specialised kernel for this grid
@@ -85,6 +85,20 @@ bool launch_inv_x(const FastPlan& fp, const Geom& g, cudaStream_t st, const floa
     return true;
 }
 
+template <int T, int E, bool PER>
+bool launch_inv_x_h(const FastPlan& fp, const Geom& g, cudaStream_t st, const float2* specA, float* out, float scale)
+{
+    const size_t bytes = (size_t)(128 / T) * T * (E + 1) * sizeof(float2);
+    static bool once = ensure_smem(k_inv_x_h<T, E, PER>, bytes);
+    if (!once) return false;
+    const int nslot = 128 / T;
+    const int npair = 3 * g.Nz * ((g.Ny + 1) / 2);
+    const int want = (npair + nslot - 1) / nslot;
+    const int grid = want < fp.nsm * 8 ? want : fp.nsm * 8;
+    k_inv_x_h<T, E, PER><<<grid, 128, bytes, st>>>(g, specA, fp.tw[0], out, scale);
+    return true;
+}
+
 template <int T, int E, int SGN, bool PER>
 bool launch_y(const FastPlan& fp, const Geom& g, cudaStream_t st, const float2* src, float2* dst)
 {
@@ -136,6 +150,19 @@ inline bool fast_inv_x(const FastPlan& fp, const Geom& g, cudaStream_t st, const
     bool r = false;
 #define CALL(T, E) r = g.perx ? ff::launch_inv_x<T, E, true>(fp, g, st, specA, ep) \
                               : ff::launch_inv_x<T, E, false>(fp, g, st, specA, ep)
+    MM_FF_SIZES(g.Px, CALL)
+#undef CALL
+    return r;
+}
+
+// split variant of the last pass, first half: H_ms * scale -> out (a field)
+inline bool fast_inv_x_h(const FastPlan& fp, const Geom& g, cudaStream_t st, const float2* specA, float* out,
+                         float scale)
+{
+    if (!fp.ok_x) return false;
+    bool r = false;
+#define CALL(T, E) r = g.perx ? ff::launch_inv_x_h<T, E, true>(fp, g, st, specA, out, scale) \
+                              : ff::launch_inv_x_h<T, E, false>(fp, g, st, specA, out, scale)
     MM_FF_SIZES(g.Px, CALL)
 #undef CALL
     return r;

@@ -114,6 +114,7 @@ struct mm_ctx {
     float* kb[7];
     float* ms[2];
     float* mtmp;
+    float* hfield;    // H_ms in units of Ms between the two halves of the split last pass
     float* mhost;     // device copy of a caller's host state (mm_steps_fixed_host)
     unsigned int* maxbits;
     // stepper state
@@ -289,7 +290,26 @@ mm_status launch_eval(mm_ctx* c, const EpiParams& ep)
             c->kt.end(KT_MID);
         }
     }
-    {   // a5-a10
+    // a5-a10
+    bool done = false;
+    if (ep.demag && (c->fast & FAST_SPLIT) && fp.ok_x && g.Nx % 4 == 0) {
+        // split variant: inverse x pass -> H_ms field, then the streaming per-cell tail
+        c->kt.begin(KT_INV_X);
+        if (ep.mode == EPI_HMS) {
+            done = fast_inv_x_h(fp, g, st, c->specA, ep.out, ep.out_scale);
+            c->kt.end(KT_INV_X);
+        } else {
+            done = fast_inv_x_h(fp, g, st, c->specA, c->hfield, 1.0f);
+            c->kt.end(KT_INV_X);
+            if (done) {
+                const size_t quads = ncell(g) / 4;
+                c->kt.begin(KT_EPI);
+                k_epi4<<<(unsigned)((quads + 255) / 256), 256, 0, st>>>(g, c->hfield, ep);
+                c->kt.end(KT_EPI);
+            }
+        }
+    }
+    if (!done) {
         c->kt.begin(KT_INV_X);
         if (!(ep.demag && (c->fast & FAST_INV_X) && fast_inv_x(fp, g, st, c->specA, ep))) {
             const int tx = pick_tx(g.Px, 2, 3, &bytes);
@@ -472,6 +492,7 @@ mm_status mm_create(mm_ctx** out, const int grid[3], const double cellsize[3], c
     std::memset(&c->kt, 0, sizeof(c->kt));
     c->kt.stream = c->stream;
     c->mhost = nullptr;
+    c->hfield = nullptr;
     c->fast = FAST_ALL;
     c->khat = nullptr; c->specA = c->specB = nullptr;
     for (int a = 0; a < 3; ++a) c->tw[a] = nullptr;
@@ -542,6 +563,7 @@ mm_status mm_demag_init(mm_ctx* c)
     for (int i = 0; i < 2; ++i) CUDA_TRY(c, cudaMalloc(&c->ms[i], fb));
     CUDA_TRY(c, cudaMalloc(&c->mtmp, fb));
     CUDA_TRY(c, cudaMalloc(&c->mhost, fb));
+    CUDA_TRY(c, cudaMalloc(&c->hfield, fb));
     CUDA_TRY(c, cudaMalloc(&c->maxbits, sizeof(unsigned int)));
     CUDA_TRY(c, cudaMemset(c->maxbits, 0, sizeof(unsigned int)));
     mm_status s;
@@ -703,7 +725,7 @@ mm_status mm_kernel_timing(mm_ctx* c, int enable)
     return MM_OK;
 }
 
-mm_status mm_kernel_times(mm_ctx* c, double sec_out[6], uint64_t count_out[6])
+mm_status mm_kernel_times(mm_ctx* c, double sec_out[7], uint64_t count_out[7])
 {
     if (!c || !sec_out || !count_out) return MM_EINVAL;
     CUDA_TRY(c, cudaStreamSynchronize(c->stream));
@@ -826,6 +848,7 @@ void mm_destroy(mm_ctx* c)
     cudaFree(c->ms[1]);
     cudaFree(c->mtmp);
     cudaFree(c->mhost);
+    cudaFree(c->hfield);
     for (int k = 0; k < KT_N; ++k) {
         for (int i = 0; i < c->kt.cap[k]; ++i) cudaEventDestroy(c->kt.ev[k][i]);
         delete[] c->kt.ev[k];

@@ -78,7 +78,7 @@ __device__ __forceinline__ float2 cmuli(float2 a)
 }
 
 // ---- optional per-pass timing with CUDA events on the launching stream (bench.py "roofline") ----
-enum KernelCat { KT_FWD_X = 0, KT_FWD_Y = 1, KT_MID = 2, KT_INV_Y = 3, KT_INV_X = 4, KT_OTHER = 5, KT_N = 6 };
+enum KernelCat { KT_FWD_X = 0, KT_FWD_Y = 1, KT_MID = 2, KT_INV_Y = 3, KT_INV_X = 4, KT_OTHER = 5, KT_EPI = 6, KT_N = 7 };
 
 struct KTimer {
     bool on;

@@ -202,9 +202,9 @@ class Sim:
         self._chk(self.L.mm_kernel_timing(self.ctx, int(enable)))
 
     def kernel_times(self):
-        sec, cnt = (C.c_double * 6)(), (C.c_uint64 * 6)()
+        sec, cnt = (C.c_double * 7)(), (C.c_uint64 * 7)()
         self._chk(self.L.mm_kernel_times(self.ctx, sec, cnt))
-        names = ("fwd_x", "fwd_y", "mid", "inv_y", "inv_x", "other")
+        names = ("fwd_x", "fwd_y", "mid", "inv_y", "inv_x", "other", "epi")
         return {n: (sec[i], int(cnt[i])) for i, n in enumerate(names)}
 
     def fused_eval(self, m, method, stage, dt, step=0):

@@ -267,7 +267,7 @@ def test_fast_passes_match_generic_pass_by_pass(grid, cell, pbc):
     Hg = sim.demag_field(md).double()
     Tg = sim.torque(md).double()
     sH, sT = float(Hg.abs().max()), float(Tg.abs().max())
-    for mask in (1, 2, 4, 8, 15):
+    for mask in (1, 2, 4, 8, 16, 15, 31):
         sim.set_fast_path(mask)
         eh = float((sim.demag_field(md).double() - Hg).abs().max()) / sH
         et = float((sim.torque(md).double() - Tg).abs().max()) / sT
@@ -294,12 +294,13 @@ def test_fast_path_rk4_and_rkdp_steps_match_generic():
     wl = util.small((64, 32, 64), (3e-9, 3e-9, 3e-9), init="xnoise", alpha=0.1)
     m = wlm.initial_m(wl)
     out = {}
-    for fast in (0, 15):
+    for fast in (0, 15, 31):
         sim = util.gpu_sim(wl, fast=fast)
         md = util.to_dev(m)
         sim.steps_fixed(md, "rk4", 5e-14, 5)
         _, err = sim.steps_fixed(md, "rkdp", 5e-14, 3)
         out[fast] = (md.double().cpu().numpy(), err)
         sim.close()
-    assert np.abs(out[0][0] - out[15][0]).max() <= 1e-5
-    assert abs(out[0][1] - out[15][1]) <= 0.02 * out[0][1] + 1e-9
+    for f in (15, 31):
+        assert np.abs(out[0][0] - out[f][0]).max() <= 1e-5
+        assert abs(out[0][1] - out[f][1]) <= 0.02 * out[0][1] + 1e-9
