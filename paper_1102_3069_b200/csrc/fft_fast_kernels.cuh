@@ -66,28 +66,41 @@ k_fwd_x(Geom g, const float* __restrict__ m, float2* __restrict__ specA, const f
 }
 
 // ---------------------------------------------------------------------------------------------
+// Where the columns of a y / last-axis pass live.  The whole-array mode uses the layouts of
+// mm_common.cuh (row stride CxS); the chunked mode works on `ncol`
+// kx columns starting at kx0, with the y-padded spectrum in a compact chunk buffer [3][Nz][Py][W]
+// that stays in L2 between the forward y pass, the last-axis pass and the inverse y pass.
+// ---------------------------------------------------------------------------------------------
+struct ColTile {
+    int kx0, ncol;                 // first global column, number of valid columns
+    size_t a_row, a_plane;         // specA side: strides in float2 (row y, plane (component, z))
+    size_t b_row, b_plane;         // specB / chunk side
+};
+
+// ---------------------------------------------------------------------------------------------
 // a2 / a4: y pass on a tile of 8 adjacent kx columns of one (component, z) plane.
-// forward (SGN = -1): src rows y < Ny (PER: all) -> dst rows ky < Py.  inverse: dst rows y < Ny.
-// thread = (column c = tid & 7, t = tid >> 3); block = 8 T threads; grid = (ceil(Cx/8), 3 Nz).
+// forward (SGN = -1): specA rows y < Ny (PER: all) -> specB rows ky < Py.  inverse: back, rows y < Ny.
+// `a` and `b` point at column kx0.  thread = (column c = tid & 7, t = tid >> 3); block = 8 T threads;
+// grid = (ceil(ncol/8), 3 Nz).
 // ---------------------------------------------------------------------------------------------
 template <int T, int E, int SGN, bool PER>
 __global__ void __launch_bounds__(8 * T)
-k_y(Geom g, const float2* __restrict__ src, float2* __restrict__ dst, const float2* __restrict__ tw)
+k_y(ColTile ct, float2* __restrict__ a, float2* __restrict__ b, const float2* __restrict__ tw)
 {
     constexpr bool FWD = SGN < 0;
     constexpr int NIN = (FWD && !PER) ? E / 2 : E;
     constexpr int NOUT = (!FWD && !PER) ? E / 2 : E;
     const int c = threadIdx.x & 7, t = threadIdx.x >> 3;
-    const int kx = blockIdx.x * 8 + c;
-    const bool valid = kx < g.Cx;
+    const int col = blockIdx.x * 8 + c;
+    const bool valid = col < ct.ncol;
     const int cz = blockIdx.y;
-    const int nin = FWD ? g.Ny : g.Py, nout = FWD ? g.Py : g.Ny;
-    const float2* __restrict__ sp = src + (size_t)cz * nin * g.CxS + kx;
-    float2* __restrict__ dp = dst + (size_t)cz * nout * g.CxS + kx;
+    const size_t s_row = FWD ? ct.a_row : ct.b_row, d_row = FWD ? ct.b_row : ct.a_row;
+    const float2* __restrict__ sp = (FWD ? a + (size_t)cz * ct.a_plane : b + (size_t)cz * ct.b_plane) + col;
+    float2* __restrict__ dp = (FWD ? b + (size_t)cz * ct.b_plane : a + (size_t)cz * ct.a_plane) + col;
     float2 v[E];
     if (valid) {
 #pragma unroll
-        for (int j = 0; j < NIN; ++j) v[j] = sp[(size_t)(t + T * j) * g.CxS];
+        for (int j = 0; j < NIN; ++j) v[j] = sp[(size_t)(t + T * j) * s_row];
     } else {
 #pragma unroll
         for (int j = 0; j < NIN; ++j) v[j] = make_float2(0.f, 0.f);
@@ -95,7 +108,7 @@ k_y(Geom g, const float2* __restrict__ src, float2* __restrict__ dst, const floa
     fft_line<T, E, SGN, (FWD && !PER)>(v, ff_smem + c, 8, t, tw, SyncBlock());
     if (valid) {
 #pragma unroll
-        for (int j = 0; j < NOUT; ++j) dp[(size_t)(t + T * j) * g.CxS] = v[j];
+        for (int j = 0; j < NOUT; ++j) dp[(size_t)(t + T * j) * d_row] = v[j];
     }
 }
 
@@ -109,18 +122,19 @@ k_y(Geom g, const float2* __restrict__ src, float2* __restrict__ dst, const floa
 //   3D: axis z (stride sz = Py CxS), other = ky.     2D (Nz = 1): axis y, PAIR = false.
 // thread = (c = tid & 15, t = tid >> 4); block = 16 T.
 // ---------------------------------------------------------------------------------------------
-template <int T, int E, bool PER, bool PAIR>
-__global__ void __launch_bounds__(16 * T, (T * E <= 128) ? 3 : 1)
-k_mid(Geom g, float2* __restrict__ spec, const float* __restrict__ khat, const float2* __restrict__ tw,
-      int axis)
+template <int T, int E, bool PER, bool PAIR, int MINB>
+__global__ void __launch_bounds__(16 * T, MINB)
+k_mid(Geom g, ColTile ct, float2* __restrict__ spec, const float* __restrict__ khat,
+      const float2* __restrict__ tw, int axis)
 {
     constexpr int L = T * E;
     constexpr int LB = T * (E + 1) * 16;       // one component's exchange tile, float2
     constexpr int NIO = PER ? E : E / 2;
     const int c = threadIdx.x & 15, t = threadIdx.x >> 4;
     const int h = PAIR ? (blockIdx.y & 1) : 0;
-    const int kx = blockIdx.x * 16 + c;
-    const bool valid = kx < g.Cx;
+    const int col = blockIdx.x * 16 + c;
+    const bool valid = col < ct.ncol;
+    const int kx = ct.kx0 + col;
     // line geometry
     const int Pother = axis == 2 ? g.Py : 1;
     const int oth_oct = PAIR ? (blockIdx.y >> 1) : blockIdx.y;     // 0 .. Pother/2
@@ -132,9 +146,10 @@ k_mid(Geom g, float2* __restrict__ spec, const float* __restrict__ khat, const f
         so = -1.f;
     }
     const bool store = valid;
-    const size_t rstride = axis == 2 ? (size_t)g.Py * g.CxS : (size_t)g.CxS;
-    const size_t cstride = (size_t)g.Nz * (axis == 2 ? g.Py : g.Ny) * g.CxS;
-    float2* __restrict__ base = spec + (axis == 2 ? (size_t)other * g.CxS : 0) + kx;
+    // `spec` points at column kx0; along z consecutive elements of a line are one (z) plane apart
+    const size_t rstride = axis == 2 ? ct.b_plane : ct.b_row;
+    const size_t cstride = (size_t)g.Nz * ct.b_plane;
+    float2* __restrict__ base = spec + (axis == 2 ? (size_t)other * ct.b_row : 0) + col;
     float2 v[3][E];
 #pragma unroll
     for (int comp = 0; comp < 3; ++comp) {
@@ -151,15 +166,15 @@ k_mid(Geom g, float2* __restrict__ spec, const float* __restrict__ khat, const f
         fft_line<T, E, -1, !PER>(v[comp], ff_smem + comp * LB + c, 16, t, tw, SyncBlock());
     // ---- multiply: the octant index of (k_axis, other) and the signs of the odd components ----
     {
-        const size_t nC = (size_t)g.Cx * g.Cy * g.Cz;
+        const size_t nC = (size_t)g.CxK * g.Cy * g.Cz;
         const int kxc = valid ? kx : 0;
 #pragma unroll
         for (int j = 0; j < E; ++j) {
             int ka = t + T * j;
             float sa = 1.f;
             if (2 * ka > L) { ka = L - ka; sa = -1.f; }
-            const size_t ko = axis == 2 ? ((size_t)ka * g.Cy + oth_oct) * g.Cx + kxc
-                                        : ((size_t)ka) * g.Cx + kxc;
+            const size_t ko = axis == 2 ? ((size_t)ka * g.Cy + oth_oct) * g.CxK + kxc
+                                        : ((size_t)ka) * g.CxK + kxc;
             const float sy = axis == 2 ? so : sa;
             const float sz = axis == 2 ? sa : 1.f;
             const float kxx = __ldg(khat + ko), kyy = __ldg(khat + ko + nC), kzz = __ldg(khat + ko + 2 * nC);
@@ -182,6 +197,127 @@ k_mid(Geom g, float2* __restrict__ spec, const float* __restrict__ khat, const f
 #pragma unroll
             for (int j = 0; j < NIO; ++j) base[comp * cstride + (size_t)(t + T * j) * rstride] = v[comp][j];
     }
+}
+
+// ---- cp.async helpers (16-byte copies global -> shared, zero-filled beyond src_bytes) ----
+__device__ __forceinline__ void cp_async16(void* smem, const void* gmem, int src_bytes)
+{
+    const unsigned s = (unsigned)__cvta_generic_to_shared(smem);
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;\n" ::"r"(s), "l"(gmem), "r"(src_bytes) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;\n" ::"n"(N) : "memory"); }
+
+// ---------------------------------------------------------------------------------------------
+// a3, persistent and software-pipelined (3D grids, z axis): same arithmetic as k_mid, but a block
+// loops over work items (16 kx columns x one ky pair {p, Py - p}) and, while it transforms one
+// line set, cp.async already brings in the next one's spectrum tile [3][Nz][16] and, once per pair,
+// the K^ octant tile [6][Cz][16], so neither load latency is exposed and the two lines of a pair
+// share one K^ fetch.  grid = min(items, 2 SMs...); block = 16 T.
+// ---------------------------------------------------------------------------------------------
+template <int T, int E, bool PER>
+__global__ void __launch_bounds__(16 * T, (T * E <= 128) ? 2 : 1)
+k_mid_p(Geom g, ColTile ct, float2* __restrict__ spec, const float* __restrict__ khat,
+        const float2* __restrict__ tw)
+{
+    constexpr int L = T * E;
+    constexpr int LB = T * (E + 1) * 16;       // one component's exchange tile, float2
+    constexpr int NIO = PER ? E : E / 2;
+    constexpr int NZ = PER ? L : L / 2;        // == g.Nz
+    constexpr int CZ = L / 2 + 1;              // == g.Cz
+    constexpr int NT = 16 * T;
+    float2* xb = ff_smem;
+    float2* ib = xb + 3 * LB;                   // [3][NZ][16]
+    float* kb = reinterpret_cast<float*>(ib + 3 * NZ * 16);     // [6][CZ][16]
+    const int tid = threadIdx.x, c = tid & 15, t = tid >> 4;
+    const int ntx = (ct.ncol + 15) >> 4;
+    const int nitem = ntx * (g.Py / 2 + 1);
+    const size_t rstride = ct.b_plane, cstride = (size_t)g.Nz * ct.b_plane;
+    const size_t nCk = (size_t)g.CxK * g.Cy * g.Cz;
+
+    auto issue_in = [&](int bx, int other) {
+        const float2* __restrict__ src0 = spec + (size_t)other * ct.b_row + bx * 16;
+        for (int u = tid; u < 3 * NZ * 8; u += NT) {
+            const int cu = u & 7, r = (u >> 3) % NZ, comp = (u >> 3) / NZ;
+            const int left = ct.ncol - (bx * 16 + 2 * cu);
+            const int nb = left >= 2 ? 16 : (left == 1 ? 8 : 0);
+            const float2* src = nb ? src0 + comp * cstride + (size_t)r * rstride + 2 * cu : spec;
+            cp_async16(ib + (comp * NZ + r) * 16 + 2 * cu, src, nb);
+        }
+    };
+    auto issue_k = [&](int bx, int p) {
+        const int kxb = ct.kx0 + bx * 16;
+        for (int u = tid; u < 6 * CZ * 4; u += NT) {
+            const int cu = u & 3, kz = (u >> 2) % CZ, comp = (u >> 2) / CZ;
+            const int kx = kxb + 4 * cu;
+            const int nb = kx < g.CxK ? 16 : 0;
+            const float* src = nb ? khat + comp * nCk + ((size_t)kz * g.Cy + p) * g.CxK + kx : khat;
+            cp_async16(kb + (comp * CZ + kz) * 16 + 4 * cu, src, nb);
+        }
+    };
+
+    int q = blockIdx.x;
+    if (q < nitem) { issue_k(q % ntx, q / ntx); issue_in(q % ntx, q / ntx); }
+    cp_async_commit();
+    cp_async_commit();                          // (empty) keeps "all but the newest group" == everything needed
+    for (; q < nitem; q += gridDim.x) {
+        const int bx = q % ntx, p = q / ntx;
+        const int mir = (g.Py - p) % g.Py;
+        const int nh = mir == p ? 1 : 2;
+        const int qn = q + gridDim.x;
+        const int col = bx * 16 + c;
+        const bool valid = col < ct.ncol;
+        for (int h = 0; h < nh; ++h) {
+            const int other = h ? mir : p;
+            const float so = h ? -1.f : 1.f;    // sign of the components odd in ky
+            cp_async_wait<1>();
+            __syncthreads();                    // this line set's spectrum tile has landed
+            float2 v[3][E];
+#pragma unroll
+            for (int comp = 0; comp < 3; ++comp)
+#pragma unroll
+                for (int j = 0; j < NIO; ++j) v[comp][j] = ib[(comp * NZ + t + T * j) * 16 + c];
+            __syncthreads();
+            if (h + 1 < nh) issue_in(bx, mir);
+            else if (qn < nitem) issue_in(qn % ntx, qn / ntx);
+            cp_async_commit();
+#pragma unroll
+            for (int comp = 0; comp < 3; ++comp)
+                fft_line<T, E, -1, !PER>(v[comp], xb + comp * LB + c, 16, t, tw, SyncBlock());
+            cp_async_wait<1>();
+            __syncthreads();                    // K^ tile of this pair has landed
+#pragma unroll
+            for (int j = 0; j < E; ++j) {
+                int ka = t + T * j;
+                float sz = 1.f;
+                if (2 * ka > L) { ka = L - ka; sz = -1.f; }
+                const float* kr = kb + ka * 16 + c;
+                const float kxx = kr[0], kyy = kr[CZ * 16], kzz = kr[2 * CZ * 16];
+                const float kxy = so * kr[3 * CZ * 16];
+                const float kxz = sz * kr[4 * CZ * 16];
+                const float kyz = so * sz * kr[5 * CZ * 16];
+                const float2 mx = v[0][j], my = v[1][j], mz = v[2][j];
+                v[0][j] = make_float2(kxx * mx.x + kxy * my.x + kxz * mz.x, kxx * mx.y + kxy * my.y + kxz * mz.y);
+                v[1][j] = make_float2(kxy * mx.x + kyy * my.x + kyz * mz.x, kxy * mx.y + kyy * my.y + kyz * mz.y);
+                v[2][j] = make_float2(kxz * mx.x + kyz * my.x + kzz * mz.x, kxz * mx.y + kyz * my.y + kzz * mz.y);
+            }
+            __syncthreads();                    // K^ tile and the forward exchange are free again
+            if (h + 1 == nh && qn < nitem) issue_k(qn % ntx, qn / ntx);
+            cp_async_commit();
+#pragma unroll
+            for (int comp = 0; comp < 3; ++comp)
+                fft_line<T, E, 1, false>(v[comp], xb + comp * LB + c, 16, t, tw, SyncBlock());
+            if (valid) {
+                float2* __restrict__ base = spec + (size_t)other * ct.b_row + col;
+#pragma unroll
+                for (int comp = 0; comp < 3; ++comp)
+#pragma unroll
+                    for (int j = 0; j < NIO; ++j) base[comp * cstride + (size_t)(t + T * j) * rstride] = v[comp][j];
+            }
+        }
+    }
+    cp_async_wait<0>();
 }
 
 // ---------------------------------------------------------------------------------------------

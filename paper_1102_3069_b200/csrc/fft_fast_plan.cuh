@@ -4,12 +4,16 @@
 
 namespace mm {
 
-enum FastBits { FAST_FWD_X = 1, FAST_Y = 2, FAST_MID = 4, FAST_INV_X = 8, FAST_SPLIT = 16, FAST_ALL = 31 };
+enum FastBits { FAST_FWD_X = 1, FAST_Y = 2, FAST_MID = 4, FAST_INV_X = 8, FAST_SPLIT = 16, FAST_CHUNK = 32, FAST_ALL = 63 };
 
 struct FastPlan {
     bool ok_x, ok_y, ok_mid3, ok_mul2;   // which passes have a size-specialised kernel for this grid
     float2* tw[3];                       // per axis: tw[k2 * T + t] = exp(-2 pi i t k2 / L)
     int nsm;                             // SM count (persistent grids)
+    int mid_pipe;                        // last-axis pass: persistent cp.async-pipelined kernel (env MM_MID_PIPE)
+    int chunk_w, nstream;                // chunked a2-a4: columns per chunk (0 = whole-array passes), streams
+    cudaStream_t stream[4];
+    cudaEvent_t ev_fork, ev_join[4];
 };
 
 namespace ff {
@@ -36,8 +40,8 @@ k_mul2d(Geom g, float2* __restrict__ spec, const float* __restrict__ khat)
     int kyy = ky;
     float sy = 1.f;
     if (2 * kyy > g.Py) { kyy = g.Py - kyy; sy = -1.f; }
-    const size_t nC = (size_t)g.Cx * g.Cy * g.Cz;
-    const size_t ko = (size_t)kyy * g.Cx + kx;
+    const size_t nC = (size_t)g.CxK * g.Cy * g.Cz;
+    const size_t ko = (size_t)kyy * g.CxK + kx;
     const float kxx = __ldg(khat + ko), kyy_ = __ldg(khat + ko + nC), kzz = __ldg(khat + ko + 2 * nC);
     const float kxy = sy * __ldg(khat + ko + 3 * nC), kxz = __ldg(khat + ko + 4 * nC);
     const float kyz = sy * __ldg(khat + ko + 5 * nC);
@@ -100,24 +104,41 @@ bool launch_inv_x_h(const FastPlan& fp, const Geom& g, cudaStream_t st, const fl
 }
 
 template <int T, int E, int SGN, bool PER>
-bool launch_y(const FastPlan& fp, const Geom& g, cudaStream_t st, const float2* src, float2* dst)
+bool launch_y(const FastPlan& fp, const Geom& g, cudaStream_t st, const ColTile& ct, float2* a, float2* b)
 {
     const size_t bytes = (size_t)T * (E + 1) * 8 * sizeof(float2);
     static bool once = ensure_smem(k_y<T, E, SGN, PER>, bytes);
     if (!once) return false;
-    dim3 grid((g.Cx + 7) / 8, 3 * g.Nz);
-    k_y<T, E, SGN, PER><<<grid, 8 * T, bytes, st>>>(g, src, dst, fp.tw[1]);
+    dim3 grid((ct.ncol + 7) / 8, 3 * g.Nz);
+    k_y<T, E, SGN, PER><<<grid, 8 * T, bytes, st>>>(ct, a, b, fp.tw[1]);
     return true;
 }
 
 template <int T, int E, bool PER>
-bool launch_mid3(const FastPlan& fp, const Geom& g, cudaStream_t st, float2* specB, const float* khat)
+bool launch_mid3(const FastPlan& fp, const Geom& g, cudaStream_t st, const ColTile& ct, float2* specB,
+                 const float* khat)
 {
+    if (fp.mid_pipe) {
+        constexpr int L = T * E;
+        constexpr int NZ = PER ? L : L / 2;
+        const size_t pb = (size_t)3 * T * (E + 1) * 16 * sizeof(float2) + (size_t)3 * NZ * 16 * sizeof(float2) +
+                          (size_t)6 * (L / 2 + 1) * 16 * sizeof(float);
+        if (pb <= 227 * 1024) {
+            static bool oncep = ensure_smem(k_mid_p<T, E, PER>, pb);
+            if (!oncep) return false;
+            const int nitem = ((ct.ncol + 15) / 16) * (g.Py / 2 + 1);
+            const int per_sm = (T * E <= 128) ? 2 : 1;
+            const int grid = nitem < fp.nsm * per_sm ? nitem : fp.nsm * per_sm;
+            k_mid_p<T, E, PER><<<grid, 16 * T, pb, st>>>(g, ct, specB, khat, fp.tw[2]);
+            return true;
+        }
+    }
     const size_t bytes = (size_t)3 * T * (E + 1) * 16 * sizeof(float2);
-    static bool once = ensure_smem(k_mid<T, E, PER, true>, bytes);
+    constexpr int MINB = (T * E <= 128) ? 2 : 1;
+    dim3 grid((ct.ncol + 15) / 16, 2 * (g.Py / 2 + 1));
+    static bool once = ensure_smem(k_mid<T, E, PER, true, MINB>, bytes);
     if (!once) return false;
-    dim3 grid((g.Cx + 15) / 16, 2 * (g.Py / 2 + 1));
-    k_mid<T, E, PER, true><<<grid, 16 * T, bytes, st>>>(g, specB, khat, fp.tw[2], 2);
+    k_mid<T, E, PER, true, MINB><<<grid, 16 * T, bytes, st>>>(g, ct, specB, khat, fp.tw[2], 2);
     return true;
 }
 
@@ -168,26 +189,28 @@ inline bool fast_inv_x_h(const FastPlan& fp, const Geom& g, cudaStream_t st, con
     return r;
 }
 
-// sgn < 0: specA rows y < Ny -> specB rows ky < Py; sgn > 0: back
-inline bool fast_y(const FastPlan& fp, const Geom& g, cudaStream_t st, int sgn, const float2* src, float2* dst)
+// sgn < 0: specA rows y < Ny -> specB rows ky < Py; sgn > 0: back.  a, b point at column ct.kx0.
+inline bool fast_y(const FastPlan& fp, const Geom& g, cudaStream_t st, int sgn, const ff::ColTile& ct, float2* a,
+                   float2* b)
 {
     if (!fp.ok_y) return false;
     bool r = false;
-#define CALL(T, E)                                                                              \
-    r = sgn < 0 ? (g.pery ? ff::launch_y<T, E, -1, true>(fp, g, st, src, dst)                   \
-                          : ff::launch_y<T, E, -1, false>(fp, g, st, src, dst))                 \
-                : (g.pery ? ff::launch_y<T, E, 1, true>(fp, g, st, src, dst)                    \
-                          : ff::launch_y<T, E, 1, false>(fp, g, st, src, dst))
+#define CALL(T, E)                                                                         \
+    r = sgn < 0 ? (g.pery ? ff::launch_y<T, E, -1, true>(fp, g, st, ct, a, b)              \
+                          : ff::launch_y<T, E, -1, false>(fp, g, st, ct, a, b))            \
+                : (g.pery ? ff::launch_y<T, E, 1, true>(fp, g, st, ct, a, b)               \
+                          : ff::launch_y<T, E, 1, false>(fp, g, st, ct, a, b))
     MM_FF_SIZES(g.Py, CALL)
 #undef CALL
     return r;
 }
 
-inline bool fast_mid3(const FastPlan& fp, const Geom& g, cudaStream_t st, float2* specB, const float* khat)
+inline bool fast_mid3(const FastPlan& fp, const Geom& g, cudaStream_t st, const ff::ColTile& ct, float2* specB,
+                      const float* khat)
 {
     if (!fp.ok_mid3) return false;
-#define CALL(T, E) return g.perz ? ff::launch_mid3<T, E, true>(fp, g, st, specB, khat) \
-                                 : ff::launch_mid3<T, E, false>(fp, g, st, specB, khat)
+#define CALL(T, E) return g.perz ? ff::launch_mid3<T, E, true>(fp, g, st, ct, specB, khat) \
+                                 : ff::launch_mid3<T, E, false>(fp, g, st, ct, specB, khat)
     switch (g.Pz) {      // three components of a line live in one thread: E <= 16
     case 64: CALL(8, 8);
     case 128: CALL(8, 16);
@@ -196,6 +219,48 @@ inline bool fast_mid3(const FastPlan& fp, const Geom& g, cudaStream_t st, float2
     }
 #undef CALL
     return false;
+}
+
+// the whole-array tile: every column, strides of mm_common.cuh
+inline ff::ColTile whole_tile(const Geom& g)
+{
+    ff::ColTile ct;
+    ct.kx0 = 0; ct.ncol = g.Cx;
+    ct.a_row = g.CxS; ct.a_plane = (size_t)g.Ny * g.CxS;
+    ct.b_row = g.CxS; ct.b_plane = (size_t)g.Py * g.CxS;
+    return ct;
+}
+
+// a2-a4 in chunks of fp.chunk_w kx columns (3D grids): forward y pass into a compact chunk buffer
+// (a slot of specB), last-axis pass in place, inverse y pass back into specA.  A chunk is a few tens
+// of MB, so between the three kernels it stays in the 126 MB L2 and the y-padded spectrum never
+// travels to HBM.  Chunks rotate over fp.nstream streams so that the tail of one kernel overlaps the
+// next chunk.  `st` is the context's stream: forked from and joined back to with events.
+inline bool fast_yzy_chunked(FastPlan& fp, const Geom& g, cudaStream_t st, float2* specA, float2* specB,
+                             const float* khat)
+{
+    if (!(fp.ok_y && fp.ok_mid3 && fp.chunk_w > 0 && fp.nstream > 0)) return false;
+    const int W = fp.chunk_w;
+    const size_t slot = (size_t)3 * g.Nz * g.Py * W;
+    cudaEventRecord(fp.ev_fork, st);
+    for (int s = 0; s < fp.nstream; ++s) cudaStreamWaitEvent(fp.stream[s], fp.ev_fork, 0);
+    int i = 0;
+    for (int kx0 = 0; kx0 < g.Cx; kx0 += W, ++i) {
+        const int s = i % fp.nstream;
+        ff::ColTile ct;
+        ct.kx0 = kx0; ct.ncol = g.Cx - kx0 < W ? g.Cx - kx0 : W;
+        ct.a_row = g.CxS; ct.a_plane = (size_t)g.Ny * g.CxS;
+        ct.b_row = W; ct.b_plane = (size_t)g.Py * W;
+        float2* buf = specB + (size_t)s * slot;
+        if (!fast_y(fp, g, fp.stream[s], -1, ct, specA + kx0, buf)) return false;
+        if (!fast_mid3(fp, g, fp.stream[s], ct, buf, khat)) return false;
+        if (!fast_y(fp, g, fp.stream[s], 1, ct, specA + kx0, buf)) return false;
+    }
+    for (int s = 0; s < fp.nstream; ++s) {
+        cudaEventRecord(fp.ev_join[s], fp.stream[s]);
+        cudaStreamWaitEvent(st, fp.ev_join[s], 0);
+    }
+    return true;
 }
 
 inline bool fast_mul2(const FastPlan& fp, const Geom& g, cudaStream_t st, float2* specB, const float* khat)
@@ -214,6 +279,33 @@ inline bool fast_plan_init(FastPlan& fp, const Geom& g, std::string* err)
     fp.ok_mid3 = g.Pz > 1 && g.Py > 1 && ff::split(g.Pz, &T, &E) && E <= 16;
     fp.ok_mul2 = g.Pz == 1 && fp.ok_y;
     fp.nsm = 148;
+    // L2-resident chunks (env MM_CHUNK_W = columns per chunk, multiple of 16): off by default -- measured on
+    // B200 at 512x512x64 they give bit-identical results and cut DRAM traffic, but no time, because the
+    // y and last-axis passes are bound by instruction issue, not by HBM (profiles/).
+    fp.chunk_w = 0;
+    fp.mid_pipe = getenv("MM_MID_PIPE") ? atoi(getenv("MM_MID_PIPE")) : 1;
+    fp.nstream = 3;
+    if (getenv("MM_CHUNK_W")) fp.chunk_w = atoi(getenv("MM_CHUNK_W"));
+    if (getenv("MM_CHUNK_STREAMS")) fp.nstream = atoi(getenv("MM_CHUNK_STREAMS"));
+    if (fp.chunk_w % 16 != 0 || fp.chunk_w < 0 || !(fp.ok_y && fp.ok_mid3)) fp.chunk_w = 0;
+    if (fp.nstream < 1) fp.nstream = 1;
+    if (fp.nstream > 4) fp.nstream = 4;
+    if ((size_t)fp.chunk_w * fp.nstream > (size_t)g.CxS) fp.chunk_w = 0;      // slots must fit specB
+    for (int s = 0; s < 4; ++s) { fp.stream[s] = nullptr; fp.ev_join[s] = nullptr; }
+    fp.ev_fork = nullptr;
+    if (fp.chunk_w > 0) {
+        for (int s = 0; s < fp.nstream; ++s) {
+            if (cudaStreamCreateWithFlags(&fp.stream[s], cudaStreamNonBlocking) != cudaSuccess ||
+                cudaEventCreateWithFlags(&fp.ev_join[s], cudaEventDisableTiming) != cudaSuccess) {
+                if (err) *err = "fast plan: stream / event creation failed";
+                return false;
+            }
+        }
+        if (cudaEventCreateWithFlags(&fp.ev_fork, cudaEventDisableTiming) != cudaSuccess) {
+            if (err) *err = "fast plan: event creation failed";
+            return false;
+        }
+    }
     cudaGetDevice(&dev);
     cudaDeviceGetAttribute(&fp.nsm, cudaDevAttrMultiProcessorCount, dev);
     const int P[3] = { g.Px, g.Py, g.Pz };
@@ -238,6 +330,13 @@ inline bool fast_plan_init(FastPlan& fp, const Geom& g, std::string* err)
 inline void fast_plan_destroy(FastPlan& fp)
 {
     for (int a = 0; a < 3; ++a) { cudaFree(fp.tw[a]); fp.tw[a] = nullptr; }
+    for (int s = 0; s < 4; ++s) {
+        if (fp.stream[s]) cudaStreamDestroy(fp.stream[s]);
+        if (fp.ev_join[s]) cudaEventDestroy(fp.ev_join[s]);
+        fp.stream[s] = nullptr; fp.ev_join[s] = nullptr;
+    }
+    if (fp.ev_fork) cudaEventDestroy(fp.ev_fork);
+    fp.ev_fork = nullptr;
 }
 
 }  // namespace mm

@@ -240,7 +240,7 @@ k_gen_mid(Geom g, FftPlan pl, float2* __restrict__ spec, const float* __restrict
     // h = K m  (the sign and 1/(Px Py Pz) are folded into K-hat)
     {
         const int ky = axis == 2 ? other : 0;
-        const size_t nC = (size_t)g.Cx * g.Cy * g.Cz;
+        const size_t nC = (size_t)g.CxK * g.Cy * g.Cz;
         for (int it = threadIdx.x; it < pl.L * ncol; it += blockDim.x) {
             const int c = it % ncol, i = it / ncol;
             int kyy = ky, kzz = 0;
@@ -248,7 +248,7 @@ k_gen_mid(Geom g, FftPlan pl, float2* __restrict__ spec, const float* __restrict
             float sy = 1.f, sz = 1.f;
             if (2 * kyy > g.Py) { kyy = g.Py - kyy; sy = -1.f; }
             if (2 * kzz > g.Pz) { kzz = g.Pz - kzz; sz = -1.f; }
-            const size_t ko = ((size_t)kzz * g.Cy + kyy) * g.Cx + kx0 + c;
+            const size_t ko = ((size_t)kzz * g.Cy + kyy) * g.CxK + kx0 + c;
             const float kxx = __ldg(&khat[ko]), kyy_ = __ldg(&khat[ko + nC]), kzz_ = __ldg(&khat[ko + 2 * nC]);
             const float kxy = sy * __ldg(&khat[ko + 3 * nC]);
             const float kxz = sz * __ldg(&khat[ko + 4 * nC]);
@@ -278,7 +278,7 @@ __global__ void k_gen_mul1d(Geom g, float2* __restrict__ spec, const float* __re
 {
     const int k = blockIdx.x * blockDim.x + threadIdx.x;
     if (k >= g.Cx) return;
-    const size_t nC = (size_t)g.Cx * g.Cy * g.Cz;
+    const size_t nC = (size_t)g.CxK * g.Cy * g.Cz;
     const float kxx = khat[k], kyy = khat[k + nC], kzz = khat[k + 2 * nC];
     const float kxy = khat[k + 3 * nC], kxz = khat[k + 4 * nC], kyz = khat[k + 5 * nC];
     const float2 mx = spec[k], my = spec[g.CxS + k], mz = spec[2 * (size_t)g.CxS + k];

@@ -233,10 +233,18 @@ mm_status launch_eval(mm_ctx* c, const EpiParams& ep)
             }
             c->kt.end(KT_FWD_X);
         }
-        if (g.Pz > 1) {
+        if (g.Pz > 1 && (c->fast & FAST_CHUNK) && (c->fast & FAST_Y) && (c->fast & FAST_MID) && fp.chunk_w > 0) {
+            // a2-a4 chunked over kx so that the y-padded spectrum stays in L2 (timed as one category)
+            c->kt.begin(KT_MID);
+            if (!fast_yzy_chunked(c->fp, g, st, c->specA, c->specB, c->khat))
+                return fail(c, MM_ECUDA, "chunked y-z-y launch failed");
+            c->kt.end(KT_MID);
+            c->kt.launches += 3 * ((g.Cx + fp.chunk_w - 1) / fp.chunk_w) - 1;
+        } else if (g.Pz > 1) {
+            const ff::ColTile wt = whole_tile(g);
             {   // a2
                 c->kt.begin(KT_FWD_Y);
-                if (!((c->fast & FAST_Y) && fast_y(fp, g, st, -1, c->specA, c->specB))) {
+                if (!((c->fast & FAST_Y) && fast_y(fp, g, st, -1, wt, c->specA, c->specB))) {
                     const int tx = pick_tx(g.Py, 2, 1, &bytes);
                     if (!tx) return fail(c, MM_EUNSUPPORTED, "y line too long for the shared-memory tile");
                     dim3 grid((g.Cx + tx - 1) / tx, 3 * g.Nz);
@@ -246,7 +254,7 @@ mm_status launch_eval(mm_ctx* c, const EpiParams& ep)
             }
             {   // a3
                 c->kt.begin(KT_MID);
-                if (!((c->fast & FAST_MID) && fast_mid3(fp, g, st, c->specB, c->khat))) {
+                if (!((c->fast & FAST_MID) && fast_mid3(fp, g, st, wt, c->specB, c->khat))) {
                     const int tx = pick_tx(g.Pz, 4, 1, &bytes);
                     if (!tx) return fail(c, MM_EUNSUPPORTED, "z line too long for the shared-memory tile");
                     dim3 grid((g.Cx + tx - 1) / tx, g.Py);
@@ -256,7 +264,7 @@ mm_status launch_eval(mm_ctx* c, const EpiParams& ep)
             }
             {   // a4
                 c->kt.begin(KT_INV_Y);
-                if (!((c->fast & FAST_Y) && fast_y(fp, g, st, 1, c->specB, c->specA))) {
+                if (!((c->fast & FAST_Y) && fast_y(fp, g, st, 1, wt, c->specA, c->specB))) {
                     const int tx = pick_tx(g.Py, 2, 1, &bytes);
                     dim3 grid((g.Cx + tx - 1) / tx, 3 * g.Nz);
                     k_gen_y<1><<<grid, 256, bytes, st>>>(g, c->plan[1], c->specB, c->specA, tx);
@@ -267,14 +275,15 @@ mm_status launch_eval(mm_ctx* c, const EpiParams& ep)
             if ((c->fast & FAST_MID) && fp.ok_mul2) {
                 // 2D: y forward, k-space multiply, y inverse as three launches (the spectra of a 2D grid
                 // are L2-resident, so the extra round trip does not reach HBM)
+                const ff::ColTile wt = whole_tile(g);
                 c->kt.begin(KT_FWD_Y);
-                fast_y(fp, g, st, -1, c->specA, c->specB);
+                fast_y(fp, g, st, -1, wt, c->specA, c->specB);
                 c->kt.end(KT_FWD_Y);
                 c->kt.begin(KT_MID);
                 fast_mul2(fp, g, st, c->specB, c->khat);
                 c->kt.end(KT_MID);
                 c->kt.begin(KT_INV_Y);
-                fast_y(fp, g, st, 1, c->specB, c->specA);
+                fast_y(fp, g, st, 1, wt, c->specA, c->specB);
                 c->kt.end(KT_INV_Y);
             } else {   // generic: y forward, multiply, y inverse in one kernel
                 const int tx = pick_tx(g.Py, 4, 1, &bytes);
@@ -485,6 +494,7 @@ mm_status mm_create(mm_ctx** out, const int grid[3], const double cellsize[3], c
     g.Px = P[0]; g.Py = P[1]; g.Pz = P[2];
     g.Cx = P[0] / 2 + 1; g.Cy = P[1] / 2 + 1; g.Cz = P[2] / 2 + 1;
     g.CxS = (g.Cx + 7) & ~7;     // rows start on 64-byte boundaries
+    g.CxK = (g.Cx + 3) & ~3;
     g.perx = pbc[0] > 0; g.pery = pbc[1] > 0; g.perz = pbc[2] > 0;
     for (int a = 0; a < 3; ++a) { c->cell[a] = cellsize[a]; c->pbc[a] = pbc[a]; }
     c->stream = (cudaStream_t)cuda_stream;
@@ -536,8 +546,11 @@ mm_status mm_demag_init(mm_ctx* c)
     std::string err;
     const int rc = mmh::build_khat(c->cell, grid, c->pbc, kh.data(), &err);
     if (rc != 0) return fail(c, (mm_status)rc, err);
-    CUDA_TRY(c, cudaMalloc(&c->khat, 6 * nC * sizeof(float)));
-    CUDA_TRY(c, cudaMemcpy(c->khat, kh.data(), 6 * nC * sizeof(float), cudaMemcpyHostToDevice));
+    const size_t nrow = (size_t)6 * g.Cz * g.Cy;         // device rows are padded to CxK floats (zeros)
+    CUDA_TRY(c, cudaMalloc(&c->khat, nrow * g.CxK * sizeof(float)));
+    CUDA_TRY(c, cudaMemset(c->khat, 0, nrow * g.CxK * sizeof(float)));
+    CUDA_TRY(c, cudaMemcpy2D(c->khat, g.CxK * sizeof(float), kh.data(), g.Cx * sizeof(float), g.Cx * sizeof(float),
+                             nrow, cudaMemcpyHostToDevice));
     const size_t nA = (size_t)3 * g.Nz * g.Ny * g.CxS;
     CUDA_TRY(c, cudaMalloc(&c->specA, nA * sizeof(float2)));
     CUDA_TRY(c, cudaMemset(c->specA, 0, nA * sizeof(float2)));
@@ -768,7 +781,10 @@ mm_status mm_get_demag_kernel(mm_ctx* c, int comp, float* host_out, size_t n)
     if (!c->has_demag) return fail(c, MM_ESTATE, "mm_demag_init has not been called");
     const size_t nC = (size_t)c->g.Cx * c->g.Cy * c->g.Cz;
     if (n < nC) return fail(c, MM_EINVAL, "host_out too small");
-    CUDA_TRY(c, cudaMemcpy(host_out, c->khat + comp * nC, nC * sizeof(float), cudaMemcpyDeviceToHost));
+    const Geom& g = c->g;
+    CUDA_TRY(c, cudaMemcpy2D(host_out, g.Cx * sizeof(float), c->khat + (size_t)comp * g.Cz * g.Cy * g.CxK,
+                             g.CxK * sizeof(float), g.Cx * sizeof(float), (size_t)g.Cz * g.Cy,
+                             cudaMemcpyDeviceToHost));
     return MM_OK;
 }
 

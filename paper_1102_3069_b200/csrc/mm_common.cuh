@@ -6,7 +6,7 @@
 //   field      float  [3][Nz][Ny][Nx]                      m, H, k_s, caller or context owned
 //   specA      float2 [3][Nz][Ny][CxS]                     after the x pass   (CxS >= Cx = Px/2+1)
 //   specB      float2 [3][Nz][Py][CxS]                     after the y pass   (3D only)
-//   khat       float  [6][Cz][Cy][Cx]  (xx,yy,zz,xy,xz,yz) one octant, includes -1/(Px Py Pz)
+//   khat       float  [6][Cz][Cy][CxK] (xx,yy,zz,xy,xz,yz) one octant, includes -1/(Px Py Pz)
 // Units on the device (section 3.3): fields in units of Ms, time in 1/(gamma0 Ms).
 #pragma once
 #include <cuda_runtime.h>
@@ -19,6 +19,7 @@ struct Geom {
     int Px, Py, Pz;      // padded transform sizes (reading A9)
     int Cx, Cy, Cz;      // P/2 + 1
     int CxS;             // row stride of the spectra, in complex elements
+    int CxK;             // row stride of K-hat, in floats (Cx rounded up to 4: 16-byte rows)
     int perx, pery, perz;
 };
 
