@@ -124,11 +124,11 @@ bool launch_mid3(const FastPlan& fp, const Geom& g, cudaStream_t st, const ColTi
         const size_t pb = (size_t)3 * T * (E + 1) * 16 * sizeof(float2) + (size_t)3 * NZ * 16 * sizeof(float2) +
                           (size_t)6 * (L / 2 + 1) * 16 * sizeof(float);
         if (pb <= 227 * 1024) {
-            static bool oncep = ensure_smem(k_mid_p<T, E, PER>, pb);
-            if (!oncep) return false;
             const int nitem = ((ct.ncol + 15) / 16) * (g.Py / 2 + 1);
             const int per_sm = (T * E <= 128) ? 2 : 1;
             const int grid = nitem < fp.nsm * per_sm ? nitem : fp.nsm * per_sm;
+            static bool oncep = ensure_smem(k_mid_p<T, E, PER>, pb);
+            if (!oncep) return false;
             k_mid_p<T, E, PER><<<grid, 16 * T, pb, st>>>(g, ct, specB, khat, fp.tw[2]);
             return true;
         }
