@@ -65,6 +65,16 @@ k_fwd_x(Geom g, const float* __restrict__ m, float2* __restrict__ specA, const f
     }
 }
 
+// ---- cp.async helpers (16-byte copies global -> shared, zero-filled beyond src_bytes) ----
+__device__ __forceinline__ void cp_async16(void* smem, const void* gmem, int src_bytes)
+{
+    const unsigned s = (unsigned)__cvta_generic_to_shared(smem);
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;\n" ::"r"(s), "l"(gmem), "r"(src_bytes) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;\n" ::"n"(N) : "memory"); }
+
 // ---------------------------------------------------------------------------------------------
 // Where the columns of a y / last-axis pass live.  The whole-array mode uses the layouts of
 // mm_common.cuh (row stride CxS); the chunked mode works on `ncol`
@@ -110,6 +120,89 @@ k_y(ColTile ct, float2* __restrict__ a, float2* __restrict__ b, const float2* __
 #pragma unroll
         for (int j = 0; j < NOUT; ++j) dp[(size_t)(t + T * j) * d_row] = v[j];
     }
+}
+
+// ---------------------------------------------------------------------------------------------
+// a2 / a4, persistent and software-pipelined: same arithmetic and thread layout as k_y, but a block
+// loops over tiles (8 columns of one plane) and the NEXT tile's rows arrive by cp.async while the
+// second register FFT and the stores of the current tile run.  The staged tile [rows][8] and the
+// exchange buffer share one shared-memory region (the tile is consumed into registers before the
+// exchange starts, and the copy for the next tile is issued once the exchange has been read back),
+// so the footprint stays that of k_y.  grid = 2 blocks per SM; tile i -> (columns i % ntx, plane i / ntx).
+// ---------------------------------------------------------------------------------------------
+template <int T, int E, int SGN, bool PER>
+__global__ void __launch_bounds__(8 * T, (T == 32) ? 2 : 1)
+k_y_p(ColTile ct, int nplane, float2* __restrict__ a, float2* __restrict__ b, const float2* __restrict__ tw)
+{
+    constexpr bool FWD = SGN < 0;
+    constexpr int NIN = (FWD && !PER) ? E / 2 : E;
+    constexpr int NOUT = (!FWD && !PER) ? E / 2 : E;
+    constexpr int NT = 8 * T;
+    constexpr int ROWS = NIN * T;               // rows of the input tile
+    float2* sm = ff_smem;
+    const int tid = threadIdx.x, c = tid & 7, t = tid >> 3;
+    const int ntx = (ct.ncol + 7) >> 3;
+    const int ntile = ntx * nplane;
+    const size_t s_row = FWD ? ct.a_row : ct.b_row, d_row = FWD ? ct.b_row : ct.a_row;
+    const size_t s_plane = FWD ? ct.a_plane : ct.b_plane, d_plane = FWD ? ct.b_plane : ct.a_plane;
+    const float2* __restrict__ src = FWD ? a : b;
+    float2* __restrict__ dst = FWD ? b : a;
+
+    auto issue = [&](int i) {
+        const int bx = i % ntx, cz = i / ntx;
+        const float2* __restrict__ s0 = src + (size_t)cz * s_plane + bx * 8;
+        for (int u = tid; u < ROWS * 4; u += NT) {
+            const int cu = u & 3, r = u >> 2;
+            const int left = ct.ncol - (bx * 8 + 2 * cu);
+            const int nb = left >= 2 ? 16 : (left == 1 ? 8 : 0);
+            cp_async16(sm + r * 8 + 2 * cu, nb ? s0 + (size_t)r * s_row + 2 * cu : src, nb);
+        }
+    };
+
+    int i = blockIdx.x;
+    if (i < ntile) issue(i);
+    cp_async_commit();
+    for (; i < ntile; i += gridDim.x) {
+        const int bx = i % ntx, cz = i / ntx;
+        const int col = bx * 8 + c;
+        cp_async_wait<0>();
+        __syncthreads();                        // this tile has landed
+        float2 v[E];
+#pragma unroll
+        for (int j = 0; j < NIN; ++j) v[j] = sm[(t + T * j) * 8 + c];
+        __syncthreads();                        // the region now serves as the exchange buffer
+        if constexpr (FWD && !PER) fft_reg_half<E, SGN>(v);
+        else fft_reg<E, SGN>(v);
+#pragma unroll
+        for (int k2 = 1; k2 < E; ++k2) {
+            float2 w = __ldg(tw + k2 * T + t);
+            if (SGN > 0) w.y = -w.y;
+            v[k2] = cmul(v[k2], w);
+        }
+#pragma unroll
+        for (int k2 = 0; k2 < E; ++k2) sm[(t * (E + 1) + k2) * 8 + c] = v[k2];
+        __syncthreads();
+        float2 u[E / T][T];
+#pragma unroll
+        for (int q = 0; q < E / T; ++q)
+#pragma unroll
+            for (int n1 = 0; n1 < T; ++n1) u[q][n1] = sm[(n1 * (E + 1) + t + T * q) * 8 + c];
+        __syncthreads();                        // exchange read back: the region is free for the next tile
+        if (i + (int)gridDim.x < ntile) issue(i + gridDim.x);
+        cp_async_commit();
+#pragma unroll
+        for (int q = 0; q < E / T; ++q) {
+            fft_reg<T, SGN>(u[q]);
+#pragma unroll
+            for (int k1 = 0; k1 < T; ++k1) v[q + (E / T) * k1] = u[q][k1];
+        }
+        if (col < ct.ncol) {
+            float2* __restrict__ dp = dst + (size_t)cz * d_plane + col;
+#pragma unroll
+            for (int j = 0; j < NOUT; ++j) dp[(size_t)(t + T * j) * d_row] = v[j];
+        }
+    }
+    cp_async_wait<0>();
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -198,16 +291,6 @@ k_mid(Geom g, ColTile ct, float2* __restrict__ spec, const float* __restrict__ k
             for (int j = 0; j < NIO; ++j) base[comp * cstride + (size_t)(t + T * j) * rstride] = v[comp][j];
     }
 }
-
-// ---- cp.async helpers (16-byte copies global -> shared, zero-filled beyond src_bytes) ----
-__device__ __forceinline__ void cp_async16(void* smem, const void* gmem, int src_bytes)
-{
-    const unsigned s = (unsigned)__cvta_generic_to_shared(smem);
-    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;\n" ::"r"(s), "l"(gmem), "r"(src_bytes) : "memory");
-}
-__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::: "memory"); }
-template <int N>
-__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;\n" ::"n"(N) : "memory"); }
 
 // ---------------------------------------------------------------------------------------------
 // a3, persistent and software-pipelined (3D grids, z axis): same arithmetic as k_mid, but a block

@@ -10,6 +10,7 @@ struct FastPlan {
     bool ok_x, ok_y, ok_mid3, ok_mul2;   // which passes have a size-specialised kernel for this grid
     float2* tw[3];                       // per axis: tw[k2 * T + t] = exp(-2 pi i t k2 / L)
     int nsm;                             // SM count (persistent grids)
+    int y_pipe;                          // y passes: persistent cp.async-pipelined kernel (env MM_Y_PIPE)
     int mid_pipe;                        // last-axis pass: persistent cp.async-pipelined kernel (env MM_MID_PIPE)
     int chunk_w, nstream;                // chunked a2-a4: columns per chunk (0 = whole-array passes), streams
     cudaStream_t stream[4];
@@ -107,6 +108,18 @@ template <int T, int E, int SGN, bool PER>
 bool launch_y(const FastPlan& fp, const Geom& g, cudaStream_t st, const ColTile& ct, float2* a, float2* b)
 {
     const size_t bytes = (size_t)T * (E + 1) * 8 * sizeof(float2);
+    if (fp.y_pipe) {
+        static bool oncep = ensure_smem(k_y_p<T, E, SGN, PER>, bytes);
+        if (!oncep) return false;
+        const int ntile = ((ct.ncol + 7) / 8) * 3 * g.Nz;
+        int per_sm = (int)((227 * 1024) / (bytes + 1024));
+        const int cap = 2048 / (8 * T) < ((T == 32) ? 2 : 8) ? 2048 / (8 * T) : ((T == 32) ? 2 : 8);
+        if (per_sm > cap) per_sm = cap;
+        if (per_sm < 1) per_sm = 1;
+        const int grid = ntile < fp.nsm * per_sm ? ntile : fp.nsm * per_sm;
+        k_y_p<T, E, SGN, PER><<<grid, 8 * T, bytes, st>>>(ct, 3 * g.Nz, a, b, fp.tw[1]);
+        return true;
+    }
     static bool once = ensure_smem(k_y<T, E, SGN, PER>, bytes);
     if (!once) return false;
     dim3 grid((ct.ncol + 7) / 8, 3 * g.Nz);
@@ -283,6 +296,7 @@ inline bool fast_plan_init(FastPlan& fp, const Geom& g, std::string* err)
     // B200 at 512x512x64 they give bit-identical results and cut DRAM traffic, but no time, because the
     // y and last-axis passes are bound by instruction issue, not by HBM (profiles/).
     fp.chunk_w = 0;
+    fp.y_pipe = getenv("MM_Y_PIPE") ? atoi(getenv("MM_Y_PIPE")) : 1;
     fp.mid_pipe = getenv("MM_MID_PIPE") ? atoi(getenv("MM_MID_PIPE")) : 1;
     fp.nstream = 3;
     if (getenv("MM_CHUNK_W")) fp.chunk_w = atoi(getenv("MM_CHUNK_W"));
