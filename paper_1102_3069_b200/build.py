@@ -28,7 +28,8 @@ def _stale() -> bool:
 def build(force: bool = False, verbose: bool = False) -> str:
     if force or _stale():
         nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-        cmd = [nvcc, *NVCC_FLAGS, "-o", LIB, *[os.path.join(CSRC, s) for s in SOURCES]]
+        extra = os.environ.get("MM_NVCC_EXTRA", "").split()       # e.g. -DMM_PACKED_F32X2 (experiments)
+        cmd = [nvcc, *NVCC_FLAGS, *extra, "-o", LIB, *[os.path.join(CSRC, s) for s in SOURCES]]
         if verbose:
             cmd += ["-Xptxas", "-v"]
         subprocess.check_call(cmd)
