@@ -228,10 +228,10 @@ def main():
         torch.cuda.synchronize()
 
     # ---- device-resident timing ----
+    sampler = ClockSampler(local)          # samples from the warm-up to the end of the e2e region
+    sampler.start()
     sim.steps_fixed(md, method, dt, max(3, args.warmup))
     barrier()
-    sampler = ClockSampler(local)
-    sampler.start()
     sim.kernel_timing(True)
     l0 = sim.launch_count()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
@@ -244,7 +244,6 @@ def main():
     launches = sim.launch_count() - l0
     kt = sim.kernel_times()
     sim.kernel_timing(False)
-    clocks = sampler.stop()
     if dist is not None:
         t = torch.tensor([sec], device="cuda", dtype=torch.float64)
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
@@ -274,6 +273,7 @@ def main():
         e2e = {"value": world * evals / sec2, "unit": UNIT, "h2d_bytes_per_step": nb, "d2h_bytes_per_step": nb,
                "ms_per_step": sec2 / args.steps * 1e3}
 
+    clocks = sampler.stop()
     if rank != 0:
         return
 
@@ -314,8 +314,8 @@ def main():
     out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
            "warmup": max(3, args.warmup), "ms_per_step": sec / args.steps * 1e3, "higher_is_better": True,
            "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-           "config": {"workload": f"{wl.name}: {wl.grid[0]}x{wl.grid[1]}x{wl.grid[2]} cells, open boundaries, "
-                                  f"vortex + noise state, RK4 dt={dt:g} s, 1 step = 4 fused evaluations",
+           "config": {"workload": f"{wl.name}: {wl.grid[0]}x{wl.grid[1]}x{wl.grid[2]} cells, pbc {tuple(wl.pbc)}, "
+                                  f"'{wl.init}' state (seed {wl.seed}), RK4 dt={dt:g} s, 1 step = 4 fused evaluations",
                       "l2": "working set > 2 GB >> 126 MB L2 (inputs larger than L2, no flush)",
                       "parallelism": "replicas" if world > 1 else "single GPU",
                       "path": "generic" if args.generic else "fast"},

@@ -391,7 +391,7 @@ __device__ __forceinline__ void block_max_atomic(unsigned int b, unsigned int* t
 // cells along x (float4 traffic), takes its x neighbours from the adjacent lanes and the y / z
 // neighbours from the rows above and below.  Needs Nx % 4 == 0.  One quad per thread.
 // ---------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(256)
+__global__ void __launch_bounds__(256, 3)
 k_epi4(Geom g, const float* __restrict__ hms, EpiParams ep)
 {
     const int nx4 = g.Nx >> 2;
