@@ -31,6 +31,25 @@ __host__ __device__ constexpr float cos32(int j)
 }
 __host__ __device__ constexpr float sin32(int j) { return cos32(j - 8); }
 
+// cos(2 pi j / 48) and sin(2 pi j / 48): the lengths with one factor 3 (24, 48)
+__host__ __device__ constexpr float cos48(int j)
+{
+    j %= 48;
+    if (j < 0) j += 48;
+    if (j > 24) j = 48 - j;
+    bool neg = false;
+    if (j > 12) { j = 24 - j; neg = true; }
+    const float t[13] = { 1.0f, 0.9914448613738104f, 0.9659258262890683f, 0.9238795325112867f, 0.8660254037844387f, 0.7933533402912352f, 0.7071067811865476f, 0.6087614290087207f, 0.5000000000000001f, 0.38268343236508984f, 0.25881904510252074f, 0.1305261922200517f, 0.0f };
+    return neg ? -t[j] : t[j];
+}
+__host__ __device__ constexpr float sin48(int j) { return cos48(j - 12); }
+
+// real and imaginary part of exp(2 pi i k / N) for N dividing 32 or 48
+template <int N>
+__host__ __device__ constexpr float cosN(int k) { return 32 % N == 0 ? cos32(k * (32 / (32 % N == 0 ? N : 1))) : cos48(k * (48 / N)); }
+template <int N>
+__host__ __device__ constexpr float sinN(int k) { return 32 % N == 0 ? sin32(k * (32 / (32 % N == 0 ? N : 1))) : sin48(k * (48 / N)); }
+
 template <int N, int SGN>
 __device__ __forceinline__ void fft_reg(float2 (&v)[N]);
 
@@ -71,12 +90,47 @@ __device__ __forceinline__ void dit_combine(float2 (&v)[N], const float2 (&e)[N 
     }
 }
 
-// in-place DFT of N = 2, 4, 8, 16, 32 register values, natural order in and out
+// top level of a length N = 3 M transform (decimation in time by 3): v[k + M m] = sum_r w3^(r m) w_N^(r k) e_r[k]
+template <int N, int SGN, int K>
+__device__ __forceinline__ void dit3_combine(float2 (&v)[N], const float2 (&e0)[N / 3], const float2 (&e1)[N / 3],
+                                             const float2 (&e2)[N / 3])
+{
+    constexpr int M = N / 3;
+    if constexpr (K < M) {
+        float2 b = e1[K], c = e2[K];
+        if constexpr (K > 0) {
+            constexpr float c1 = cosN<N>(K), s1 = SGN * sinN<N>(K);
+            constexpr float c2 = cosN<N>(2 * K), s2 = SGN * sinN<N>(2 * K);
+            b = make_float2(fmaf(c1, b.x, -s1 * b.y), fmaf(c1, b.y, s1 * b.x));
+            c = make_float2(fmaf(c2, c.x, -s2 * c.y), fmaf(c2, c.y, s2 * c.x));
+        }
+        const float S = 0.86602540378443864676f;
+        const float2 a = e0[K];
+        const float2 s = padd(b, c);
+        const float2 d = cmuli<SGN>(cscale(psub(b, c), S));
+        const float2 m = make_float2(fmaf(-0.5f, s.x, a.x), fmaf(-0.5f, s.y, a.y));
+        v[K] = padd(a, s);
+        v[K + M] = cadd(m, d);
+        v[K + 2 * M] = csub(m, d);
+        dit3_combine<N, SGN, K + 1>(v, e0, e1, e2);
+    }
+}
+
+// in-place DFT of N = 2, 4, 8, 16, 32 or 24, 48 register values, natural order in and out
 template <int N, int SGN>
 __device__ __forceinline__ void fft_reg(float2 (&v)[N])
 {
-    static_assert(N == 2 || N == 4 || N == 8 || N == 16 || N == 32, "register FFT size");
-    if constexpr (N == 2) {
+    static_assert(N == 2 || N == 4 || N == 8 || N == 16 || N == 32 || N == 12 || N == 24 || N == 48, "register FFT size");
+    if constexpr (N % 3 == 0) {
+        constexpr int M = N / 3;
+        float2 e0[M], e1[M], e2[M];
+#pragma unroll
+        for (int i = 0; i < M; ++i) { e0[i] = v[3 * i]; e1[i] = v[3 * i + 1]; e2[i] = v[3 * i + 2]; }
+        fft_reg<M, SGN>(e0);
+        fft_reg<M, SGN>(e1);
+        fft_reg<M, SGN>(e2);
+        dit3_combine<N, SGN, 0>(v, e0, e1, e2);
+    } else if constexpr (N == 2) {
         const float2 a = v[0], b = v[1];
         v[0] = padd(a, b);
         v[1] = psub(a, b);
@@ -104,8 +158,8 @@ __device__ __forceinline__ void half_twiddle(float2 (&b)[N / 2])
         if constexpr (4 * K == N) {
             b[K] = cmuli<SGN>(b[K]);
         } else if constexpr (K > 0) {
-            constexpr float c = cos32(K * (32 / N));
-            constexpr float s = SGN * sin32(K * (32 / N));
+            constexpr float c = cosN<N>(K);
+            constexpr float s = SGN * sinN<N>(K);
             const float2 x = b[K];
             b[K] = make_float2(fmaf(c, x.x, -s * x.y), fmaf(c, x.y, s * x.x));
         }

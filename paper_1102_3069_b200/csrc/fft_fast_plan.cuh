@@ -23,6 +23,9 @@ inline bool split(int L, int* T, int* E)
 {
     switch (L) {
     case 64: *T = 8; *E = 8; return true;
+    case 192: *T = 8; *E = 24; return true;
+    case 384: *T = 8; *E = 48; return true;
+    case 768: *T = 16; *E = 48; return true;
     case 128: *T = 8; *E = 16; return true;
     case 256: *T = 16; *E = 16; return true;
     case 512: *T = 16; *E = 32; return true;
@@ -158,6 +161,9 @@ bool launch_mid3(const FastPlan& fp, const Geom& g, cudaStream_t st, const ColTi
 #define MM_FF_SIZES(L, CALL)                 \
     switch (L) {                              \
     case 64: { CALL(8, 8); } break;           \
+    case 192: { CALL(8, 24); } break;         \
+    case 384: { CALL(8, 48); } break;         \
+    case 768: { CALL(16, 48); } break;        \
     case 128: { CALL(8, 16); } break;         \
     case 256: { CALL(16, 16); } break;        \
     case 512: { CALL(16, 32); } break;        \
