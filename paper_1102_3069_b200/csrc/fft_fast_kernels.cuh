@@ -582,6 +582,102 @@ k_inv_x_h(Geom g, const float2* __restrict__ specA, const float2* __restrict__ t
     }
 }
 
+// ---------------------------------------------------------------------------------------------
+// a1 / a5 for x lengths Px = 2 Lc whose half Lc = T E has a register plan (1536 = 2 * 768,
+// 2048 = 2 * 1024): the real transform of ONE row through a complex transform of half the length,
+// z[n] = x[2n] + i x[2n+1] (read straight from the row as float2), then
+//   X[k] = E[k] + w^k O[k],  E = (Z[k] + conj Z[Lc-k]) / 2,  O = (Z[k] - conj Z[Lc-k]) / (2i),  w = exp(-i pi / Lc)
+// with the partner Z[Lc-k] taken from lane T-t, register E-1-j as in k_fwd_x.  twx[k] = w^k.
+// ---------------------------------------------------------------------------------------------
+template <int T, int E, bool PER>
+__global__ void __launch_bounds__(128)
+k_fwd_x_r(Geom g, const float* __restrict__ m, float2* __restrict__ specA, const float2* __restrict__ tw,
+          const float2* __restrict__ twx)
+{
+    constexpr int Lc = T * E;
+    constexpr int LB = T * (E + 1);
+    constexpr int NIN = PER ? E : E / 2;
+    const int t = threadIdx.x % T;
+    const int slot = threadIdx.x / T;
+    const int nslot = 128 / T;
+    float2* sb = ff_smem + slot * LB;
+    const int nrow = 3 * g.Nz * g.Ny;
+    const unsigned lane = threadIdx.x & 31;
+    const unsigned src = lane - t + ((T - t) % T);
+    for (int rb = blockIdx.x * nslot; rb < nrow; rb += gridDim.x * nslot) {
+        const bool act = rb + slot < nrow;
+        const int row = act ? rb + slot : nrow - 1;
+        const float2* __restrict__ r0 = reinterpret_cast<const float2*>(m + (size_t)row * g.Nx);
+        float2 v[E];
+#pragma unroll
+        for (int j = 0; j < NIN; ++j) v[j] = r0[t + T * j];
+        __syncwarp();
+        fft_line<T, E, -1, !PER>(v, sb, 1, t, tw, SyncWarp());
+        float2* __restrict__ o = specA + (size_t)row * g.CxS;
+#pragma unroll
+        for (int j = 0; j < E; ++j) {
+            float2 p;
+            p.x = __shfl_sync(0xffffffffu, v[E - 1 - j].x, src);
+            p.y = __shfl_sync(0xffffffffu, v[E - 1 - j].y, src);
+            if (t == 0) p = v[(E - j) % E];
+            const float2 z = v[j];
+            const float2 ek = make_float2(0.5f * (z.x + p.x), 0.5f * (z.y - p.y));
+            const float2 ok = make_float2(0.5f * (z.y + p.y), 0.5f * (p.x - z.x));
+            const float2 w = __ldg(twx + t + T * j);
+            if (act) o[t + T * j] = cadd(ek, cmul(w, ok));
+        }
+        if (t == 0 && act) o[Lc] = make_float2(v[0].x - v[0].y, 0.f);
+    }
+}
+
+template <int T, int E, bool PER>
+__global__ void __launch_bounds__(128)
+k_inv_x_h_r(Geom g, const float2* __restrict__ specA, const float2* __restrict__ tw,
+            const float2* __restrict__ twx, float* __restrict__ out, float scale)
+{
+    constexpr int Lc = T * E;
+    constexpr int LB = T * (E + 1);
+    constexpr int NOUT = PER ? E : E / 2;
+    const int t = threadIdx.x % T;
+    const int slot = threadIdx.x / T;
+    const int nslot = 128 / T;
+    float2* sb = ff_smem + slot * LB;
+    const int nrow = 3 * g.Nz * g.Ny;
+    const unsigned lane = threadIdx.x & 31;
+    const unsigned src = lane - t + ((T - t) % T);
+    for (int rb = blockIdx.x * nslot; rb < nrow; rb += gridDim.x * nslot) {
+        const bool act = rb + slot < nrow;
+        const int row = act ? rb + slot : nrow - 1;
+        const float2* __restrict__ a0 = specA + (size_t)row * g.CxS;
+        float2 x[E], v[E];
+#pragma unroll
+        for (int j = 0; j < E; ++j) x[j] = a0[t + T * j];
+        float2 xn = make_float2(0.f, 0.f);
+        if (t == 0) xn = a0[Lc];
+        // 2 Z[k] = (X[k] + conj X[Lc-k]) + i conj(w^k) (X[k] - conj X[Lc-k])
+#pragma unroll
+        for (int j = 0; j < E; ++j) {
+            float2 p;
+            p.x = __shfl_sync(0xffffffffu, x[E - 1 - j].x, src);
+            p.y = __shfl_sync(0xffffffffu, x[E - 1 - j].y, src);
+            if (t == 0) p = j == 0 ? xn : x[(E - j) % E];
+            const float2 z = x[j];
+            const float2 e2 = make_float2(z.x + p.x, z.y - p.y);
+            const float2 d = make_float2(z.x - p.x, z.y + p.y);
+            const float2 w = cconj(__ldg(twx + t + T * j));
+            const float2 o2 = cmul(w, d);
+            v[j] = make_float2(e2.x - o2.y, e2.y + o2.x);
+        }
+        __syncwarp();
+        fft_line<T, E, 1, false>(v, sb, 1, t, tw, SyncWarp());
+        float2* __restrict__ o = reinterpret_cast<float2*>(out + (size_t)row * g.Nx);
+        if (act) {
+#pragma unroll
+            for (int j = 0; j < NOUT; ++j) o[t + T * j] = make_float2(scale * v[j].x, scale * v[j].y);
+        }
+    }
+}
+
 }  // namespace ff
 }  // namespace mm
 

@@ -8,6 +8,8 @@ enum FastBits { FAST_FWD_X = 1, FAST_Y = 2, FAST_MID = 4, FAST_INV_X = 8, FAST_S
 
 struct FastPlan {
     bool ok_x, ok_y, ok_mid3, ok_mul2;   // which passes have a size-specialised kernel for this grid
+    bool ok_xr;                          // x passes through the half-length complex transform (Px = 1536, 2048)
+    float2* twx;                         // ok_xr: exp(-i pi k / Lc), k < Lc = Px / 2
     float2* tw[3];                       // per axis: tw[k2 * T + t] = exp(-2 pi i t k2 / L)
     int nsm;                             // SM count (persistent grids)
     int y_pipe;                          // y passes: persistent cp.async-pipelined kernel (env MM_Y_PIPE)
@@ -107,6 +109,33 @@ bool launch_inv_x_h(const FastPlan& fp, const Geom& g, cudaStream_t st, const fl
     return true;
 }
 
+template <int T, int E, bool PER>
+bool launch_fwd_x_r(const FastPlan& fp, const Geom& g, cudaStream_t st, const float* m, float2* specA)
+{
+    const size_t bytes = (size_t)(128 / T) * T * (E + 1) * sizeof(float2);
+    static bool once = ensure_smem(k_fwd_x_r<T, E, PER>, bytes);
+    if (!once) return false;
+    const int nslot = 128 / T;
+    const int want = (3 * g.Nz * g.Ny + nslot - 1) / nslot;
+    const int grid = want < fp.nsm * 8 ? want : fp.nsm * 8;
+    k_fwd_x_r<T, E, PER><<<grid, 128, bytes, st>>>(g, m, specA, fp.tw[0], fp.twx);
+    return true;
+}
+
+template <int T, int E, bool PER>
+bool launch_inv_x_h_r(const FastPlan& fp, const Geom& g, cudaStream_t st, const float2* specA, float* out,
+                      float scale)
+{
+    const size_t bytes = (size_t)(128 / T) * T * (E + 1) * sizeof(float2);
+    static bool once = ensure_smem(k_inv_x_h_r<T, E, PER>, bytes);
+    if (!once) return false;
+    const int nslot = 128 / T;
+    const int want = (3 * g.Nz * g.Ny + nslot - 1) / nslot;
+    const int grid = want < fp.nsm * 8 ? want : fp.nsm * 8;
+    k_inv_x_h_r<T, E, PER><<<grid, 128, bytes, st>>>(g, specA, fp.tw[0], fp.twx, out, scale);
+    return true;
+}
+
 template <int T, int E, int SGN, bool PER>
 bool launch_y(const FastPlan& fp, const Geom& g, cudaStream_t st, const ColTile& ct, float2* a, float2* b)
 {
@@ -175,6 +204,13 @@ bool launch_mid3(const FastPlan& fp, const Geom& g, cudaStream_t st, const ColTi
 
 inline bool fast_fwd_x(const FastPlan& fp, const Geom& g, cudaStream_t st, const float* m, float2* specA)
 {
+    if (fp.ok_xr) {
+        if (g.Px == 1536) return g.perx ? ff::launch_fwd_x_r<16, 48, true>(fp, g, st, m, specA)
+                                        : ff::launch_fwd_x_r<16, 48, false>(fp, g, st, m, specA);
+        if (g.Px == 2048) return g.perx ? ff::launch_fwd_x_r<32, 32, true>(fp, g, st, m, specA)
+                                        : ff::launch_fwd_x_r<32, 32, false>(fp, g, st, m, specA);
+        return false;
+    }
     if (!fp.ok_x) return false;
     bool r = false;
 #define CALL(T, E) r = g.perx ? ff::launch_fwd_x<T, E, true>(fp, g, st, m, specA) \
@@ -199,6 +235,13 @@ inline bool fast_inv_x(const FastPlan& fp, const Geom& g, cudaStream_t st, const
 inline bool fast_inv_x_h(const FastPlan& fp, const Geom& g, cudaStream_t st, const float2* specA, float* out,
                          float scale)
 {
+    if (fp.ok_xr) {
+        if (g.Px == 1536) return g.perx ? ff::launch_inv_x_h_r<16, 48, true>(fp, g, st, specA, out, scale)
+                                        : ff::launch_inv_x_h_r<16, 48, false>(fp, g, st, specA, out, scale);
+        if (g.Px == 2048) return g.perx ? ff::launch_inv_x_h_r<32, 32, true>(fp, g, st, specA, out, scale)
+                                        : ff::launch_inv_x_h_r<32, 32, false>(fp, g, st, specA, out, scale);
+        return false;
+    }
     if (!fp.ok_x) return false;
     bool r = false;
 #define CALL(T, E) r = g.perx ? ff::launch_inv_x_h<T, E, true>(fp, g, st, specA, out, scale) \
@@ -294,6 +337,8 @@ inline bool fast_plan_init(FastPlan& fp, const Geom& g, std::string* err)
 {
     int T, E, dev = 0;
     fp.ok_x = ff::split(g.Px, &T, &E);
+    fp.ok_xr = !fp.ok_x && (g.Px == 1536 || g.Px == 2048) && g.Nx % 2 == 0;
+    fp.twx = nullptr;
     fp.ok_y = g.Py > 1 && ff::split(g.Py, &T, &E);
     fp.ok_mid3 = g.Pz > 1 && g.Py > 1 && ff::split(g.Pz, &T, &E) && E <= 16;
     fp.ok_mul2 = g.Pz == 1 && fp.ok_y;
@@ -328,7 +373,20 @@ inline bool fast_plan_init(FastPlan& fp, const Geom& g, std::string* err)
     }
     cudaGetDevice(&dev);
     cudaDeviceGetAttribute(&fp.nsm, cudaDevAttrMultiProcessorCount, dev);
-    const int P[3] = { g.Px, g.Py, g.Pz };
+    const int P[3] = { fp.ok_xr ? g.Px / 2 : g.Px, g.Py, g.Pz };
+    if (fp.ok_xr) {
+        const int Lc = g.Px / 2;
+        std::vector<float2> tx((size_t)Lc);
+        for (int k = 0; k < Lc; ++k) {
+            const long double ang = -3.14159265358979323846264338327950288L * k / Lc;
+            tx[k] = make_float2((float)cosl(ang), (float)sinl(ang));
+        }
+        if (cudaMalloc(&fp.twx, tx.size() * sizeof(float2)) != cudaSuccess ||
+            cudaMemcpy(fp.twx, tx.data(), tx.size() * sizeof(float2), cudaMemcpyHostToDevice) != cudaSuccess) {
+            if (err) *err = "fast plan: twiddle table allocation failed";
+            return false;
+        }
+    }
     for (int a = 0; a < 3; ++a) {
         fp.tw[a] = nullptr;
         if (!ff::split(P[a], &T, &E)) continue;
@@ -350,6 +408,8 @@ inline bool fast_plan_init(FastPlan& fp, const Geom& g, std::string* err)
 inline void fast_plan_destroy(FastPlan& fp)
 {
     for (int a = 0; a < 3; ++a) { cudaFree(fp.tw[a]); fp.tw[a] = nullptr; }
+    cudaFree(fp.twx);
+    fp.twx = nullptr;
     for (int s = 0; s < 4; ++s) {
         if (fp.stream[s]) cudaStreamDestroy(fp.stream[s]);
         if (fp.ev_join[s]) cudaEventDestroy(fp.ev_join[s]);

@@ -257,6 +257,9 @@ FAST_GRIDS = [
     ((192, 96, 32), (3e-9, 3e-9, 3e-9), (0, 0, 0)),     # one factor 3: 384 x 192 x 64, all fast
     ((384, 192, 4), (3e-9, 4e-9, 5e-9), (0, 0, 0)),     # 768 x 384 x 8 (z generic)
     ((384, 192, 1), (4e-9, 4e-9, 2e-9), (1, 1, 0)),     # periodic film 384 x 192, 2D
+    ((768, 24, 2), (3e-9, 3e-9, 3e-9), (0, 0, 0)),      # x = 1536 through the half-length real transform
+    ((1024, 16, 2), (3e-9, 3e-9, 3e-9), (0, 0, 0)),     # x = 2048, same
+    ((1536, 8, 1), (3e-9, 3e-9, 3e-9), (1, 0, 0)),      # x = 1536 periodic (no padding)
 ]
 
 
@@ -278,7 +281,7 @@ def test_fast_passes_match_generic_pass_by_pass(grid, cell, pbc):
     sim.close()
 
 
-@pytest.mark.parametrize("grid,cell,pbc", FAST_GRIDS[:4] + FAST_GRIDS[6:8] + FAST_GRIDS[9:10] + FAST_GRIDS[11:12])
+@pytest.mark.parametrize("grid,cell,pbc", FAST_GRIDS[:4] + FAST_GRIDS[6:8] + FAST_GRIDS[9:10] + FAST_GRIDS[11:13])
 def test_fast_path_matches_oracle(grid, cell, pbc):
     wl = util.small(grid, cell, pbc, T=300.0, seed=77, j=(1e12, -5e11, 2e11), P=0.5, xi=0.04)
     m = wlm.initial_m(wl)
