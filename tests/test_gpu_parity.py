@@ -332,3 +332,88 @@ def test_chunked_l2_resident_passes_match_whole_array_passes(grid, pbc, monkeypa
     ref = util.oracle_problem(wl).demag_field(m.astype(np.float64))
     _cmp(H1.float(), ref, TOL_H)
     sim.close()
+
+
+def test_full_size_headline_grid_sampled_against_the_definition():
+    """BASELINE.json's metric size (512x512x64, the launch configuration bench.py times).  The oracle
+    cannot evaluate a dense state at this size in test time, so: (a) a sparse state of a few source
+    cells -- H_ms is linear, so every output is a sum of a few tensor values the oracle computes one by
+    one from the definition; (b) pin P7: uniform states give the sample's demagnetising factors;
+    (c) pin P18: reciprocity and positive energy for two dense random states (no oracle needed)."""
+    import torch
+    wl = wlm.config(5)
+    Nx, Ny, Nz = wl.grid
+    Ms = wl.mat["Ms"]
+    sim = util.gpu_sim(wl)
+    # (a) sparse sources, incl. the corners that exercise the padding and every sign of the offsets
+    src = [((0, 0, 0), (1.0, 0.0, 0.0)), ((Nx - 1, Ny - 1, Nz - 1), (0.0, 1.0, 0.0)),
+           ((Nx // 2, Ny // 2, Nz // 2), (0.3, -0.5, 0.8)), ((Nx - 1, 0, 5), (0.0, 0.0, 1.0)),
+           ((17, Ny - 3, Nz - 1), (-0.6, 0.6, 0.5)), ((300, 100, 20), (0.2, 0.9, -0.4))]
+    m = torch.zeros((3, Nz, Ny, Nx), dtype=torch.float32, device="cuda")
+    for (x, y, z), vec in src:
+        for c in range(3):
+            m[c, z, y, x] = vec[c]
+    H = sim.demag_field(m)
+    rng = np.random.default_rng(11)
+    obs = []
+    for (x, y, z), _ in src:                       # the sources themselves and their neighbourhoods
+        for d in [(0, 0, 0), (1, 0, 0), (-1, 0, 0), (0, 1, 0), (0, -2, 0), (0, 0, 1), (0, 0, -1), (3, -2, 1),
+                  (-7, 5, -3), (25, 14, 6)]:
+            p = (x + d[0], y + d[1], z + d[2])
+            if 0 <= p[0] < Nx and 0 <= p[1] < Ny and 0 <= p[2] < Nz:
+                obs.append(p)
+    obs += [(0, Ny - 1, 0), (Nx - 1, 0, Nz - 1), (Nx - 1, Ny - 1, 0), (0, 0, Nz - 1)]
+    obs += [tuple(int(v) for v in (rng.integers(0, Nx), rng.integers(0, Ny), rng.integers(0, Nz))) for _ in range(20)]
+    offs = np.array([[o[0] - s[0][0], o[1] - s[0][1], o[2] - s[0][2]] for o in obs for s in src])
+    N6 = orc.tensor_at(offs, wl.cell).reshape(len(obs), len(src), 6)
+    ref = np.zeros((len(obs), 3))
+    for i in range(len(obs)):
+        for k, (_, vec) in enumerate(src):
+            xx, yy, zz, xy, xz, yz = N6[i, k]
+            Nm = np.array([[xx, xy, xz], [xy, yy, yz], [xz, yz, zz]])
+            ref[i] -= Ms * Nm @ np.array(vec)
+    got = np.array([[float(H[c, o[2], o[1], o[0]]) for c in range(3)] for o in obs])
+    scale = float(H.abs().max())
+    assert np.abs(got - ref).max() <= TOL_H * scale, (np.abs(got - ref).max(), scale)
+    big = np.abs(ref) > 1e-4 * scale               # mid-range values must be right on their own scale too
+    assert big.sum() > 30
+    assert (np.abs(got - ref)[big] <= 2e-3 * np.abs(ref)[big] + 2e-7 * scale).all()
+    # (b) uniform states: mean field = - (demagnetising factor of the whole sample) Ms
+    big_cell = tuple(c * n for c, n in zip(wl.cell, wl.grid))
+    Nbig = orc.tensor_at([[0, 0, 0]], big_cell)[0]
+    for a in range(3):
+        m.zero_()
+        m[a] = 1.0
+        Hu = sim.demag_field(m)
+        assert abs(float(Hu[a].double().mean()) / Ms + Nbig[a]) <= 2e-6
+    # (c) reciprocity and positive energy, dense random states
+    g = torch.Generator(device="cuda").manual_seed(5)
+    m1 = torch.nn.functional.normalize(torch.randn((3, Nz, Ny, Nx), device="cuda", generator=g), dim=0)
+    m2 = torch.nn.functional.normalize(torch.randn((3, Nz, Ny, Nx), device="cuda", generator=g), dim=0)
+    H1 = sim.demag_field(m1).double()
+    H2 = sim.demag_field(m2).double()
+    a_, b_ = float((m1.double() * H2).sum()), float((m2.double() * H1).sum())
+    assert abs(a_ - b_) <= 1e-5 * float((m1.double() * H1).sum().abs())
+    assert float((m1.double() * H1).sum()) < 0.0
+    sim.close()
+
+
+def test_full_size_headline_grid_local_terms_and_torque():
+    """Same size: the per-cell tail.  The local field terms (exchange, anisotropy, Zeeman) have no
+    magnetostatic part, so the oracle evaluates them densely; the torque kernel is then checked by
+    feeding the oracle's Landau-Lifshitz formula with the H_eff the GPU returned."""
+    wl = wlm.config(5)
+    m = wlm.initial_m(wl)
+    m64 = m.astype(np.float64)
+    md = util.to_dev(m)
+    mat = util.oracle_material(wl.mat)
+    Hloc = orc.exchange_field(m64, mat, wl.grid, wl.cell, wl.pbc) + orc.anisotropy_field(m64, mat) \
+        + orc.zeeman_field(m64, mat)
+    sim = util.gpu_sim(wl)
+    Hms = sim.demag_field(md).double().cpu().numpy()
+    Heff = sim.heff(md).double().cpu().numpy()
+    s = np.abs(Heff).max()
+    assert np.abs(Heff - (Hms + Hloc)).max() <= TOL_H * s
+    Tref = orc.ll_torque(m64, Heff, mat, wl.grid, wl.cell, wl.pbc)
+    _cmp(sim.torque(md), Tref, TOL_H)
+    sim.close()
