@@ -197,7 +197,9 @@ mm_status mm_kernel_times(mm_ctx* ctx, double sec_out[7], uint64_t count_out[7])
 /* mm_set_fast_path -- bit mask of the passes that may use the size-specialised register FFT kernels
  * when the grid allows (1 forward x, 2 the y passes, 4 last axis + K-hat multiply, 8 inverse x +
  * fused epilogue, 16 the split last pass: inverse x to an H_ms field, then a streaming per-cell
- * kernel; 16 wins over 8); a negative value (and the default) enables all, 0 forces the generic shared-memory
+ * kernel; 16 wins over 8; 32 allows the L2-resident kx chunks of the y / last-axis passes when the
+ * environment variable MM_CHUNK_W asks for them); a negative value (and the default) enables all, 0
+ * forces the generic shared-memory
  * radix-2/3/4/5 kernels.  Both families use the same layouts, so tests compare them pass by pass. */
 mm_status mm_set_fast_path(mm_ctx* ctx, int enable);
 

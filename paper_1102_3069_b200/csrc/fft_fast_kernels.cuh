@@ -88,47 +88,14 @@ struct ColTile {
 };
 
 // ---------------------------------------------------------------------------------------------
-// a2 / a4: y pass on a tile of 8 adjacent kx columns of one (component, z) plane.
-// forward (SGN = -1): specA rows y < Ny (PER: all) -> specB rows ky < Py.  inverse: back, rows y < Ny.
-// `a` and `b` point at column kx0.  thread = (column c = tid & 7, t = tid >> 3); block = 8 T threads;
-// grid = (ceil(ncol/8), 3 Nz).
-// ---------------------------------------------------------------------------------------------
-template <int T, int E, int SGN, bool PER>
-__global__ void __launch_bounds__(8 * T)
-k_y(ColTile ct, float2* __restrict__ a, float2* __restrict__ b, const float2* __restrict__ tw)
-{
-    constexpr bool FWD = SGN < 0;
-    constexpr int NIN = (FWD && !PER) ? E / 2 : E;
-    constexpr int NOUT = (!FWD && !PER) ? E / 2 : E;
-    const int c = threadIdx.x & 7, t = threadIdx.x >> 3;
-    const int col = blockIdx.x * 8 + c;
-    const bool valid = col < ct.ncol;
-    const int cz = blockIdx.y;
-    const size_t s_row = FWD ? ct.a_row : ct.b_row, d_row = FWD ? ct.b_row : ct.a_row;
-    const float2* __restrict__ sp = (FWD ? a + (size_t)cz * ct.a_plane : b + (size_t)cz * ct.b_plane) + col;
-    float2* __restrict__ dp = (FWD ? b + (size_t)cz * ct.b_plane : a + (size_t)cz * ct.a_plane) + col;
-    float2 v[E];
-    if (valid) {
-#pragma unroll
-        for (int j = 0; j < NIN; ++j) v[j] = sp[(size_t)(t + T * j) * s_row];
-    } else {
-#pragma unroll
-        for (int j = 0; j < NIN; ++j) v[j] = make_float2(0.f, 0.f);
-    }
-    fft_line<T, E, SGN, (FWD && !PER)>(v, ff_smem + c, 8, t, tw, SyncBlock());
-    if (valid) {
-#pragma unroll
-        for (int j = 0; j < NOUT; ++j) dp[(size_t)(t + T * j) * d_row] = v[j];
-    }
-}
-
-// ---------------------------------------------------------------------------------------------
-// a2 / a4, persistent and software-pipelined: same arithmetic and thread layout as k_y, but a block
-// loops over tiles (8 columns of one plane) and the NEXT tile's rows arrive by cp.async while the
-// second register FFT and the stores of the current tile run.  The staged tile [rows][8] and the
-// exchange buffer share one shared-memory region (the tile is consumed into registers before the
-// exchange starts, and the copy for the next tile is issued once the exchange has been read back),
-// so the footprint stays that of k_y.  grid = 2 blocks per SM; tile i -> (columns i % ntx, plane i / ntx).
+// a2 / a4: y pass, persistent and software-pipelined.  A tile is 8 adjacent kx columns (64-byte
+// segments) of one (component, z) plane; thread = (column c = tid & 7, t = tid >> 3), block = 8 T.
+// forward (SGN = -1): specA rows y < Ny (PER: all) -> specB rows ky < Py; inverse: back, rows y < Ny;
+// `a` and `b` point at column kx0.  A block loops over tiles and the NEXT tile's rows arrive by
+// cp.async while the second register FFT and the stores of the current tile run.  The staged tile
+// [rows][8] and the exchange buffer share one shared-memory region (the tile is consumed into
+// registers before the exchange starts, and the copy for the next tile is issued once the exchange
+// has been read back).  grid = resident blocks; tile i -> (columns i % ntx, plane i / ntx).
 // ---------------------------------------------------------------------------------------------
 template <int T, int E, int SGN, bool PER>
 __global__ void __launch_bounds__(8 * T, (T == 32) ? 2 : 1)

@@ -12,7 +12,6 @@ struct FastPlan {
     float2* twx;                         // ok_xr: exp(-i pi k / Lc), k < Lc = Px / 2
     float2* tw[3];                       // per axis: tw[k2 * T + t] = exp(-2 pi i t k2 / L)
     int nsm;                             // SM count (persistent grids)
-    int y_pipe;                          // y passes: persistent cp.async-pipelined kernel (env MM_Y_PIPE)
     int mid_pipe;                        // last-axis pass: persistent cp.async-pipelined kernel (env MM_MID_PIPE)
     int chunk_w, nstream;                // chunked a2-a4: columns per chunk (0 = whole-array passes), streams
     cudaStream_t stream[4];
@@ -140,22 +139,15 @@ template <int T, int E, int SGN, bool PER>
 bool launch_y(const FastPlan& fp, const Geom& g, cudaStream_t st, const ColTile& ct, float2* a, float2* b)
 {
     const size_t bytes = (size_t)T * (E + 1) * 8 * sizeof(float2);
-    if (fp.y_pipe) {
-        static bool oncep = ensure_smem(k_y_p<T, E, SGN, PER>, bytes);
-        if (!oncep) return false;
-        const int ntile = ((ct.ncol + 7) / 8) * 3 * g.Nz;
-        int per_sm = (int)((227 * 1024) / (bytes + 1024));
-        const int cap = 2048 / (8 * T) < ((T == 32) ? 2 : 8) ? 2048 / (8 * T) : ((T == 32) ? 2 : 8);
-        if (per_sm > cap) per_sm = cap;
-        if (per_sm < 1) per_sm = 1;
-        const int grid = ntile < fp.nsm * per_sm ? ntile : fp.nsm * per_sm;
-        k_y_p<T, E, SGN, PER><<<grid, 8 * T, bytes, st>>>(ct, 3 * g.Nz, a, b, fp.tw[1]);
-        return true;
-    }
-    static bool once = ensure_smem(k_y<T, E, SGN, PER>, bytes);
-    if (!once) return false;
-    dim3 grid((ct.ncol + 7) / 8, 3 * g.Nz);
-    k_y<T, E, SGN, PER><<<grid, 8 * T, bytes, st>>>(ct, a, b, fp.tw[1]);
+    static bool oncep = ensure_smem(k_y_p<T, E, SGN, PER>, bytes);
+    if (!oncep) return false;
+    const int ntile = ((ct.ncol + 7) / 8) * 3 * g.Nz;
+    int per_sm = (int)((227 * 1024) / (bytes + 1024));
+    const int cap = 2048 / (8 * T) < ((T == 32) ? 2 : 8) ? 2048 / (8 * T) : ((T == 32) ? 2 : 8);
+    if (per_sm > cap) per_sm = cap;
+    if (per_sm < 1) per_sm = 1;
+    const int grid = ntile < fp.nsm * per_sm ? ntile : fp.nsm * per_sm;
+    k_y_p<T, E, SGN, PER><<<grid, 8 * T, bytes, st>>>(ct, 3 * g.Nz, a, b, fp.tw[1]);
     return true;
 }
 
@@ -220,15 +212,22 @@ inline bool fast_fwd_x(const FastPlan& fp, const Geom& g, cudaStream_t st, const
     return r;
 }
 
+// fused inverse x + epilogue (bit 8): power-of-two lengths only; the split pass (bit 16) is the default
 inline bool fast_inv_x(const FastPlan& fp, const Geom& g, cudaStream_t st, const float2* specA, const EpiParams& ep)
 {
     if (!fp.ok_x) return false;
-    bool r = false;
-#define CALL(T, E) r = g.perx ? ff::launch_inv_x<T, E, true>(fp, g, st, specA, ep) \
-                              : ff::launch_inv_x<T, E, false>(fp, g, st, specA, ep)
-    MM_FF_SIZES(g.Px, CALL)
+#define CALL(T, E) return g.perx ? ff::launch_inv_x<T, E, true>(fp, g, st, specA, ep) \
+                                 : ff::launch_inv_x<T, E, false>(fp, g, st, specA, ep)
+    switch (g.Px) {
+    case 64: CALL(8, 8);
+    case 128: CALL(8, 16);
+    case 256: CALL(16, 16);
+    case 512: CALL(16, 32);
+    case 1024: CALL(32, 32);
+    default: break;
+    }
 #undef CALL
-    return r;
+    return false;
 }
 
 // split variant of the last pass, first half: H_ms * scale -> out (a field)
@@ -347,7 +346,6 @@ inline bool fast_plan_init(FastPlan& fp, const Geom& g, std::string* err)
     // B200 at 512x512x64 they give bit-identical results and cut DRAM traffic, but no time, because the
     // y and last-axis passes are bound by instruction issue, not by HBM (profiles/).
     fp.chunk_w = 0;
-    fp.y_pipe = getenv("MM_Y_PIPE") ? atoi(getenv("MM_Y_PIPE")) : 1;
     fp.mid_pipe = getenv("MM_MID_PIPE") ? atoi(getenv("MM_MID_PIPE")) : 1;
     fp.nstream = 3;
     if (getenv("MM_CHUNK_W")) fp.chunk_w = atoi(getenv("MM_CHUNK_W"));
