@@ -106,6 +106,9 @@ struct mm_ctx {
     std::string err;
     KTimer kt;
     int fast;
+    cudaStream_t gstream;   // the context's own stream for graph capture / replay (created on first use)
+    cudaEvent_t gev[2];
+    int use_graph;    // mm_steps_fixed may replay a captured step (env MM_GRAPH=0 switches it off)
     // device
     float* khat;
     float2 *specA, *specB;
@@ -504,6 +507,9 @@ mm_status mm_create(mm_ctx** out, const int grid[3], const double cellsize[3], c
     c->mhost = nullptr;
     c->hfield = nullptr;
     c->fast = FAST_ALL;
+    c->gstream = nullptr;
+    c->gev[0] = c->gev[1] = nullptr;
+    c->use_graph = getenv("MM_GRAPH") ? atoi(getenv("MM_GRAPH")) : 1;
     c->khat = nullptr; c->specA = c->specB = nullptr;
     for (int a = 0; a < 3; ++a) c->tw[a] = nullptr;
     for (int i = 0; i < 7; ++i) c->kb[i] = nullptr;
@@ -577,8 +583,8 @@ mm_status mm_demag_init(mm_ctx* c)
     CUDA_TRY(c, cudaMalloc(&c->mtmp, fb));
     CUDA_TRY(c, cudaMalloc(&c->mhost, fb));
     CUDA_TRY(c, cudaMalloc(&c->hfield, fb));
-    CUDA_TRY(c, cudaMalloc(&c->maxbits, sizeof(unsigned int)));
-    CUDA_TRY(c, cudaMemset(c->maxbits, 0, sizeof(unsigned int)));
+    CUDA_TRY(c, cudaMalloc(&c->maxbits, 2 * sizeof(unsigned int)));     // [0] per step, [1] running maximum
+    CUDA_TRY(c, cudaMemset(c->maxbits, 0, 2 * sizeof(unsigned int)));
     mm_status s;
     if ((s = set_smem(c, k_gen_fwd_x)) != MM_OK) return s;
     if ((s = set_smem(c, k_gen_y<-1>)) != MM_OK) return s;
@@ -674,6 +680,74 @@ mm_status mm_step(mm_ctx* c, float* m_dev, mm_method method, double* dt_inout, d
     return MM_OK;
 }
 
+// running maximum over the steps of one mm_steps_fixed call (bit patterns: NaN / Inf compare largest)
+__global__ void k_track_max(const unsigned int* __restrict__ maxbits, unsigned int* __restrict__ run)
+{
+    atomicMax(run, *maxbits);
+}
+
+static mm_status steps_fixed_impl(mm_ctx* c, float* m_dev, mm_method method, const Tableau& tab, double dt, int n,
+                                  bool graph_ok, double* t_inout, double* max_err_out)
+{
+    mm_status s = MM_OK;
+    unsigned int* run = c->maxbits + 1;
+    CUDA_TRY(c, cudaMemsetAsync(run, 0, sizeof(unsigned int), c->stream));
+    auto one_step = [&]() -> mm_status {
+        float* newstate = nullptr;
+        mm_status st = enqueue_step(c, m_dev, method, tab, dt, false, &newstate);
+        if (st == MM_OK) st = commit_step(c, m_dev, method, tab, newstate);
+        if (st != MM_OK) return st;
+        k_track_max<<<1, 1, 0, c->stream>>>(c->maxbits, run);
+        c->kt.launches++;
+        return MM_OK;
+    };
+    int done = 0;
+    if (graph_ok) {
+        if ((s = one_step()) != MM_OK) return s;          // also sets the kernels' attributes outside the capture
+        done = 1;
+        cudaGraph_t graph = nullptr;
+        cudaGraphExec_t exec = nullptr;
+        const uint64_t l0 = c->kt.launches;
+        if (cudaStreamBeginCapture(c->stream, cudaStreamCaptureModeThreadLocal) == cudaSuccess) {
+            const mm_status sc = one_step();
+            const cudaError_t ec = cudaStreamEndCapture(c->stream, &graph);
+            if (sc == MM_OK && ec == cudaSuccess && graph &&
+                cudaGraphInstantiate(&exec, graph, 0) == cudaSuccess) {
+                const uint64_t per = c->kt.launches - l0;
+                c->kt.launches = l0;
+                c->step_index--;                           // the captured step has not run yet
+                for (; done < n; ++done) {
+                    if (cudaGraphLaunch(exec, c->stream) != cudaSuccess) break;
+                    c->kt.launches += per;
+                    c->step_index++;
+                }
+            } else {
+                c->kt.launches = l0;
+                c->step_index--;
+            }
+            if (exec) cudaGraphExecDestroy(exec);
+            if (graph) cudaGraphDestroy(graph);
+        }
+        cudaGetLastError();                                // a refused capture must not surface later
+    }
+    for (; done < n; ++done)
+        if ((s = one_step()) != MM_OK) return s;
+    unsigned int bits = 0;
+    if (n > 0) {
+        CUDA_TRY(c, cudaMemcpyAsync(&bits, run, sizeof(unsigned int), cudaMemcpyDeviceToHost, c->stream));
+        CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+    }
+    float f;
+    std::memcpy(&f, &bits, sizeof(f));
+    if (!std::isfinite(f)) {
+        c->k0_valid = false;
+        return fail(c, MM_ENUMERIC, "non-finite value met by the max-norm reduction");
+    }
+    if (t_inout) *t_inout += dt * n;
+    if (max_err_out) *max_err_out = tab.embedded ? (double)f : 0.0;
+    return MM_OK;
+}
+
 mm_status mm_steps_fixed(mm_ctx* c, float* m_dev, mm_method method, double dt, int n, double* t_inout,
                          double* max_err_out)
 {
@@ -682,35 +756,30 @@ mm_status mm_steps_fixed(mm_ctx* c, float* m_dev, mm_method method, double dt, i
     if (!m_dev || !(dt > 0) || n < 0) return fail(c, MM_EINVAL, "bad m_dev / dt / n");
     const Tableau tab = make_tableau(method);
     if (tab.S == 0) return fail(c, MM_EINVAL, "unknown method");
-    std::vector<unsigned int> bits((size_t)n, 0u);
-    unsigned int* dbits = nullptr;
-    if (n > 0) CUDA_TRY(c, cudaMalloc(&dbits, (size_t)n * sizeof(unsigned int)));
-    for (int i = 0; i < n; ++i) {
-        float* newstate = nullptr;
-        s = enqueue_step(c, m_dev, method, tab, dt, false, &newstate);
-        if (s == MM_OK) s = commit_step(c, m_dev, method, tab, newstate);
-        if (s != MM_OK) { cudaFree(dbits); return s; }
-        cudaMemcpyAsync(dbits + i, c->maxbits, sizeof(unsigned int), cudaMemcpyDeviceToDevice, c->stream);
-    }
-    if (n > 0) {
-        cudaMemcpyAsync(bits.data(), dbits, (size_t)n * sizeof(unsigned int), cudaMemcpyDeviceToHost, c->stream);
-        cudaError_t e = cudaStreamSynchronize(c->stream);
-        cudaFree(dbits);
-        if (e != cudaSuccess) return fail(c, MM_ECUDA, cudaGetErrorString(e));
-    }
-    double maxerr = 0.0;
-    for (int i = 0; i < n; ++i) {
-        float f;
-        std::memcpy(&f, &bits[i], sizeof(f));
-        if (!std::isfinite(f)) {
-            c->k0_valid = false;
-            return fail(c, MM_ENUMERIC, "non-finite value met by the max-norm reduction");
+    // Every step of a fixed-step, non-FSAL method without thermal field enqueues the same launches with
+    // the same arguments: capture the second step into a CUDA graph and replay it (launch-bound grids).
+    // The caller's stream may be the legacy default stream, which cannot be captured: the sequence runs
+    // on a stream of the context's own, ordered after and before the caller's stream with events.
+    const bool chunked = (c->fast & FAST_CHUNK) && c->fp.chunk_w > 0 && c->g.Pz > 1;
+    bool graph_ok = c->use_graph && n >= 4 && !tab.fsal && !(c->mat.T > 0) && !c->kt.on && !chunked;
+    if (graph_ok && !c->gstream) {
+        if (cudaStreamCreateWithFlags(&c->gstream, cudaStreamNonBlocking) != cudaSuccess ||
+            cudaEventCreateWithFlags(&c->gev[0], cudaEventDisableTiming) != cudaSuccess ||
+            cudaEventCreateWithFlags(&c->gev[1], cudaEventDisableTiming) != cudaSuccess) {
+            cudaGetLastError();
+            graph_ok = false;
         }
-        if (tab.embedded && f > maxerr) maxerr = f;
     }
-    if (t_inout) *t_inout += dt * n;
-    if (max_err_out) *max_err_out = maxerr;
-    return MM_OK;
+    if (!graph_ok) return steps_fixed_impl(c, m_dev, method, tab, dt, n, false, t_inout, max_err_out);
+    cudaStream_t user = c->stream;
+    CUDA_TRY(c, cudaEventRecord(c->gev[0], user));
+    CUDA_TRY(c, cudaStreamWaitEvent(c->gstream, c->gev[0], 0));
+    c->stream = c->gstream;
+    s = steps_fixed_impl(c, m_dev, method, tab, dt, n, true, t_inout, max_err_out);
+    c->stream = user;
+    cudaEventRecord(c->gev[1], c->gstream);
+    cudaStreamWaitEvent(user, c->gev[1], 0);
+    return s;
 }
 
 mm_status mm_steps_fixed_host(mm_ctx* c, float* m_host, mm_method method, double dt, int n, double* t_inout,
@@ -870,6 +939,9 @@ void mm_destroy(mm_ctx* c)
         delete[] c->kt.ev[k];
     }
     cudaFree(c->maxbits);
+    if (c->gstream) cudaStreamDestroy(c->gstream);
+    for (int i = 0; i < 2; ++i)
+        if (c->gev[i]) cudaEventDestroy(c->gev[i]);
     fast_plan_destroy(c->fp);
     delete c;
 }

@@ -417,3 +417,22 @@ def test_full_size_headline_grid_local_terms_and_torque():
     Tref = orc.ll_torque(m64, Heff, mat, wl.grid, wl.cell, wl.pbc)
     _cmp(sim.torque(md), Tref, TOL_H)
     sim.close()
+
+
+@pytest.mark.parametrize("method", ["rk1", "rk4"])
+def test_graph_replayed_steps_equal_plain_launches(method, monkeypatch):
+    """mm_steps_fixed replays a captured step for the fixed-step, non-FSAL methods: same bits as plain launches."""
+    wl = util.small((32, 32, 1), (4e-9, 4e-9, 4e-9), alpha=0.5)
+    m = wlm.initial_m(wl)
+    out = []
+    for flag in ("1", "0"):
+        monkeypatch.setenv("MM_GRAPH", flag)
+        sim = util.gpu_sim(wl)
+        md = util.to_dev(m)
+        t, _ = sim.steps_fixed(md, method, 1e-13, 25)
+        l0 = sim.launch_count()
+        t, _ = sim.steps_fixed(md, method, 1e-13, 3)         # below the replay threshold
+        assert abs(t - 3e-13) < 1e-25 and sim.launch_count() > l0
+        out.append(md.cpu().numpy().copy())
+        sim.close()
+    assert np.array_equal(out[0], out[1])
