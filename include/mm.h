@@ -140,6 +140,19 @@ mm_status mm_step(mm_ctx* ctx, float* m_dev, mm_method method, double* dt_inout,
 mm_status mm_steps_fixed(mm_ctx* ctx, float* m_dev, mm_method method, double dt, int n,
                          double* t_inout, double* max_err_out);
 
+/* mm_steps_adaptive -- ntrials trial steps of an embedded method (MM_RKDP, MM_RK23, MM_RK12) with the
+ * step controller of reading A10 running ON THE DEVICE (step a11 of DESIGN.md):
+ * the error norm, the accept / reject decision, the new step length, the time and the commit of an
+ * accepted state never leave the GPU, so the whole sequence is enqueued without a host synchronisation
+ * per step (mm_step synchronises once per step).  Synchronises once at the end to return the scalars.
+ *   dt_inout       host: first trial step length in, next proposed step length out (seconds)
+ *   t_inout        host, may be NULL: time in, time after the accepted steps out
+ *   naccepted_out  host, may be NULL: how many of the ntrials steps were accepted
+ *   last_err_out   host, may be NULL: error estimate of the last trial step
+ * The cell count must be divisible by 4.  Thermal field: MM_EUNSUPPORTED (reading A6). */
+mm_status mm_steps_adaptive(mm_ctx* ctx, float* m_dev, mm_method method, int ntrials, double* dt_inout,
+                            double tol, double* t_inout, int* naccepted_out, double* last_err_out);
+
 /* mm_steps_fixed_host -- the same as mm_steps_fixed for a state held in HOST memory (pinned memory
  * gives the full PCIe rate): m_host is copied to the device, advanced n steps and copied back, all on
  * the context's stream; returns after the copy back.  This is the end-to-end call bench.py times. */

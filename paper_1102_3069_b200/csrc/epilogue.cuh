@@ -152,16 +152,17 @@ __device__ __forceinline__ float epilogue_finish_v(const EpiParams& p, size_t id
         return 0.f;
     }
     // ---- Runge-Kutta stage combine ----
+    const float ds = p.dt_scale ? __ldg(p.dt_scale) : 1.0f;     // step length kept on the device (a11)
     float r[3][V];
     if (p.m_out) {
         float acc[3][V];
 #pragma unroll
         for (int c = 0; c < 3; ++c)
 #pragma unroll
-            for (int u = 0; u < V; ++u) acc[c][u] = p.a_self * k[c][u];
+            for (int u = 0; u < V; ++u) acc[c][u] = ds * p.a_self * k[c][u];
         for (int j = 0; j < p.na; ++j) {
             const float* __restrict__ kj = p.ka[j];
-            const float aj = p.a[j];
+            const float aj = ds * p.a[j];
 #pragma unroll
             for (int c = 0; c < 3; ++c) {
                 float t[V];
@@ -191,10 +192,10 @@ __device__ __forceinline__ float epilogue_finish_v(const EpiParams& p, size_t id
 #pragma unroll
         for (int c = 0; c < 3; ++c)
 #pragma unroll
-            for (int u = 0; u < V; ++u) e[c][u] = p.e_self * k[c][u];
+            for (int u = 0; u < V; ++u) e[c][u] = ds * p.e_self * k[c][u];
         for (int j = 0; j < p.ne; ++j) {
             const float* __restrict__ kj = p.ke[j];
-            const float ej = p.e[j];
+            const float ej = ds * p.e[j];
 #pragma unroll
             for (int c = 0; c < 3; ++c) {
                 float t[V];

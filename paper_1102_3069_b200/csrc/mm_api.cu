@@ -120,6 +120,7 @@ struct mm_ctx {
     float* hfield;    // H_ms in units of Ms between the two halves of the split last pass
     float* mhost;     // device copy of a caller's host state (mm_steps_fixed_host)
     unsigned int* maxbits;
+    StepCtl* ctl;     // device-side step controller state (a11)
     // stepper state
     uint64_t step_index;
     bool k0_valid;
@@ -348,8 +349,10 @@ double gamma0_of(const mm_ctx* c) { return c->mat.gamma0 > 0 ? c->mat.gamma0 : G
 
 // m_out = [normalise](m_n + sum_j a_j k_j): used when an evaluation is skipped (FSAL reuse).
 __global__ void k_combine(size_t n, const float* __restrict__ m_n, float* __restrict__ m_out, int na,
-                          float a0, float a1, const float* __restrict__ k0, const float* __restrict__ k1)
+                          float a0, float a1, const float* __restrict__ k0, const float* __restrict__ k1,
+                          const float* __restrict__ dt_scale)
 {
+    if (dt_scale) { a0 *= *dt_scale; a1 *= *dt_scale; }
     for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < 3 * n;
          i += (size_t)gridDim.x * blockDim.x) {
         float v = m_n[i] + a0 * k0[i];
@@ -366,12 +369,14 @@ __global__ void k_copy4(const float4* __restrict__ src, float4* __restrict__ dst
 
 // One stage of `tab` (0-based s).  Enqueues only.
 mm_status run_stage(mm_ctx* c, float* m_dev, const Tableau& tab, int s, double dt, uint64_t step,
-                    bool adaptive_target)
+                    bool adaptive_target, bool dev_dt = false)
 {
     const int S = tab.S;
-    const double dtr = dt * gamma0_of(c) * c->mat.Ms;
+    // dev_dt: the step length lives on the device (StepCtl::dtr); the tableau goes in unscaled
+    const double dtr = dev_dt ? 1.0 : dt * gamma0_of(c) * c->mat.Ms;
     EpiParams ep;
     std::memset(&ep, 0, sizeof(ep));
+    if (dev_dt) ep.dt_scale = &c->ctl->dtr;
     fill_material(c, ep, step, dt);
     ep.mode = EPI_STAGE;
     ep.m_in = s == 0 ? m_dev : c->ms[(s - 1) & 1];
@@ -425,7 +430,7 @@ mm_status run_stage(mm_ctx* c, float* m_dev, const Tableau& tab, int s, double d
 // One trial step; enqueues everything, no synchronisation.  After it, maxbits holds the error
 // estimate and the new state is in *newstate (m_dev itself when written in place).
 mm_status enqueue_step(mm_ctx* c, float* m_dev, mm_method method, const Tableau& tab, double dt,
-                       bool adaptive_target, float** newstate)
+                       bool adaptive_target, float** newstate, bool dev_dt = false)
 {
     const int S = tab.S;
     const size_t n = ncell(c->g);
@@ -434,15 +439,15 @@ mm_status enqueue_step(mm_ctx* c, float* m_dev, mm_method method, const Tableau&
     int s0 = 0;
     if (tab.fsal && c->k0_valid && c->k0_method == (int)method) {
         // k_1 of this step is the last stage of the previous accepted step: skip the evaluation
-        const double dtr = dt * gamma0_of(c) * c->mat.Ms;
+        const double dtr = dev_dt ? 1.0 : dt * gamma0_of(c) * c->mat.Ms;
         c->kt.begin(KT_OTHER);
         k_combine<<<148 * 8, 256, 0, c->stream>>>(n, m_dev, c->ms[0], 1, (float)(dtr * tab.A[1][0]), 0.f,
-                                                  c->kb[0], c->kb[0]);
+                                                  c->kb[0], c->kb[0], dev_dt ? &c->ctl->dtr : nullptr);
         c->kt.end(KT_OTHER);
         s0 = 1;
     }
     for (int s = s0; s < S; ++s) {
-        mm_status st = run_stage(c, m_dev, tab, s, dt, step, adaptive_target);
+        mm_status st = run_stage(c, m_dev, tab, s, dt, step, adaptive_target, dev_dt);
         if (st != MM_OK) return st;
     }
     if (tab.fsal) *newstate = c->ms[(S - 2) & 1];
@@ -515,6 +520,7 @@ mm_status mm_create(mm_ctx** out, const int grid[3], const double cellsize[3], c
     for (int i = 0; i < 7; ++i) c->kb[i] = nullptr;
     c->ms[0] = c->ms[1] = c->mtmp = nullptr;
     c->maxbits = nullptr;
+    c->ctl = nullptr;
     c->step_index = 0;
     c->k0_valid = false;
     c->k0_method = -1;
@@ -585,6 +591,8 @@ mm_status mm_demag_init(mm_ctx* c)
     CUDA_TRY(c, cudaMalloc(&c->hfield, fb));
     CUDA_TRY(c, cudaMalloc(&c->maxbits, 2 * sizeof(unsigned int)));     // [0] per step, [1] running maximum
     CUDA_TRY(c, cudaMemset(c->maxbits, 0, 2 * sizeof(unsigned int)));
+    CUDA_TRY(c, cudaMalloc(&c->ctl, sizeof(StepCtl)));
+    CUDA_TRY(c, cudaMemset(c->ctl, 0, sizeof(StepCtl)));
     mm_status s;
     if ((s = set_smem(c, k_gen_fwd_x)) != MM_OK) return s;
     if ((s = set_smem(c, k_gen_y<-1>)) != MM_OK) return s;
@@ -782,6 +790,85 @@ mm_status mm_steps_fixed(mm_ctx* c, float* m_dev, mm_method method, double dt, i
     return s;
 }
 
+// ---- a11 on the device: accept / reject and the next step length (reading A10), one thread ----
+__global__ void k_step_control(StepCtl* __restrict__ ctl, const unsigned int* __restrict__ maxbits)
+{
+    const float ef = __uint_as_float(*maxbits);
+    const double err = (double)ef;
+    ctl->ntrial++;
+    ctl->last_err = err;
+    if (!isfinite(ef)) { ctl->nonfinite = 1; ctl->last_accept = 0; return; }
+    const int accept = err <= ctl->tol;
+    const double fac = err == 0.0 ? 2.0 : fmin(2.0, fmax(0.2, 0.8 * pow(ctl->tol / err, 1.0 / ctl->order)));
+    if (accept) { ctl->t += ctl->dt; ctl->naccept++; }
+    ctl->dt *= fac;
+    ctl->dtr = (float)(ctl->dt * ctl->g0Ms);
+    ctl->last_accept = accept;
+}
+
+// commit of a trial step decided on the device: new state -> m, last stage -> first stage (FSAL)
+__global__ void k_step_commit(size_t n4, const float4* __restrict__ newstate, float4* __restrict__ m,
+                              const float4* __restrict__ klast, float4* __restrict__ kfirst,
+                              const StepCtl* __restrict__ ctl)
+{
+    if (!ctl->last_accept) return;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n4; i += (size_t)gridDim.x * blockDim.x) {
+        m[i] = newstate[i];
+        if (kfirst) kfirst[i] = klast[i];
+    }
+}
+
+mm_status mm_steps_adaptive(mm_ctx* c, float* m_dev, mm_method method, int ntrials, double* dt_inout, double tol,
+                            double* t_inout, int* naccepted_out, double* last_err_out)
+{
+    mm_status s = check_ready(c);
+    if (s != MM_OK) return s;
+    if (!m_dev || !dt_inout || !(*dt_inout > 0) || ntrials < 0 || !(tol > 0))
+        return fail(c, MM_EINVAL, "bad m_dev / dt / ntrials / tol");
+    const Tableau tab = make_tableau(method);
+    if (tab.S == 0 || !tab.embedded) return fail(c, MM_EINVAL, "mm_steps_adaptive needs an embedded method");
+    if (c->mat.T > 0) return fail(c, MM_EUNSUPPORTED, "thermal field needs a fixed-step method (reading A6)");
+    if (ncell(c->g) % 4 != 0) return fail(c, MM_EUNSUPPORTED, "mm_steps_adaptive needs a cell count divisible by 4");
+    StepCtl h;
+    std::memset(&h, 0, sizeof(h));
+    h.t = t_inout ? *t_inout : 0.0;
+    h.dt = *dt_inout;
+    h.tol = tol;
+    h.g0Ms = gamma0_of(c) * c->mat.Ms;
+    h.order = method == MM_RKDP ? 5.0 : (method == MM_RK23 ? 3.0 : 2.0);
+    h.dtr = (float)(h.dt * h.g0Ms);
+    CUDA_TRY(c, cudaMemcpyAsync(c->ctl, &h, sizeof(h), cudaMemcpyHostToDevice, c->stream));
+    const size_t n4 = 3 * ncell(c->g) / 4;
+    for (int i = 0; i < ntrials; ++i) {
+        float* newstate = nullptr;
+        s = enqueue_step(c, m_dev, method, tab, 0.0, true, &newstate, true);
+        if (s != MM_OK) return s;
+        k_step_control<<<1, 1, 0, c->stream>>>(c->ctl, c->maxbits);
+        const bool fs = tab.fsal;
+        k_step_commit<<<148 * 8, 256, 0, c->stream>>>(n4, (const float4*)newstate, (float4*)m_dev,
+                                                       fs ? (const float4*)c->kb[tab.S - 1] : nullptr,
+                                                       fs ? (float4*)c->kb[0] : nullptr, c->ctl);
+        c->kt.launches += 2;
+        if (fs) {
+            // accepted: k_1 <- k_S; rejected: k_1 = f(m_n) is still in place -- valid either way
+            c->k0_valid = true;
+            c->k0_method = (int)method;
+        }
+    }
+    CUDA_TRY(c, cudaMemcpyAsync(&h, c->ctl, sizeof(h), cudaMemcpyDeviceToHost, c->stream));
+    CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+    c->step_index += (uint64_t)h.naccept;
+    *dt_inout = h.dt;
+    if (t_inout) *t_inout = h.t;
+    if (naccepted_out) *naccepted_out = h.naccept;
+    if (last_err_out) *last_err_out = h.last_err;
+    if (h.nonfinite) {
+        c->k0_valid = false;
+        return fail(c, MM_ENUMERIC, "non-finite value met by the max-norm reduction");
+    }
+    return MM_OK;
+}
+
 mm_status mm_steps_fixed_host(mm_ctx* c, float* m_host, mm_method method, double dt, int n, double* t_inout,
                               double* max_err_out)
 {
@@ -939,6 +1026,7 @@ void mm_destroy(mm_ctx* c)
         delete[] c->kt.ev[k];
     }
     cudaFree(c->maxbits);
+    cudaFree(c->ctl);
     if (c->gstream) cudaStreamDestroy(c->gstream);
     for (int i = 0; i < 2; ++i)
         if (c->gev[i]) cudaEventDestroy(c->gev[i]);

@@ -61,6 +61,7 @@ struct EpiParams {
     float e[MM_MAXK];
     const float* ke[MM_MAXK];
     unsigned int* maxbits;   // atomicMax target (bit pattern of a non-negative float)
+    const float* dt_scale;   // device scalar dt gamma0 Ms multiplying a_self, a[], e_self, e[] (NULL: already folded in)
 };
 
 __device__ __forceinline__ float2 cadd(float2 a, float2 b) { return make_float2(a.x + b.x, a.y + b.y); }
@@ -102,6 +103,18 @@ struct KTimer {
         }
         cudaEventRecord(ev[cat][nev[cat]++], stream);
     }
+};
+
+// device-side state of the step controller (reading A10; step a11): lives in the context
+struct StepCtl {
+    double t, dt, tol;       // seconds
+    double g0Ms;             // gamma0 Ms: reduced time step = dt * g0Ms
+    double order;            // exponent 1/order in the step-size rule
+    double last_err;
+    float dtr;               // (float)(dt * g0Ms), what the kernels multiply the tableau by
+    int last_accept;
+    int naccept, ntrial;
+    int nonfinite;
 };
 
 }  // namespace mm

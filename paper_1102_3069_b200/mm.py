@@ -68,6 +68,7 @@ def lib():
         L.mm_step.argtypes = [vp, vp, C.c_int, d3, C.c_double, d3, d3, i3]
         L.mm_steps_fixed.argtypes = [vp, vp, C.c_int, C.c_double, C.c_int, d3, d3]
         L.mm_steps_fixed_host.argtypes = [vp, vp, C.c_int, C.c_double, C.c_int, d3, d3]
+        L.mm_steps_adaptive.argtypes = [vp, vp, C.c_int, C.c_int, d3, C.c_double, d3, i3, d3]
         L.mm_kernel_timing.argtypes = [vp, C.c_int]
         L.mm_kernel_times.argtypes = [vp, d3, C.POINTER(C.c_uint64)]
         L.mm_fused_eval.argtypes = [vp, vp, C.c_int, C.c_int, C.c_double, C.c_uint64]
@@ -188,6 +189,13 @@ class Sim:
         self._chk(self.L.mm_steps_fixed(self.ctx, self._dev(m), METHODS[method], dt, n, C.byref(tv),
                                         C.byref(err)))
         return tv.value, err.value
+
+    def steps_adaptive(self, m, method, ntrials, dt, tol=1e-5, t=0.0):
+        """ntrials trial steps with the step controller on the device; returns (naccepted, last_err, dt_next, t)."""
+        dtv, tv, err, nacc = C.c_double(dt), C.c_double(t), C.c_double(0.0), C.c_int(0)
+        self._chk(self.L.mm_steps_adaptive(self.ctx, self._dev(m), METHODS[method], int(ntrials), C.byref(dtv), tol,
+                                           C.byref(tv), C.byref(nacc), C.byref(err)))
+        return nacc.value, err.value, dtv.value, tv.value
 
     def steps_fixed_host(self, m_host, method, dt, n, t=0.0):
         """m_host: CPU float32 tensor (pinned for full PCIe rate), updated in place."""

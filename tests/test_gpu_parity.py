@@ -436,3 +436,38 @@ def test_graph_replayed_steps_equal_plain_launches(method, monkeypatch):
         out.append(md.cpu().numpy().copy())
         sim.close()
     assert np.array_equal(out[0], out[1])
+
+
+@pytest.mark.parametrize("method", ["rkdp", "rk23"])
+def test_device_side_step_controller_follows_the_host_controlled_run(method):
+    """Step a11: mm_steps_adaptive keeps error norm, accept / reject, dt and t on the device; it must
+    take the same decisions as mm_step (one host sync per step) and end in the same state."""
+    wl = util.small((24, 12, 8), init="tilted", alpha=0.02, Bext=(-0.0246, 0.0043, 0.0), Ku=0.0)
+    m = wlm.initial_m(wl)
+    tol, ntr = 1e-5, 40
+    sim = util.gpu_sim(wl)
+    md = util.to_dev(m)
+    dt, t, nacc = 4e-13, 0.0, 0              # starts too long: the first trials are rejected
+    for _ in range(ntr):
+        acc, err, dt, t = sim.step(md, method, dt, tol, t)
+        nacc += int(acc)
+    ref = md.double().cpu().numpy()
+    assert 0 < nacc < ntr
+    sim2 = util.gpu_sim(wl)
+    md2 = util.to_dev(m)
+    nacc2, err2, dt2, t2 = sim2.steps_adaptive(md2, method, ntr, 4e-13, tol, 0.0)
+    assert nacc2 == nacc
+    # the tableau is scaled by dt in fp32 on the device and in fp64 on the host: the error estimates, hence
+    # the step lengths, agree to a few 1e-5
+    assert abs(t2 - t) <= 1e-4 * t and abs(dt2 - dt) <= 2e-3 * dt
+    assert abs(err2 - err) <= 0.02 * err + 1e-12
+    assert np.abs(md2.double().cpu().numpy() - ref).max() <= 1e-5
+    # split into two calls: the FSAL stage and the device scalars carry over
+    sim3 = util.gpu_sim(wl)
+    md3 = util.to_dev(m)
+    n1, _, dt3, t3 = sim3.steps_adaptive(md3, method, 15, 4e-13, tol, 0.0)
+    n2, _, dt3, t3 = sim3.steps_adaptive(md3, method, ntr - 15, dt3, tol, t3)
+    assert n1 + n2 == nacc and abs(t3 - t) <= 1e-4 * t
+    assert np.abs(md3.double().cpu().numpy() - ref).max() <= 1e-5
+    for s_ in (sim, sim2, sim3):
+        s_.close()
