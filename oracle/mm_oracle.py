@@ -467,6 +467,26 @@ def _F(*args):
 TABLEAUX = {
     # RK1: Euler's method
     "rk1": ([Fraction(0)], [[]], [Fraction(1)], None),
+    # RK2: Heun's method
+    "rk2": (_F(0, 1), [[], _F(1)], _F((1, 2), (1, 2)), None),
+    # RK12: Heun-Euler, adaptive: Heun's solution, Euler's as the embedded one
+    "rk12": (_F(0, 1), [[], _F(1)], _F((1, 2), (1, 2)), _F(1, 0)),
+    # RK3: Kutta's third-order method
+    "rk3": (_F(0, (1, 2), 1), [[], _F((1, 2)), _F(-1, 2)], _F((1, 6), (2, 3), (1, 6)), None),
+    # RK23: Bogacki-Shampine 3(2), adaptive, first-same-as-last
+    "rk23": (_F(0, (1, 2), (3, 4), 1),
+             [[], _F((1, 2)), _F(0, (3, 4)), _F((2, 9), (1, 3), (4, 9))],
+             _F((2, 9), (1, 3), (4, 9), 0), _F((7, 24), (1, 4), (1, 3), (1, 8))),
+    # RKCK: Cash-Karp 5(4), adaptive
+    "rkck": (_F(0, (1, 5), (3, 10), (3, 5), 1, (7, 8)),
+             [[],
+              _F((1, 5)),
+              _F((3, 40), (9, 40)),
+              _F((3, 10), (-9, 10), (6, 5)),
+              _F((-11, 54), (5, 2), (-70, 27), (35, 27)),
+              _F((1631, 55296), (175, 512), (575, 13824), (44275, 110592), (253, 4096))],
+             _F((37, 378), 0, (250, 621), (125, 594), 0, (512, 1771)),
+             _F((2825, 27648), 0, (18575, 48384), (13525, 55296), (277, 14336), (1, 4))),
     # RK4: classical Runge-Kutta
     "rk4": (_F(0, (1, 2), (1, 2), 1),
             [[], _F((1, 2)), _F(0, (1, 2)), _F(0, 0, 1)],
@@ -520,6 +540,56 @@ def rkdp_step(f, m, dt, k1=None):
     e = sum(float(b[j] - bs[j]) * k[j] for j in range(7) if b[j] != bs[j])
     err = dt * float(np.max(np.sqrt(np.sum(e * e, axis=0))))
     return m_new, err, k[6]
+
+
+# order p of the propagated solution: the exponent of the step-size rule is 1/p (reading A10)
+ORDER = {"rk1": 1, "rk2": 2, "rk12": 2, "rk3": 3, "rk23": 3, "rk4": 4, "rkck": 5, "rkdp": 5}
+FSAL = ("rk23", "rkdp")      # last row of A equals b: the last stage is f(new state)
+
+
+def rk_step(f, m, dt, name, k1=None):
+    """One step of any tableau of TABLEAUX, stage by stage as the textbook states it
+    (reading A10).  k_s = f(m + dt sum_j a_sj k_j), no normalisation between
+    stages; m_new = normalise(m + dt sum_s b_s k_s).  For the first-same-as-last pairs the last
+    stage is evaluated on the renormalised m_new and returned for reuse as the next k_1.
+    Embedded pairs: err = dt max_i || sum_s (b_s - b*_s) k_s(i) ||_2, else err = None.
+    Returns (m_new, err, k_last)."""
+    c, A, b, bs = TABLEAUX[name]
+    S = len(b)
+    fsal = name in FSAL
+    k = [f(m) if k1 is None else k1]
+    for s in range(1, S - 1 if fsal else S):
+        ms = m + dt * sum(float(A[s][j]) * k[j] for j in range(s) if A[s][j] != 0)
+        k.append(f(ms))
+    nb = S - 1 if fsal else S
+    m_new = _normalise(m + dt * sum(float(b[j]) * k[j] for j in range(nb) if b[j] != 0))
+    if fsal:
+        k.append(f(m_new))
+    err = None
+    if bs is not None:
+        e = sum(float(b[j] - bs[j]) * k[j] for j in range(S) if b[j] != bs[j])
+        err = dt * float(np.max(np.sqrt(np.sum(e * e, axis=0))))
+    return m_new, err, k[-1]
+
+
+def rk_controller(dt, err, tol, name):
+    """Reading A10 for any embedded pair: accept iff err <= tol;
+    dt <- dt * clamp(0.8 (tol/err)^(1/p), 0.2, 2), p = ORDER[name] (err = 0 => factor 2)."""
+    accept = err <= tol
+    fac = 2.0 if err == 0.0 else min(2.0, max(0.2, 0.8 * (tol / err) ** (1.0 / ORDER[name])))
+    return accept, dt * fac
+
+
+def max_dm_step_length(f, m, max_dm):
+    """PAPER.md:141 "a fixed maximum variation of m per step" for the fixed-step methods:
+    dt = max_dm / max_i ||dm/dt(i)||_2, evaluated on the state at the start of the step."""
+    k = f(m)
+    return max_dm / float(np.max(np.sqrt(np.sum(k * k, axis=0)))), k
+
+
+def average_m(m):
+    """<m> over all cells (PAPER.md:273 output quantity)."""
+    return m.reshape(3, -1).mean(axis=1)
 
 
 def rkdp_controller(dt, err, tol):

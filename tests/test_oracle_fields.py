@@ -272,7 +272,9 @@ def _order_conditions(c, A, b, order):
 
 
 def test_butcher_tableaux_satisfy_order_conditions_exactly():
-    for name, order, order_star in (("rk1", 1, None), ("rk4", 4, None), ("rkdp", 5, 4)):
+    for name, order, order_star in (("rk1", 1, None), ("rk2", 2, None), ("rk12", 2, 1), ("rk3", 3, None),
+                                    ("rk23", 3, 2), ("rk4", 4, None), ("rkck", 5, 4), ("rkdp", 5, 4)):
+        assert orc.ORDER[name] == order
         c, A, b, bs = orc.TABLEAUX[name]
         for i, row in enumerate(A):
             assert sum(row, Fraction(0)) == c[i]
@@ -282,6 +284,47 @@ def test_butcher_tableaux_satisfy_order_conditions_exactly():
         if bs is not None:
             assert _order_conditions(c, A, bs, order_star)
             assert not _order_conditions(c, A, bs, order_star + 1)
+
+
+def test_generic_stepper_reduces_to_the_written_out_ones_and_converges_at_its_order():
+    """rk_step from the tableau == the hand-written rk1 / rk4 / rkdp steps; every other tableau
+    converges on the macrospin closed form (pin P14) at its nominal order (pin P15)."""
+    alpha, Hz = 0.3, 2e5
+    pb = _macrospin(alpha, Hz)
+    m0 = np.array([0.8, 0.0, 0.6])
+    T0 = 1.0 / (orc.GAMMA0_DEFAULT * Hz)
+    ms = m0.reshape(3, 1, 1, 1)
+    dt = 0.2 * T0
+    assert np.allclose(orc.rk_step(pb.torque, ms, dt, "rk1")[0], orc.rk1_step(pb.torque, ms, dt), rtol=0, atol=1e-15)
+    assert np.allclose(orc.rk_step(pb.torque, ms, dt, "rk4")[0], orc.rk4_step(pb.torque, ms, dt), rtol=0, atol=1e-15)
+    a, ea, ka = orc.rk_step(pb.torque, ms, dt, "rkdp")
+    b, eb, kb = orc.rkdp_step(pb.torque, ms, dt)
+    assert np.allclose(a, b, rtol=0, atol=1e-15) and math.isclose(ea, eb, rel_tol=1e-12) and np.allclose(ka, kb)
+
+    def run(name, n, T):
+        m, k1 = ms.copy(), None
+        for _ in range(n):
+            m, _, kl = orc.rk_step(pb.torque, m, T / n, name, k1)
+            k1 = kl if name in orc.FSAL else None
+        return np.abs(m.ravel() - _macrospin_exact(m0, alpha, Hz, orc.GAMMA0_DEFAULT, T)).max()
+
+    for name, ns, T in (("rk2", (20, 40), 3 * T0), ("rk12", (20, 40), 3 * T0), ("rk3", (10, 20), 3 * T0),
+                        ("rk23", (10, 20), 3 * T0), ("rkck", (12, 24), 2 * T0)):
+        e1, e2 = run(name, ns[0], T), run(name, ns[1], T)
+        assert abs(math.log2(e1 / e2) - orc.ORDER[name]) < 0.45, (name, e1, e2)
+    # embedded error estimates scale with the order of the lower solution + 1
+    for name, lo in (("rk12", 2), ("rk23", 3), ("rkck", 5)):
+        _, e1, _ = orc.rk_step(pb.torque, ms, T0, name)
+        _, e2, _ = orc.rk_step(pb.torque, ms, T0 / 2, name)
+        assert abs(math.log2(e1 / e2) - lo) < 0.7, (name, e1, e2)
+    # controller and the maximum-variation step length
+    ok, dtn = orc.rk_controller(1e-13, 1e-5, 1e-5, "rk23")
+    assert ok and math.isclose(dtn, 0.8e-13)
+    ok, dtn = orc.rk_controller(1e-13, 8e-5, 1e-5, "rk23")
+    assert (not ok) and math.isclose(dtn, 0.4e-13)
+    dtm, k = orc.max_dm_step_length(pb.torque, ms, 0.01)
+    assert math.isclose(dtm * np.sqrt((k * k).sum()), 0.01, rel_tol=1e-12)
+    assert np.allclose(orc.average_m(np.concatenate([ms, -ms], axis=3)), 0.0)
 
 
 def test_dormand_prince_tableau_matches_published_coefficients():
