@@ -52,7 +52,9 @@ typedef enum {
     MM_RK4 = 2,  /* classical 4th order                                            */
     MM_RKDP = 3, /* Dormand-Prince 5(4), adaptive; controller: reading A10         */
     MM_RK12 = 4, /* Heun-Euler 2(1), adaptive                                      */
-    MM_RK23 = 5  /* Bogacki-Shampine 3(2), adaptive                                */
+    MM_RK23 = 5, /* Bogacki-Shampine 3(2), adaptive                                */
+    MM_RK3 = 6,  /* Kutta's third-order method                                     */
+    MM_RKCK = 7  /* Cash-Karp 5(4), adaptive                                       */
 } mm_method;
 
 /* Material and drive, SI units in; converted once to the internal reduced units mu0 = gamma0 = Ms = 1
@@ -152,6 +154,21 @@ mm_status mm_steps_fixed(mm_ctx* ctx, float* m_dev, mm_method method, double dt,
  * The cell count must be divisible by 4.  Thermal field: MM_EUNSUPPORTED (reading A6). */
 mm_status mm_steps_adaptive(mm_ctx* ctx, float* m_dev, mm_method method, int ntrials, double* dt_inout,
                             double tol, double* t_inout, int* naccepted_out, double* last_err_out);
+
+/* mm_steps_maxdm -- n steps of a fixed-step method (MM_RK1, MM_RK2, MM_RK3, MM_RK4) with "a fixed
+ * maximum variation of m per step": every step takes dt = max_dm / max_i |dm/dt(i)|
+ * evaluated on the state at the start of the step.  The norm, dt and t stay on the device (no host
+ * synchronisation per step); synchronises once at the end.
+ *   max_dm        largest change of a unit vector per step (dimensionless, > 0)
+ *   t_inout       host, may be NULL: time in, time after the n steps out
+ *   last_dt_out   host, may be NULL: length of the last step (seconds) */
+mm_status mm_steps_maxdm(mm_ctx* ctx, float* m_dev, mm_method method, double max_dm, int n,
+                         double* t_inout, double* last_dt_out);
+
+/* mm_average -- <f> over all cells of a field f [3][Nz][Ny][Nx] (e.g. the average magnetisation the
+ * paper's output tables list): fp64 accumulation on the device, avg_host[3] out.
+ * Synchronises the stream. */
+mm_status mm_average(mm_ctx* ctx, const float* field_dev, double avg_host[3]);
 
 /* mm_steps_fixed_host -- the same as mm_steps_fixed for a state held in HOST memory (pinned memory
  * gives the full PCIe rate): m_host is copied to the device, advanced n steps and copied back, all on

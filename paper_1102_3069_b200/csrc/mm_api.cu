@@ -62,6 +62,27 @@ Tableau make_tableau(mm_method m)
         t.bs[0] = 7.0 / 24; t.bs[1] = 0.25; t.bs[2] = 1.0 / 3; t.bs[3] = 0.125;
         t.embedded = true; t.fsal = true;
         break;
+    case MM_RK3:    // Kutta's third-order method
+        t.S = 3; t.A[1][0] = 0.5; t.A[2][0] = -1.0; t.A[2][1] = 2.0;
+        t.b[0] = 1.0 / 6; t.b[1] = 2.0 / 3; t.b[2] = 1.0 / 6;
+        break;
+    case MM_RKCK: {  // Cash-Karp 5(4)
+        t.S = 6;
+        const double A[7][7] = {
+            { 0 },
+            { 1.0 / 5 },
+            { 3.0 / 40, 9.0 / 40 },
+            { 3.0 / 10, -9.0 / 10, 6.0 / 5 },
+            { -11.0 / 54, 5.0 / 2, -70.0 / 27, 35.0 / 27 },
+            { 1631.0 / 55296, 175.0 / 512, 575.0 / 13824, 44275.0 / 110592, 253.0 / 4096 } };
+        std::memcpy(t.A, A, sizeof(A));
+        const double b[7] = { 37.0 / 378, 0, 250.0 / 621, 125.0 / 594, 0, 512.0 / 1771, 0 };
+        const double bs[7] = { 2825.0 / 27648, 0, 18575.0 / 48384, 13525.0 / 55296, 277.0 / 14336, 1.0 / 4, 0 };
+        std::memcpy(t.b, b, sizeof(b));
+        std::memcpy(t.bs, bs, sizeof(bs));
+        t.embedded = true;
+        break;
+    }
     case MM_RKDP: {  // Dormand-Prince 5(4)
         t.S = 7;
         const double A[7][7] = {
@@ -121,6 +142,7 @@ struct mm_ctx {
     float* mhost;     // device copy of a caller's host state (mm_steps_fixed_host)
     unsigned int* maxbits;
     StepCtl* ctl;     // device-side step controller state (a11)
+    double* ctl_scratch;   // 4 doubles of device scratch (mm_average)
     // stepper state
     uint64_t step_index;
     bool k0_valid;
@@ -361,6 +383,15 @@ __global__ void k_combine(size_t n, const float* __restrict__ m_n, float* __rest
     }
 }
 
+__global__ void k_normalise(size_t n, const float* __restrict__ src, float* __restrict__ dst)
+{
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
+        const float x = src[i], y = src[i + n], z = src[i + 2 * n];
+        const float s = rsqrtf(x * x + y * y + z * z);
+        dst[i] = x * s; dst[i + n] = y * s; dst[i + 2 * n] = z * s;
+    }
+}
+
 __global__ void k_copy4(const float4* __restrict__ src, float4* __restrict__ dst, size_t n4)
 {
     for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n4; i += (size_t)gridDim.x * blockDim.x)
@@ -521,6 +552,7 @@ mm_status mm_create(mm_ctx** out, const int grid[3], const double cellsize[3], c
     c->ms[0] = c->ms[1] = c->mtmp = nullptr;
     c->maxbits = nullptr;
     c->ctl = nullptr;
+    c->ctl_scratch = nullptr;
     c->step_index = 0;
     c->k0_valid = false;
     c->k0_method = -1;
@@ -593,6 +625,7 @@ mm_status mm_demag_init(mm_ctx* c)
     CUDA_TRY(c, cudaMemset(c->maxbits, 0, 2 * sizeof(unsigned int)));
     CUDA_TRY(c, cudaMalloc(&c->ctl, sizeof(StepCtl)));
     CUDA_TRY(c, cudaMemset(c->ctl, 0, sizeof(StepCtl)));
+    CUDA_TRY(c, cudaMalloc(&c->ctl_scratch, 4 * sizeof(double)));
     mm_status s;
     if ((s = set_smem(c, k_gen_fwd_x)) != MM_OK) return s;
     if ((s = set_smem(c, k_gen_y<-1>)) != MM_OK) return s;
@@ -668,7 +701,7 @@ mm_status mm_step(mm_ctx* c, float* m_dev, mm_method method, double* dt_inout, d
         // reading A10: accept iff err <= tol; dt <- dt clamp(0.8 (tol/err)^(1/order), 0.2, 2)
         err = (double)errf;
         accept = err <= tol;
-        const double order = method == MM_RKDP ? 5.0 : (method == MM_RK23 ? 3.0 : 2.0);
+        const double order = (method == MM_RKDP || method == MM_RKCK) ? 5.0 : (method == MM_RK23 ? 3.0 : 2.0);
         const double fac = err == 0.0 ? 2.0 : std::fmin(2.0, std::fmax(0.2, 0.8 * std::pow(tol / err, 1.0 / order)));
         *dt_inout = dt * fac;
     }
@@ -835,7 +868,7 @@ mm_status mm_steps_adaptive(mm_ctx* c, float* m_dev, mm_method method, int ntria
     h.dt = *dt_inout;
     h.tol = tol;
     h.g0Ms = gamma0_of(c) * c->mat.Ms;
-    h.order = method == MM_RKDP ? 5.0 : (method == MM_RK23 ? 3.0 : 2.0);
+    h.order = (method == MM_RKDP || method == MM_RKCK) ? 5.0 : (method == MM_RK23 ? 3.0 : 2.0);
     h.dtr = (float)(h.dt * h.g0Ms);
     CUDA_TRY(c, cudaMemcpyAsync(c->ctl, &h, sizeof(h), cudaMemcpyHostToDevice, c->stream));
     const size_t n4 = 3 * ncell(c->g) / 4;
@@ -866,6 +899,108 @@ mm_status mm_steps_adaptive(mm_ctx* c, float* m_dev, mm_method method, int ntria
         c->k0_valid = false;
         return fail(c, MM_ENUMERIC, "non-finite value met by the max-norm reduction");
     }
+    return MM_OK;
+}
+
+// ---- "fixed maximum variation of m per step": dt = max_dm / max |dm/dtau|, on the device ----
+__global__ void k_maxdm_dt(StepCtl* __restrict__ ctl, const unsigned int* __restrict__ maxbits, double max_dm)
+{
+    const float kmax = __uint_as_float(*maxbits);        // max_i |dm/dtau(i)|, reduced time
+    if (!isfinite(kmax) || !(kmax > 0.f)) { ctl->nonfinite = 1; ctl->dtr = 0.f; return; }
+    const double dtr = max_dm / (double)kmax;
+    ctl->dtr = (float)dtr;
+    ctl->dt = dtr / ctl->g0Ms;
+    ctl->t += ctl->dt;
+    ctl->ntrial++;
+}
+
+mm_status mm_steps_maxdm(mm_ctx* c, float* m_dev, mm_method method, double max_dm, int n, double* t_inout,
+                         double* last_dt_out)
+{
+    mm_status s = check_ready(c);
+    if (s != MM_OK) return s;
+    if (!m_dev || !(max_dm > 0) || n < 0) return fail(c, MM_EINVAL, "bad m_dev / max_dm / n");
+    const Tableau tab = make_tableau(method);
+    if (tab.S == 0 || tab.embedded) return fail(c, MM_EINVAL, "mm_steps_maxdm needs a fixed-step method");
+    if (c->mat.T > 0) return fail(c, MM_EUNSUPPORTED, "thermal field needs a step length known in advance (reading A6)");
+    StepCtl h;
+    std::memset(&h, 0, sizeof(h));
+    h.t = t_inout ? *t_inout : 0.0;
+    h.g0Ms = gamma0_of(c) * c->mat.Ms;
+    CUDA_TRY(c, cudaMemcpyAsync(c->ctl, &h, sizeof(h), cudaMemcpyHostToDevice, c->stream));
+    const size_t ncl = ncell(c->g);
+    for (int i = 0; i < n; ++i) {
+        // stage 1 on its own: k_1 -> kb[0] and max |k_1|, then dt, then m_2 = m + dt a_21 k_1 (or the Euler update)
+        CUDA_TRY(c, cudaMemsetAsync(c->maxbits, 0, sizeof(unsigned int), c->stream));
+        EpiParams ep;
+        std::memset(&ep, 0, sizeof(ep));
+        fill_material(c, ep, c->step_index, 0.0);
+        ep.mode = EPI_STAGE;
+        ep.m_in = m_dev;
+        ep.m_n = m_dev;
+        ep.k_out = c->kb[0];
+        ep.do_err = 1;
+        ep.e_self = 1.0f;
+        ep.maxbits = c->maxbits;
+        if ((s = launch_eval(c, ep)) != MM_OK) return s;
+        k_maxdm_dt<<<1, 1, 0, c->stream>>>(c->ctl, c->maxbits, max_dm);
+        c->kt.launches++;
+        if (tab.S == 1) {
+            k_combine<<<148 * 8, 256, 0, c->stream>>>(ncl, m_dev, c->mtmp, 1, (float)tab.b[0], 0.f, c->kb[0], c->kb[0],
+                                                      &c->ctl->dtr);
+            k_normalise<<<148 * 8, 256, 0, c->stream>>>(ncl, c->mtmp, m_dev);
+            c->kt.launches += 2;
+        } else {
+            k_combine<<<148 * 8, 256, 0, c->stream>>>(ncl, m_dev, c->ms[0], 1, (float)tab.A[1][0], 0.f, c->kb[0],
+                                                      c->kb[0], &c->ctl->dtr);
+            c->kt.launches++;
+            for (int st = 1; st < tab.S; ++st)
+                if ((s = run_stage(c, m_dev, tab, st, 0.0, c->step_index, false, true)) != MM_OK) return s;
+        }
+        c->step_index++;
+    }
+    c->k0_valid = false;
+    CUDA_TRY(c, cudaMemcpyAsync(&h, c->ctl, sizeof(h), cudaMemcpyDeviceToHost, c->stream));
+    CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+    if (t_inout) *t_inout = h.t;
+    if (last_dt_out) *last_dt_out = h.dt;
+    if (h.nonfinite) return fail(c, MM_ENUMERIC, "non-finite or zero torque norm in the maximum-variation step");
+    return MM_OK;
+}
+
+// ---- <f> over all cells, fp64 accumulation ----
+__global__ void k_average(size_t n, const float* __restrict__ f, double* __restrict__ out)
+{
+    double acc[3] = { 0.0, 0.0, 0.0 };
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x)
+        for (int cc = 0; cc < 3; ++cc) acc[cc] += (double)f[i + cc * n];
+    __shared__ double sh[3][8];
+    for (int cc = 0; cc < 3; ++cc) {
+        double v = acc[cc];
+        for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+        if ((threadIdx.x & 31) == 0) sh[cc][threadIdx.x >> 5] = v;
+    }
+    __syncthreads();
+    if (threadIdx.x < 3) {
+        double v = 0.0;
+        for (int w = 0; w < (int)(blockDim.x >> 5); ++w) v += sh[threadIdx.x][w];
+        atomicAdd(out + threadIdx.x, v);
+    }
+}
+
+mm_status mm_average(mm_ctx* c, const float* field_dev, double avg_host[3])
+{
+    if (!c || !field_dev || !avg_host) return MM_EINVAL;
+    if (!c->has_demag) return fail(c, MM_ESTATE, "mm_demag_init has not been called");
+    double* acc = reinterpret_cast<double*>(c->ctl_scratch);
+    CUDA_TRY(c, cudaMemsetAsync(acc, 0, 3 * sizeof(double), c->stream));
+    const size_t n = ncell(c->g);
+    k_average<<<148 * 4, 256, 0, c->stream>>>(n, field_dev, acc);
+    c->kt.launches++;
+    double h[3];
+    CUDA_TRY(c, cudaMemcpyAsync(h, acc, sizeof(h), cudaMemcpyDeviceToHost, c->stream));
+    CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+    for (int i = 0; i < 3; ++i) avg_host[i] = h[i] / (double)n;
     return MM_OK;
 }
 
@@ -1027,6 +1162,7 @@ void mm_destroy(mm_ctx* c)
     }
     cudaFree(c->maxbits);
     cudaFree(c->ctl);
+    cudaFree(c->ctl_scratch);
     if (c->gstream) cudaStreamDestroy(c->gstream);
     for (int i = 0; i < 2; ++i)
         if (c->gev[i]) cudaEventDestroy(c->gev[i]);

@@ -17,7 +17,7 @@ _LIBPATH = os.path.join(_HERE, "libmm_b200.so")
 MM_OK = 0
 STATUS = {0: "MM_OK", 1: "MM_EINVAL", 2: "MM_ENOMEM", 3: "MM_ECUDA", 4: "MM_ESTATE",
           5: "MM_EUNSUPPORTED", 6: "MM_ENUMERIC"}
-METHODS = {"rk1": 0, "rk2": 1, "rk4": 2, "rkdp": 3, "rk12": 4, "rk23": 5}
+METHODS = {"rk1": 0, "rk2": 1, "rk4": 2, "rkdp": 3, "rk12": 4, "rk23": 5, "rk3": 6, "rkck": 7}
 
 
 class MMError(RuntimeError):
@@ -69,6 +69,8 @@ def lib():
         L.mm_steps_fixed.argtypes = [vp, vp, C.c_int, C.c_double, C.c_int, d3, d3]
         L.mm_steps_fixed_host.argtypes = [vp, vp, C.c_int, C.c_double, C.c_int, d3, d3]
         L.mm_steps_adaptive.argtypes = [vp, vp, C.c_int, C.c_int, d3, C.c_double, d3, i3, d3]
+        L.mm_steps_maxdm.argtypes = [vp, vp, C.c_int, C.c_double, C.c_int, d3, d3]
+        L.mm_average.argtypes = [vp, vp, d3]
         L.mm_kernel_timing.argtypes = [vp, C.c_int]
         L.mm_kernel_times.argtypes = [vp, d3, C.POINTER(C.c_uint64)]
         L.mm_fused_eval.argtypes = [vp, vp, C.c_int, C.c_int, C.c_double, C.c_uint64]
@@ -196,6 +198,18 @@ class Sim:
         self._chk(self.L.mm_steps_adaptive(self.ctx, self._dev(m), METHODS[method], int(ntrials), C.byref(dtv), tol,
                                            C.byref(tv), C.byref(nacc), C.byref(err)))
         return nacc.value, err.value, dtv.value, tv.value
+
+    def steps_maxdm(self, m, method, max_dm, n, t=0.0):
+        """n steps with dt = max_dm / max|dm/dt| each; returns (t, last_dt)."""
+        tv, dtv = C.c_double(t), C.c_double(0.0)
+        self._chk(self.L.mm_steps_maxdm(self.ctx, self._dev(m), METHODS[method], max_dm, int(n), C.byref(tv),
+                                        C.byref(dtv)))
+        return tv.value, dtv.value
+
+    def average(self, f):
+        out = (C.c_double * 3)()
+        self._chk(self.L.mm_average(self.ctx, self._dev(f), out))
+        return np.array([out[0], out[1], out[2]])
 
     def steps_fixed_host(self, m_host, method, dt, n, t=0.0):
         """m_host: CPU float32 tensor (pinned for full PCIe rate), updated in place."""

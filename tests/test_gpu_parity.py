@@ -471,3 +471,86 @@ def test_device_side_step_controller_follows_the_host_controlled_run(method):
     assert np.abs(md3.double().cpu().numpy() - ref).max() <= 1e-5
     for s_ in (sim, sim2, sim3):
         s_.close()
+
+
+# ---- the remaining Runge-Kutta tableaux, the maximum-variation step, <m> ----
+@pytest.mark.parametrize("method", ["rk2", "rk3", "rk12", "rk23", "rkck"])
+def test_remaining_tableaux_follow_the_oracle(method):
+    wl = util.small((24, 10, 6), init="tilted", alpha=0.05, Bext=(-0.0246, 0.0043, 0.0))
+    m = wlm.initial_m(wl)
+    pb = util.oracle_problem(wl)
+    dt, n = 4e-14, 12
+    mo, k1, errs = m.astype(np.float64), None, []
+    for _ in range(n):
+        mo, err, kl = orc.rk_step(pb.torque, mo, dt, method, k1)
+        k1 = kl if method in orc.FSAL else None
+        errs.append(err)
+    sim = util.gpu_sim(wl)
+    md = util.to_dev(m)
+    for i in range(n):
+        _, ge = sim.steps_fixed(md, method, dt, 1)
+        if errs[i] is not None:
+            # fp32 floor of the embedded difference: a few 1e-10 (dimensionless), far below any tolerance in use
+            assert abs(ge - errs[i]) <= 0.02 * errs[i] + 1e-9, (i, ge, errs[i])
+    assert np.abs(md.double().cpu().numpy() - mo).max() <= TOL_M
+    md2 = util.to_dev(m)                       # the same in one call
+    sim.reset_stepper(0)
+    sim.steps_fixed(md2, method, dt, n)
+    assert np.abs(md2.double().cpu().numpy() - mo).max() <= TOL_M
+    sim.close()
+
+
+def test_cash_karp_adaptive_run_matches_the_oracle_controller():
+    wl = util.small((24, 10, 6), init="tilted", alpha=0.02, Bext=(-0.0246, 0.0043, 0.0), Ku=0.0)
+    m = wlm.initial_m(wl)
+    pb = util.oracle_problem(wl)
+    tol, dt, mo, seq, trials = 1e-5, 3e-13, m.astype(np.float64), [], 0
+    while len(seq) < 20:
+        mn, err, _ = orc.rk_step(pb.torque, mo, dt, "rkck")
+        ok, dtn = orc.rk_controller(dt, err, tol, "rkck")
+        trials += 1
+        if ok:
+            seq.append(dt); mo = mn
+        dt = dtn
+    sim = util.gpu_sim(wl)
+    md = util.to_dev(m)
+    dt, t, nacc, ntr = 3e-13, 0.0, 0, 0
+    while nacc < 20:
+        acc, err, dt, t = sim.step(md, "rkck", dt, tol, t)
+        ntr += 1; nacc += int(acc)
+    assert abs(ntr - trials) <= 1 and abs(t - sum(seq)) <= 0.02 * sum(seq)
+    assert np.abs(md.double().cpu().numpy() - mo).max() <= 1e-3
+    md2 = util.to_dev(m)                       # controller on the device
+    sim.reset_stepper(0)
+    n2, _, _, t2 = sim.steps_adaptive(md2, "rkck", ntr, 3e-13, tol, 0.0)
+    assert n2 == 20 and abs(t2 - t) <= 1e-3 * t
+    sim.close()
+
+
+@pytest.mark.parametrize("method", ["rk1", "rk2", "rk4"])
+def test_maximum_variation_step_length(method):
+    """the fixed-step methods with 'a fixed maximum variation of m per step'."""
+    wl = util.small((24, 10, 6), init="tilted", alpha=0.1, Bext=(-0.0246, 0.0043, 0.0))
+    m = wlm.initial_m(wl)
+    pb = util.oracle_problem(wl)
+    max_dm, n = 2e-3, 10
+    mo, t_ref, dt_ref = m.astype(np.float64), 0.0, 0.0
+    for _ in range(n):
+        dt_ref, k1 = orc.max_dm_step_length(pb.torque, mo, max_dm)
+        mo, _, _ = orc.rk_step(pb.torque, mo, dt_ref, method, k1)
+        t_ref += dt_ref
+    sim = util.gpu_sim(wl)
+    md = util.to_dev(m)
+    t, last_dt = sim.steps_maxdm(md, method, max_dm, n)
+    assert abs(t - t_ref) <= 1e-4 * t_ref and abs(last_dt - dt_ref) <= 1e-4 * dt_ref
+    assert np.abs(md.double().cpu().numpy() - mo).max() <= TOL_M
+    sim.close()
+
+
+def test_average_magnetisation():
+    wl = util.small((40, 6, 3), (2e-9, 2e-9, 4e-9))
+    m = wlm.initial_m(wl)
+    sim = util.gpu_sim(wl)
+    avg = sim.average(util.to_dev(m))
+    assert np.abs(avg - orc.average_m(m.astype(np.float64))).max() <= 1e-7
+    sim.close()
