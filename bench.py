@@ -178,6 +178,45 @@ def run_reference(args):
     print(json.dumps(out))
 
 
+# PAPER.md:239-250 (Table 1): GPU time per Euler step on a GTX580, ms -- context, another machine
+PAPER_TABLE1_GPU_MS = {(32, 32, 1): 0.59, (64, 64, 1): 0.60, (128, 128, 1): 0.69, (256, 256, 1): 1.11,
+                       (512, 512, 1): 2.75, (1024, 1024, 1): 9.07, (2048, 2048, 1): 35.78, (8, 8, 8): 0.79,
+                       (16, 16, 16): 1.03, (32, 32, 32): 1.70, (64, 64, 64): 5.52, (128, 128, 128): 35.42}
+
+
+def run_sweep(args):
+    """time per Euler step (one evaluation + update) on power-of-two
+    N x N and N x N x N grids, shaped like the paper's Table 1 / Fig. 6.  One JSON line."""
+    import torch
+    import paper_1102_3069_b200 as mm
+    from paper_1102_3069_b200 import workloads as wlm
+    torch.cuda.set_device(0)
+    # 2048^2 of the paper's table is left out: its padded x length 4096 exceeds the longest line of the kernels
+    grids = [(n, n, 1) for n in (32, 64, 128, 256, 512, 1024)] + [(n, n, n) for n in (8, 16, 32, 64, 128, 256)]
+    rows = []
+    for g in grids:
+        wl = wlm.scaled(wlm.config(5), g)
+        sim = mm.Sim(wl.grid, wl.cell, wl.pbc, wl.mat)
+        md = torch.from_numpy(wlm.initial_m(wl)).cuda()
+        n = 200 if g[0] * g[1] * g[2] <= (1 << 21) else 20
+        sim.steps_fixed(md, "rk1", 1e-15, n)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        e0.record()
+        sim.steps_fixed(md, "rk1", 1e-15, n)
+        e1.record()
+        torch.cuda.synchronize()
+        ms = e0.elapsed_time(e1) / n
+        assert torch.isfinite(md).all()
+        rows.append({"grid": "x".join(map(str, g)), "ms_per_euler_step": ms,
+                     "ns_per_cell": ms * 1e6 / (g[0] * g[1] * g[2]),
+                     "paper_gtx580_ms": PAPER_TABLE1_GPU_MS.get(g)})
+        sim.close()
+        del md
+    print(json.dumps({"metric": "time per Euler step (PAPER.md Table 1 shape)", "unit": "ms", "dtype": "f32",
+                      "data": "synthetic", "higher_is_better": False, "n_gpus": 1, "sweep": rows}))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -189,9 +228,12 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--generic", action="store_true", help="force the generic shared-memory FFT kernels")
     ap.add_argument("--fast", type=int, default=-1, help="bit mask for mm_set_fast_path (default: all)")
+    ap.add_argument("--sweep", action="store_true", help="Euler-step time on N^2 / N^3 grids (Table 1 shape)")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
+    if args.sweep:
+        return run_sweep(args)
 
     import numpy as np
     import torch

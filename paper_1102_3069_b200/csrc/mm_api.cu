@@ -311,13 +311,27 @@ mm_status launch_eval(mm_ctx* c, const EpiParams& ep)
                 c->kt.begin(KT_INV_Y);
                 fast_y(fp, g, st, 1, wt, c->specA, c->specB);
                 c->kt.end(KT_INV_Y);
-            } else {   // generic: y forward, multiply, y inverse in one kernel
-                const int tx = pick_tx(g.Py, 4, 1, &bytes);
-                if (!tx) return fail(c, MM_EUNSUPPORTED, "y line too long for the shared-memory tile");
+            } else if (const int tx = pick_tx(g.Py, 4, 1, &bytes)) {
+                // generic: y forward, multiply, y inverse in one kernel
                 dim3 grid((g.Cx + tx - 1) / tx, 1);
                 c->kt.begin(KT_MID);
                 k_gen_mid<<<grid, 256, bytes, st>>>(g, c->plan[1], c->specA, c->khat, 1, tx);
                 c->kt.end(KT_MID);
+            } else {
+                // very long y lines (four tile buffers do not fit): three launches through specB
+                const int ty = pick_tx(g.Py, 2, 1, &bytes);
+                if (!ty) return fail(c, MM_EUNSUPPORTED, "y line too long for the shared-memory tile");
+                dim3 grid((g.Cx + ty - 1) / ty, 3 * g.Nz);
+                c->kt.begin(KT_FWD_Y);
+                k_gen_y<-1><<<grid, 256, bytes, st>>>(g, c->plan[1], c->specA, c->specB, ty);
+                c->kt.end(KT_FWD_Y);
+                c->kt.begin(KT_MID);
+                dim3 gm((g.Cx + 255) / 256, g.Py);
+                ff::k_mul2d<<<gm, 256, 0, st>>>(g, c->specB, c->khat);
+                c->kt.end(KT_MID);
+                c->kt.begin(KT_INV_Y);
+                k_gen_y<1><<<grid, 256, bytes, st>>>(g, c->plan[1], c->specB, c->specA, ty);
+                c->kt.end(KT_INV_Y);
             }
         } else {
             c->kt.begin(KT_MID);
