@@ -42,7 +42,12 @@ __device__ __forceinline__ float neg2ln_u(uint32_t x)
 __device__ __forceinline__ void thermal_eta(const EpiParams& p, uint64_t cell, float eta[3])
 {
     uint32_t w[4];
-    philox4x32_10((uint32_t)cell, (uint32_t)(cell >> 32), p.step0, p.step1, p.key0, p.key1, w);
+    uint32_t st0 = p.step0, st1 = p.step1;
+    if (p.step_dev) {
+        const unsigned long long st = __ldg(p.step_dev);
+        st0 = (uint32_t)st; st1 = (uint32_t)(st >> 32);
+    }
+    philox4x32_10((uint32_t)cell, (uint32_t)(cell >> 32), st0, st1, p.key0, p.key1, w);
     const float r1 = sqrtf(neg2ln_u(w[0]));
     const float r2 = sqrtf(neg2ln_u(w[2]));
     float s1, c1, s2, c2;

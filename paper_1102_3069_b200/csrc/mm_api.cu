@@ -143,6 +143,8 @@ struct mm_ctx {
     unsigned int* maxbits;
     StepCtl* ctl;     // device-side step controller state (a11)
     double* ctl_scratch;   // 4 doubles of device scratch (mm_average)
+    unsigned long long* step_dev;   // device copy of step_index, advanced on the device during graph replay
+    bool step_on_device;
     // stepper state
     uint64_t step_index;
     bool k0_valid;
@@ -221,6 +223,7 @@ void fill_material(const mm_ctx* c, EpiParams& p, uint64_t step, double dt_therm
     p.key1 = (uint32_t)(M.seed >> 32);
     p.step0 = (uint32_t)(step & 0xffffffffu);
     p.step1 = (uint32_t)(step >> 32);
+    p.step_dev = c->step_on_device ? c->step_dev : nullptr;
     p.alpha = (float)M.alpha;
     p.inv1pa2 = (float)(1.0 / (1.0 + M.alpha * M.alpha));
     p.stt = (M.j[0] != 0.0 || M.j[1] != 0.0 || M.j[2] != 0.0) ? 1 : 0;
@@ -567,6 +570,8 @@ mm_status mm_create(mm_ctx** out, const int grid[3], const double cellsize[3], c
     c->maxbits = nullptr;
     c->ctl = nullptr;
     c->ctl_scratch = nullptr;
+    c->step_dev = nullptr;
+    c->step_on_device = false;
     c->step_index = 0;
     c->k0_valid = false;
     c->k0_method = -1;
@@ -640,6 +645,7 @@ mm_status mm_demag_init(mm_ctx* c)
     CUDA_TRY(c, cudaMalloc(&c->ctl, sizeof(StepCtl)));
     CUDA_TRY(c, cudaMemset(c->ctl, 0, sizeof(StepCtl)));
     CUDA_TRY(c, cudaMalloc(&c->ctl_scratch, 4 * sizeof(double)));
+    CUDA_TRY(c, cudaMalloc(&c->step_dev, sizeof(unsigned long long)));
     mm_status s;
     if ((s = set_smem(c, k_gen_fwd_x)) != MM_OK) return s;
     if ((s = set_smem(c, k_gen_y<-1>)) != MM_OK) return s;
@@ -736,9 +742,11 @@ mm_status mm_step(mm_ctx* c, float* m_dev, mm_method method, double* dt_inout, d
 }
 
 // running maximum over the steps of one mm_steps_fixed call (bit patterns: NaN / Inf compare largest)
-__global__ void k_track_max(const unsigned int* __restrict__ maxbits, unsigned int* __restrict__ run)
+__global__ void k_track_max(const unsigned int* __restrict__ maxbits, unsigned int* __restrict__ run,
+                            unsigned long long* __restrict__ step_dev)
 {
     atomicMax(run, *maxbits);
+    if (step_dev) *step_dev += 1ull;          // the step index of the next thermal draw (reading A6)
 }
 
 static mm_status steps_fixed_impl(mm_ctx* c, float* m_dev, mm_method method, const Tableau& tab, double dt, int n,
@@ -752,13 +760,20 @@ static mm_status steps_fixed_impl(mm_ctx* c, float* m_dev, mm_method method, con
         mm_status st = enqueue_step(c, m_dev, method, tab, dt, false, &newstate);
         if (st == MM_OK) st = commit_step(c, m_dev, method, tab, newstate);
         if (st != MM_OK) return st;
-        k_track_max<<<1, 1, 0, c->stream>>>(c->maxbits, run);
+        k_track_max<<<1, 1, 0, c->stream>>>(c->maxbits, run, c->step_on_device ? c->step_dev : nullptr);
         c->kt.launches++;
         return MM_OK;
     };
     int done = 0;
     if (graph_ok) {
-        if ((s = one_step()) != MM_OK) return s;          // also sets the kernels' attributes outside the capture
+        // with a thermal field the step index that selects the draw lives on the device during the replay
+        c->step_on_device = c->mat.T > 0;
+        if (c->step_on_device) {
+            const unsigned long long si = c->step_index;
+            cudaMemcpyAsync(c->step_dev, &si, sizeof(si), cudaMemcpyHostToDevice, c->stream);
+            cudaStreamSynchronize(c->stream);              // `si` is a stack variable
+        }
+        if ((s = one_step()) != MM_OK) { c->step_on_device = false; return s; }   // also sets kernel attributes outside the capture
         done = 1;
         cudaGraph_t graph = nullptr;
         cudaGraphExec_t exec = nullptr;
@@ -784,6 +799,11 @@ static mm_status steps_fixed_impl(mm_ctx* c, float* m_dev, mm_method method, con
             if (graph) cudaGraphDestroy(graph);
         }
         cudaGetLastError();                                // a refused capture must not surface later
+        if (c->step_on_device) {
+            // the remaining plain steps (if any) take the index from the host again
+            cudaStreamSynchronize(c->stream);
+            c->step_on_device = false;
+        }
     }
     for (; done < n; ++done)
         if ((s = one_step()) != MM_OK) return s;
@@ -816,7 +836,7 @@ mm_status mm_steps_fixed(mm_ctx* c, float* m_dev, mm_method method, double dt, i
     // The caller's stream may be the legacy default stream, which cannot be captured: the sequence runs
     // on a stream of the context's own, ordered after and before the caller's stream with events.
     const bool chunked = (c->fast & FAST_CHUNK) && c->fp.chunk_w > 0 && c->g.Pz > 1;
-    bool graph_ok = c->use_graph && n >= 4 && !tab.fsal && !(c->mat.T > 0) && !c->kt.on && !chunked;
+    bool graph_ok = c->use_graph && n >= 4 && !tab.fsal && !c->kt.on && !chunked;
     if (graph_ok && !c->gstream) {
         if (cudaStreamCreateWithFlags(&c->gstream, cudaStreamNonBlocking) != cudaSuccess ||
             cudaEventCreateWithFlags(&c->gev[0], cudaEventDisableTiming) != cudaSuccess ||
@@ -1177,6 +1197,7 @@ void mm_destroy(mm_ctx* c)
     cudaFree(c->maxbits);
     cudaFree(c->ctl);
     cudaFree(c->ctl_scratch);
+    cudaFree(c->step_dev);
     if (c->gstream) cudaStreamDestroy(c->gstream);
     for (int i = 0; i < 2; ++i)
         if (c->gev[i]) cudaEventDestroy(c->gev[i]);

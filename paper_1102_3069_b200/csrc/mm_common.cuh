@@ -41,6 +41,7 @@ struct EpiParams {
     int thermal;         // Eq. (6)
     float sig_th;        // sqrt(2 alpha kB T/(gamma0 mu0 Ms V dt)) / Ms
     uint32_t key0, key1, step0, step1;
+    const unsigned long long* step_dev;   // if set, the step index of the thermal draw is read here (graph replay)
     // torque
     float alpha, inv1pa2;   // Eq. (1)
     int stt;                // Eq. (7)-(8)

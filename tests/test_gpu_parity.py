@@ -554,3 +554,25 @@ def test_average_magnetisation():
     avg = sim.average(util.to_dev(m))
     assert np.abs(avg - orc.average_m(m.astype(np.float64))).max() <= 1e-7
     sim.close()
+
+
+def test_graph_replay_with_thermal_field_draws_per_step(monkeypatch):
+    """With a thermal field the step index that selects the draw is advanced on the device during the
+    replay: same bits as plain launches, and as the oracle's per-step draws (reading A6)."""
+    wl = util.small((16, 12, 1), (4e-9, 4e-9, 2e-9), (2, 2, 0), init="xnoise", alpha=0.1, T=300.0, seed=3)
+    m = wlm.initial_m(wl)
+    out = []
+    for flag in ("1", "0"):
+        monkeypatch.setenv("MM_GRAPH", flag)
+        sim = util.gpu_sim(wl)
+        md = util.to_dev(m)
+        sim.steps_fixed(md, "rk4", 5e-14, 8)
+        sim.steps_fixed(md, "rk4", 5e-14, 6)          # continues at step index 8
+        out.append(md.cpu().numpy().copy())
+        sim.close()
+    assert np.array_equal(out[0], out[1])
+    pb = util.oracle_problem(wl)
+    mo = m.astype(np.float64)
+    for s_ in range(14):
+        mo = orc.rk4_step(lambda x: pb.torque(x, s_, 5e-14), mo, 5e-14)
+    assert np.abs(out[0].astype(np.float64) - mo).max() <= TOL_M
