@@ -92,6 +92,10 @@ class Material:
     P: float = 0.0                  # polarisation, Eq. (8)
     xi: float = 0.0                 # non-adiabaticity, Eq. (7)
     stt_literal_eq7: bool = False   # reading A7
+    K1: float = 0.0                 # J/m^3      Eq. (5), cubic anisotropy
+    K2: float = 0.0                 # J/m^3      Eq. (5)
+    anis_c1: tuple = (1.0, 0.0, 0.0)   # first two cubic axes; the third is c1 x c2 (reading A14)
+    anis_c2: tuple = (0.0, 1.0, 0.0)
 
 
 # --------------------------------------------------------------------------
@@ -301,6 +305,40 @@ def anisotropy_field(m, mat: Material) -> np.ndarray:
     return (2.0 * mat.Ku / (MU0 * mat.Ms)) * u[:, None, None, None] * mu[None]
 
 
+def cubic_axes(mat: Material):
+    """Reading A14 (the paper names "the cubic easy magnetization axes" without saying how they are
+    given): c1 normalised, c2 made orthogonal to c1 and normalised, c3 = c1 x c2."""
+    c1 = np.asarray(mat.anis_c1, dtype=np.float64)
+    c1 = c1 / np.linalg.norm(c1)
+    c2 = np.asarray(mat.anis_c2, dtype=np.float64)
+    c2 = c2 - np.dot(c2, c1) * c1
+    c2 = c2 / np.linalg.norm(c2)
+    return c1, c2, np.cross(c1, c2)
+
+
+def cubic_anisotropy_energy_density(m, mat: Material) -> np.ndarray:
+    """Eq. (5): K1 (a1^2 a2^2 + a2^2 a3^2 + a1^2 a3^2) + K2 a1^2 a2^2 a3^2,
+    a_i the direction cosines of m on the cubic axes.  J/m^3 per cell."""
+    a = [np.tensordot(c, m, axes=(0, 0)) for c in cubic_axes(mat)]
+    return mat.K1 * (a[0] ** 2 * a[1] ** 2 + a[1] ** 2 * a[2] ** 2 + a[0] ** 2 * a[2] ** 2) \
+        + mat.K2 * a[0] ** 2 * a[1] ** 2 * a[2] ** 2
+
+
+def cubic_anisotropy_field(m, mat: Material) -> np.ndarray:
+    """H = -(1/(mu0 Ms)) dE/dm of Eq. (5): with dE/da1 = 2 K1 a1 (a2^2 + a3^2) + 2 K2 a1 a2^2 a3^2
+    (and cyclic), H = -(1/(mu0 Ms)) sum_i (dE/da_i) c_i."""
+    if mat.K1 == 0.0 and mat.K2 == 0.0:
+        return np.zeros_like(m, dtype=np.float64)
+    c = cubic_axes(mat)
+    a = [np.tensordot(ci, m, axes=(0, 0)) for ci in c]
+    H = np.zeros_like(m, dtype=np.float64)
+    for i in range(3):
+        j, k = (i + 1) % 3, (i + 2) % 3
+        dE = 2.0 * mat.K1 * a[i] * (a[j] ** 2 + a[k] ** 2) + 2.0 * mat.K2 * a[i] * a[j] ** 2 * a[k] ** 2
+        H -= c[i][:, None, None, None] * dE[None] / (MU0 * mat.Ms)
+    return H
+
+
 def zeeman_field(m, mat: Material) -> np.ndarray:
     """Applied field: H_ext = B_ext / mu0, uniform."""
     B = np.asarray(mat.Bext, dtype=np.float64)
@@ -402,6 +440,7 @@ class Problem:
         H = self.demag_field(m)
         H = H + exchange_field(m, self.mat, self.grid, self.cell, self.pbc)
         H = H + anisotropy_field(m, self.mat)
+        H = H + cubic_anisotropy_field(m, self.mat)
         H = H + zeeman_field(m, self.mat)
         if self.mat.T != 0.0:
             H = H + thermal_field(self.mat, self.grid, self.cell, step, dt_thermal)

@@ -169,6 +169,36 @@ def test_anisotropy_special_cases():
     assert np.allclose(H, -g / (orc.MU0 * mat.Ms), rtol=1e-8)
 
 
+def test_cubic_anisotropy_field_is_minus_the_energy_gradient():
+    """Eq. (5).  Pins: (i) the field is -(1/mu0 Ms) dE/dm of the printed energy, checked by
+    central differences of that energy; (ii) along a cube axis the energy and the field vanish (K1 > 0:
+    <100> easy); (iii) along <111> the energy is K1/3 + K2/27; (iv) it is invariant under the cube group
+    (a permutation / sign change of the axes)."""
+    rng = np.random.default_rng(3)
+    mat = orc.Material(Ms=4.8e5, K1=-4.5e3, K2=2.3e3, anis_c1=(1.0, 1.0, 0.0), anis_c2=(-1.0, 1.0, 0.3))
+    m = rng.standard_normal((3, 2, 3, 4))
+    m /= np.sqrt((m * m).sum(0))
+    H = orc.cubic_anisotropy_field(m, mat)
+    h = 1e-6
+    for c in range(3):
+        dm = np.zeros_like(m); dm[c] = h
+        dE = (orc.cubic_anisotropy_energy_density(m + dm, mat) - orc.cubic_anisotropy_energy_density(m - dm, mat)) / (2 * h)
+        assert np.allclose(H[c], -dE / (orc.MU0 * mat.Ms), rtol=1e-7, atol=1e-6)
+    c1, c2, c3 = orc.cubic_axes(mat)
+    assert abs(np.dot(c1, c2)) < 1e-15 and abs(np.dot(c1, c3)) < 1e-15 and np.allclose(np.cross(c1, c2), c3)
+    for ax in (c1, c2, c3):
+        ma = ax.reshape(3, 1, 1, 1)
+        assert abs(orc.cubic_anisotropy_energy_density(ma, mat)).max() < 1e-12
+        assert np.abs(orc.cubic_anisotropy_field(ma, mat)).max() < 1e-9
+    m111 = ((c1 + c2 + c3) / np.sqrt(3.0)).reshape(3, 1, 1, 1)
+    assert np.isclose(orc.cubic_anisotropy_energy_density(m111, mat)[0, 0, 0], mat.K1 / 3 + mat.K2 / 27)
+    mat2 = orc.Material(Ms=4.8e5, K1=-4.5e3, K2=2.3e3, anis_c1=tuple(-c3), anis_c2=tuple(c1))
+    assert np.allclose(orc.cubic_anisotropy_field(m, mat2), H, rtol=0, atol=1e-9)
+    # and it enters H_eff
+    pb = orc.Problem((4, 3, 2), (3e-9, 3e-9, 3e-9), (0, 0, 0), mat, demag="none")
+    assert np.allclose(pb.heff(m), H + orc.exchange_field(m, mat, (4, 3, 2), (3e-9,) * 3) + orc.zeeman_field(m, mat))
+
+
 def test_zeeman():
     mat = orc.Material(Ms=8e5, Bext=(0.0, 10e-3, 0.0))
     H = orc.zeeman_field(np.zeros((3, 2, 2, 2)), mat)
