@@ -74,6 +74,9 @@ typedef struct {
     double xi;        /* degree of non-adiabaticity               Eq. (7)                         */
     int stt_literal_eq7; /* 0: (1 + alpha xi) on the adiabatic term; 1: Eq. (7) as printed (A7)   */
     int demag;        /* 1: magnetostatic field on (default use); 0: off (tests of local terms)   */
+    double K1, K2;    /* cubic anisotropy constants, J/m^3         Eq. (5)            */
+    double anis_c1[3], anis_c2[3]; /* first two cubic axes; c2 is made orthogonal to c1, c3 = c1 x c2
+                       * (reading A14); ignored if K1 == K2 == 0                                 */
 } mm_material;
 
 /* mm_create -- set up a context for a grid of equal cuboid cells.

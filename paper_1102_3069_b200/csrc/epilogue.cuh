@@ -106,6 +106,21 @@ __device__ __forceinline__ float epilogue_finish_v(const EpiParams& p, size_t id
 #pragma unroll
         for (int c = 0; c < 3; ++c) h[c][u] += s * p.u[c] + p.hext[c];
     }
+    // ---- cubic anisotropy (Eq. (5), reading A14): h -= sum_i (dE/da_i) c_i ----
+    if (p.cubic) {
+#pragma unroll
+        for (int u = 0; u < V; ++u) {
+            const float a1 = m[0][u] * p.c1[0] + m[1][u] * p.c1[1] + m[2][u] * p.c1[2];
+            const float a2 = m[0][u] * p.c2[0] + m[1][u] * p.c2[1] + m[2][u] * p.c2[2];
+            const float a3 = m[0][u] * p.c3[0] + m[1][u] * p.c3[1] + m[2][u] * p.c3[2];
+            const float q1 = a1 * a1, q2 = a2 * a2, q3 = a3 * a3;
+            const float d1 = a1 * (p.k1c * (q2 + q3) + p.k2c * q2 * q3);
+            const float d2 = a2 * (p.k1c * (q3 + q1) + p.k2c * q3 * q1);
+            const float d3 = a3 * (p.k1c * (q1 + q2) + p.k2c * q1 * q2);
+#pragma unroll
+            for (int c = 0; c < 3; ++c) h[c][u] -= d1 * p.c1[c] + d2 * p.c2[c] + d3 * p.c3[c];
+        }
+    }
     // ---- thermal field (Eq. (6), reading A6) ----
     if (p.thermal) {
 #pragma unroll

@@ -213,6 +213,21 @@ void fill_material(const mm_ctx* c, EpiParams& p, uint64_t step, double dt_therm
         p.u[a] = un > 0 ? (float)(u[a] / un) : 0.f;
         p.hext[a] = (float)(M.Bext[a] / (MU0 * Ms));
     }
+    p.cubic = (M.K1 != 0.0 || M.K2 != 0.0) ? 1 : 0;
+    if (p.cubic) {
+        // reading A14: c1 normalised, c2 orthogonalised against c1, c3 = c1 x c2
+        double a[3] = { M.anis_c1[0], M.anis_c1[1], M.anis_c1[2] }, b[3] = { M.anis_c2[0], M.anis_c2[1], M.anis_c2[2] };
+        const double na = std::sqrt(a[0] * a[0] + a[1] * a[1] + a[2] * a[2]);
+        for (int i = 0; i < 3; ++i) a[i] /= na;
+        const double ab = a[0] * b[0] + a[1] * b[1] + a[2] * b[2];
+        for (int i = 0; i < 3; ++i) b[i] -= ab * a[i];
+        const double nb = std::sqrt(b[0] * b[0] + b[1] * b[1] + b[2] * b[2]);
+        for (int i = 0; i < 3; ++i) b[i] /= nb;
+        const double cc[3] = { a[1] * b[2] - a[2] * b[1], a[2] * b[0] - a[0] * b[2], a[0] * b[1] - a[1] * b[0] };
+        for (int i = 0; i < 3; ++i) { p.c1[i] = (float)a[i]; p.c2[i] = (float)b[i]; p.c3[i] = (float)cc[i]; }
+        p.k1c = (float)(2.0 * M.K1 / (MU0 * Ms * Ms));
+        p.k2c = (float)(2.0 * M.K2 / (MU0 * Ms * Ms));
+    }
     p.thermal = (M.T > 0.0 && dt_thermal > 0.0) ? 1 : 0;
     p.sig_th = 0.f;
     if (p.thermal) {
@@ -587,6 +602,12 @@ mm_status mm_set_material(mm_ctx* c, const mm_material* mat)
     if (mat->Aex < 0 || mat->alpha < 0 || mat->T < 0) return fail(c, MM_EINVAL, "Aex, alpha, T must be >= 0");
     if (mat->Ku != 0.0 && mat->anis_u[0] == 0.0 && mat->anis_u[1] == 0.0 && mat->anis_u[2] == 0.0)
         return fail(c, MM_EINVAL, "anisotropy axis is zero");
+    if (mat->K1 != 0.0 || mat->K2 != 0.0) {
+        const double* a = mat->anis_c1;
+        const double* b = mat->anis_c2;
+        const double cx = a[1] * b[2] - a[2] * b[1], cy = a[2] * b[0] - a[0] * b[2], cz = a[0] * b[1] - a[1] * b[0];
+        if (cx * cx + cy * cy + cz * cz == 0.0) return fail(c, MM_EINVAL, "cubic anisotropy axes are zero or parallel");
+    }
     c->mat = *mat;
     c->has_mat = true;
     c->k0_valid = false;

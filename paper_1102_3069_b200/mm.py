@@ -31,7 +31,8 @@ class Material(C.Structure):
     _fields_ = [("Ms", C.c_double), ("Aex", C.c_double), ("alpha", C.c_double), ("gamma0", C.c_double),
                 ("Ku", C.c_double), ("anis_u", C.c_double * 3), ("Bext", C.c_double * 3),
                 ("T", C.c_double), ("seed", C.c_uint64), ("j", C.c_double * 3), ("P", C.c_double),
-                ("xi", C.c_double), ("stt_literal_eq7", C.c_int), ("demag", C.c_int)]
+                ("xi", C.c_double), ("stt_literal_eq7", C.c_int), ("demag", C.c_int),
+                ("K1", C.c_double), ("K2", C.c_double), ("anis_c1", C.c_double * 3), ("anis_c2", C.c_double * 3)]
 
     @classmethod
     def from_dict(cls, d, demag=True):
@@ -45,6 +46,9 @@ class Material(C.Structure):
         m.P = d.get("P", 0.0); m.xi = d.get("xi", 0.0)
         m.stt_literal_eq7 = int(bool(d.get("stt_literal_eq7", False)))
         m.demag = int(bool(demag))
+        m.K1 = d.get("K1", 0.0); m.K2 = d.get("K2", 0.0)
+        m.anis_c1 = (C.c_double * 3)(*d.get("anis_c1", (1.0, 0.0, 0.0)))
+        m.anis_c2 = (C.c_double * 3)(*d.get("anis_c2", (0.0, 1.0, 0.0)))
         return m
 
 

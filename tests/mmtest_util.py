@@ -10,7 +10,9 @@ def oracle_material(matd):
                         gamma0=matd.get("gamma0") or orc.GAMMA0_DEFAULT, Ku=matd["Ku"],
                         anis_u=tuple(matd["anis_u"]), Bext=tuple(matd["Bext"]), T=matd["T"],
                         seed=matd["seed"], j=tuple(matd["j"]), P=matd["P"], xi=matd["xi"],
-                        stt_literal_eq7=bool(matd["stt_literal_eq7"]))
+                        stt_literal_eq7=bool(matd["stt_literal_eq7"]), K1=matd.get("K1", 0.0), K2=matd.get("K2", 0.0),
+                        anis_c1=tuple(matd.get("anis_c1", (1.0, 0.0, 0.0))),
+                        anis_c2=tuple(matd.get("anis_c2", (0.0, 1.0, 0.0))))
 
 
 def oracle_problem(wl, demag="fft"):

@@ -579,3 +579,29 @@ def test_graph_replay_with_thermal_field_draws_per_step(monkeypatch):
     for s_ in range(14):
         mo = orc.rk4_step(lambda x: pb.torque(x, s_, 5e-14), mo, 5e-14)
     assert np.abs(out[0].astype(np.float64) - mo).max() <= TOL_M
+
+
+@pytest.mark.parametrize("grid,fast", [((24, 10, 6), 0), ((64, 32, 32), 63), ((15, 9, 5), 0)])
+def test_cubic_anisotropy_matches_oracle(grid, fast):
+    """Eq. (5) with tilted axes, next to every other field term."""
+    wl = util.small(grid, (3e-9, 4e-9, 5e-9), K1=-4.5e4, K2=2.3e4, anis_c1=(1.0, 1.0, 0.0), anis_c2=(-1.0, 1.0, 0.3),
+                    j=(1e12, 0, 0), P=0.5, xi=0.04)
+    m = wlm.initial_m(wl)
+    m64 = m.astype(np.float64)
+    pb = util.oracle_problem(wl)
+    sim = util.gpu_sim(wl, fast=fast)
+    md = util.to_dev(m)
+    _cmp(sim.heff(md), pb.heff(m64), TOL_H)
+    _cmp(sim.torque(md), pb.torque(m64), TOL_H)
+    # the cubic term on its own scale: switch everything else off
+    wl2 = util.small(grid, (3e-9, 4e-9, 5e-9), K1=-4.5e4, K2=2.3e4, anis_c1=(1.0, 1.0, 0.0), anis_c2=(-1.0, 1.0, 0.3),
+                     Aex=0.0, Ku=0.0, Bext=(0.0, 0.0, 0.0))
+    sim2 = util.gpu_sim(wl2, demag=False)
+    ref = orc.cubic_anisotropy_field(m64, util.oracle_material(wl2.mat))
+    _cmp(sim2.heff(md), ref, 2e-6)
+    mo = m64.copy()
+    for _ in range(5):
+        mo = orc.rk4_step(pb.torque, mo, 5e-14)
+    sim.steps_fixed(md, "rk4", 5e-14, 5)
+    assert np.abs(md.double().cpu().numpy() - mo).max() <= TOL_M
+    sim.close(); sim2.close()
