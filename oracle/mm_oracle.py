@@ -96,6 +96,7 @@ class Material:
     K2: float = 0.0                 # J/m^3      Eq. (5)
     anis_c1: tuple = (1.0, 0.0, 0.0)   # first two cubic axes; the third is c1 x c2 (reading A14)
     anis_c2: tuple = (0.0, 1.0, 0.0)
+    exchange_in_kernel: bool = False   # exchange added to the convolution kernel (reading A3')
 
 
 # --------------------------------------------------------------------------
@@ -294,6 +295,35 @@ def exchange_field(m, mat: Material, grid, cell, pbc=(0, 0, 0)) -> np.ndarray:
     return H
 
 
+def exchange_field_in_kernel(m, mat: Material, grid, cell, pbc=(0, 0, 0)) -> np.ndarray:
+    """The paper's own variant (reading A3'): the exchange stencil is added to the
+    magnetostatic kernel, so at an open face the zero padding of the convolution makes a missing
+    neighbour count as m = 0:  H_ex(i) = 2A/(mu0 Ms) sum_a [ m_(i+a) + m_(i-a) - 2 m_i ] / d_a^2 with
+    m = 0 outside the grid.  Written here as exactly that sum (no convolution)."""
+    H = np.zeros_like(m, dtype=np.float64)
+    if mat.Aex == 0.0:
+        return H
+    pref = 2.0 * mat.Aex / (MU0 * mat.Ms)
+    for ax, (n, d, p) in enumerate(((grid[2], cell[2], pbc[2]), (grid[1], cell[1], pbc[1]),
+                                    (grid[0], cell[0], pbc[0]))):
+        if n == 1:
+            continue
+        a = ax + 1
+        if p > 0:
+            H += pref * (np.roll(m, 1, axis=a) + np.roll(m, -1, axis=a) - 2.0 * m) / d ** 2
+        else:
+            mp = np.zeros_like(m, dtype=np.float64)      # m_(i+a), zero beyond the last cell
+            mm = np.zeros_like(m, dtype=np.float64)      # m_(i-a), zero before the first cell
+            up = [slice(None)] * 4
+            dn = [slice(None)] * 4
+            up[a] = slice(1, None)
+            dn[a] = slice(None, -1)
+            mp[tuple(dn)] = m[tuple(up)]
+            mm[tuple(up)] = m[tuple(dn)]
+            H += pref * (mp + mm - 2.0 * m) / d ** 2
+    return H
+
+
 def anisotropy_field(m, mat: Material) -> np.ndarray:
     """From the energy density Eq. (4): E = Ku sin^2(theta) = Ku (1 - (m.u)^2)
     => H = -(1/(mu0 Ms)) dE/dm = 2 Ku/(mu0 Ms) (m.u) u   (reading A5)."""
@@ -438,7 +468,10 @@ class Problem:
         """H_eff = H_ms + H_ex + H_an + H_ext + H_th  (PAPER.md:59), in A/m."""
         m = np.asarray(m, dtype=np.float64)
         H = self.demag_field(m)
-        H = H + exchange_field(m, self.mat, self.grid, self.cell, self.pbc)
+        if self.mat.exchange_in_kernel:
+            H = H + exchange_field_in_kernel(m, self.mat, self.grid, self.cell, self.pbc)
+        else:
+            H = H + exchange_field(m, self.mat, self.grid, self.cell, self.pbc)
         H = H + anisotropy_field(m, self.mat)
         H = H + cubic_anisotropy_field(m, self.mat)
         H = H + zeeman_field(m, self.mat)

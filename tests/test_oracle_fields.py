@@ -150,6 +150,44 @@ def test_exchange_open_boundary_is_neumann_and_matches_brute_force():
                 assert np.allclose(H[:, z, y, x], h, rtol=1e-12)
 
 
+def test_exchange_in_kernel_variant_differs_only_at_open_faces_and_gives_the_same_torque():
+    """PAPER.md:85 (reading A3').  Pins: (i) interior cells: identical to the free-boundary stencil;
+    (ii) a cell with k missing neighbours along axis a differs by exactly -(2A/mu0 Ms d_a^2) k m_i, a field
+    parallel to m_i; hence (iii) the torque is the same under both readings; (iv) periodic axes: identical;
+    (v) it equals the circular convolution of the zero-padded m with the stencil kernel."""
+    rng = np.random.default_rng(8)
+    grid, cell = (6, 5, 4), (3e-9, 4e-9, 5e-9)
+    mat = orc.Material(Ms=8e5, Aex=1.3e-11, alpha=0.1)
+    m = rng.standard_normal((3, grid[2], grid[1], grid[0]))
+    m /= np.sqrt((m * m).sum(0))
+    Hn = orc.exchange_field(m, mat, grid, cell)
+    Hk = orc.exchange_field_in_kernel(m, mat, grid, cell)
+    assert np.allclose(Hn[:, 1:-1, 1:-1, 1:-1], Hk[:, 1:-1, 1:-1, 1:-1], rtol=0, atol=1e-6)
+    pref = 2 * mat.Aex / (orc.MU0 * mat.Ms)
+    miss = np.zeros(m.shape[1:])
+    for a, (n, d) in zip((2, 1, 0), zip(grid, cell)):           # array axes z, y, x <-> grid x, y, z reversed
+        pass
+    for ax_arr, n, d in ((2, grid[0], cell[0]), (1, grid[1], cell[1]), (0, grid[2], cell[2])):
+        idx = np.arange(n)
+        k = ((idx == 0).astype(float) + (idx == n - 1).astype(float)) / d ** 2
+        shape = [1, 1, 1]; shape[ax_arr] = n
+        miss = miss + k.reshape(shape)
+    assert np.allclose(Hk - Hn, -pref * miss[None] * m, rtol=0, atol=1e-6 * np.abs(Hn).max())
+    assert np.allclose(orc.ll_torque(m, Hk, mat), orc.ll_torque(m, Hn, mat), rtol=0, atol=1e-9 * np.abs(orc.ll_torque(m, Hn, mat)).max())
+    assert np.allclose(orc.exchange_field(m, mat, grid, cell, (1, 1, 1)), orc.exchange_field_in_kernel(m, mat, grid, cell, (1, 1, 1)))
+    # (v) circular convolution of the padded state with the stencil
+    P = [2 * n for n in grid]
+    ker = np.zeros((P[2], P[1], P[0]))
+    for ax_arr, d in ((2, cell[0]), (1, cell[1]), (0, cell[2])):
+        ker[0, 0, 0] -= 2 * pref / d ** 2
+        for sgn in (1, -1):
+            i = [0, 0, 0]; i[ax_arr] = sgn
+            ker[tuple(i)] += pref / d ** 2
+    mp = np.zeros((3, P[2], P[1], P[0])); mp[:, :grid[2], :grid[1], :grid[0]] = m
+    conv = np.fft.ifftn(np.fft.fftn(mp, axes=(1, 2, 3)) * np.fft.fftn(ker)[None], axes=(1, 2, 3)).real
+    assert np.allclose(conv[:, :grid[2], :grid[1], :grid[0]], Hk, rtol=0, atol=1e-8 * np.abs(Hk).max())
+
+
 def test_anisotropy_special_cases():
     mat = orc.Material(Ms=1.1e6, Ku=5e5, anis_u=(0.0, 0.0, 2.0))
     m = np.zeros((3, 1, 1, 2))
