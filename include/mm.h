@@ -75,6 +75,9 @@ typedef struct {
     int stt_literal_eq7; /* 0: (1 + alpha xi) on the adiabatic term; 1: Eq. (7) as printed (A7)   */
     int demag;        /* 1: magnetostatic field on (default use); 0: off (tests of local terms)   */
     double K1, K2;    /* cubic anisotropy constants, J/m^3         Eq. (5)            */
+    int exchange_in_kernel; /* 1: the paper's variant (reading A3'): the exchange stencil is added
+                       * to the convolution kernel, so a missing neighbour at an open face counts as m = 0;
+                       * 0 (default): stencil in the epilogue, free boundary (reading A3).  Needs demag = 1. */
     double anis_c1[3], anis_c2[3]; /* first two cubic axes; c2 is made orthogonal to c1, c3 = c1 x c2
                        * (reading A14); ignored if K1 == K2 == 0                                 */
 } mm_material;

@@ -131,7 +131,8 @@ struct mm_ctx {
     cudaEvent_t gev[2];
     int use_graph;    // mm_steps_fixed may replay a captured step (env MM_GRAPH=0 switches it off)
     // device
-    float* khat;
+    float* khat;      // demag kernel octant
+    float* khat_ex;   // khat + exchange stencil on the diagonal (exchange_in_kernel), built at mm_set_material
     float2 *specA, *specB;
     float2* tw[3];
     FftPlan plan[3];
@@ -204,8 +205,9 @@ void fill_material(const mm_ctx* c, EpiParams& p, uint64_t step, double dt_therm
     const double g0 = M.gamma0 > 0 ? M.gamma0 : GAMMA0_DEFAULT;
     const int ext[3] = { g.Nx, g.Ny, g.Nz };
     p.demag = M.demag ? 1 : 0;
+    const bool ex_in_k = M.exchange_in_kernel && M.demag;      // then the convolution carries the exchange field
     for (int a = 0; a < 3; ++a)
-        p.wex[a] = ext[a] > 1 ? (float)(2.0 * M.Aex / (MU0 * Ms * Ms * c->cell[a] * c->cell[a])) : 0.f;
+        p.wex[a] = (ext[a] > 1 && !ex_in_k) ? (float)(2.0 * M.Aex / (MU0 * Ms * Ms * c->cell[a] * c->cell[a])) : 0.f;
     double u[3] = { M.anis_u[0], M.anis_u[1], M.anis_u[2] };
     const double un = std::sqrt(u[0] * u[0] + u[1] * u[1] + u[2] * u[2]);
     p.kan = (M.Ku != 0.0 && un > 0) ? (float)(2.0 * M.Ku / (MU0 * Ms * Ms)) : 0.f;
@@ -266,6 +268,9 @@ mm_status launch_eval(mm_ctx* c, const EpiParams& ep)
     cudaStream_t st = c->stream;
     const FastPlan& fp = c->fp;
     size_t bytes;
+    // mm_demag_field (EPI_HMS) always uses the pure magnetostatic kernel
+    const float* kh = (ep.mode != EPI_HMS && c->mat.exchange_in_kernel && c->mat.demag && c->khat_ex) ? c->khat_ex
+                                                                                                       : c->khat;
     if (ep.demag) {
         {   // a1
             c->kt.begin(KT_FWD_X);
@@ -280,7 +285,7 @@ mm_status launch_eval(mm_ctx* c, const EpiParams& ep)
         if (g.Pz > 1 && (c->fast & FAST_CHUNK) && (c->fast & FAST_Y) && (c->fast & FAST_MID) && fp.chunk_w > 0) {
             // a2-a4 chunked over kx so that the y-padded spectrum stays in L2 (timed as one category)
             c->kt.begin(KT_MID);
-            if (!fast_yzy_chunked(c->fp, g, st, c->specA, c->specB, c->khat))
+            if (!fast_yzy_chunked(c->fp, g, st, c->specA, c->specB, kh))
                 return fail(c, MM_ECUDA, "chunked y-z-y launch failed");
             c->kt.end(KT_MID);
             c->kt.launches += 3 * ((g.Cx + fp.chunk_w - 1) / fp.chunk_w) - 1;
@@ -298,11 +303,11 @@ mm_status launch_eval(mm_ctx* c, const EpiParams& ep)
             }
             {   // a3
                 c->kt.begin(KT_MID);
-                if (!((c->fast & FAST_MID) && fast_mid3(fp, g, st, wt, c->specB, c->khat))) {
+                if (!((c->fast & FAST_MID) && fast_mid3(fp, g, st, wt, c->specB, kh))) {
                     const int tx = pick_tx(g.Pz, 4, 1, &bytes);
                     if (!tx) return fail(c, MM_EUNSUPPORTED, "z line too long for the shared-memory tile");
                     dim3 grid((g.Cx + tx - 1) / tx, g.Py);
-                    k_gen_mid<<<grid, 256, bytes, st>>>(g, c->plan[2], c->specB, c->khat, 2, tx);
+                    k_gen_mid<<<grid, 256, bytes, st>>>(g, c->plan[2], c->specB, kh, 2, tx);
                 }
                 c->kt.end(KT_MID);
             }
@@ -324,7 +329,7 @@ mm_status launch_eval(mm_ctx* c, const EpiParams& ep)
                 fast_y(fp, g, st, -1, wt, c->specA, c->specB);
                 c->kt.end(KT_FWD_Y);
                 c->kt.begin(KT_MID);
-                fast_mul2(fp, g, st, c->specB, c->khat);
+                fast_mul2(fp, g, st, c->specB, kh);
                 c->kt.end(KT_MID);
                 c->kt.begin(KT_INV_Y);
                 fast_y(fp, g, st, 1, wt, c->specA, c->specB);
@@ -333,7 +338,7 @@ mm_status launch_eval(mm_ctx* c, const EpiParams& ep)
                 // generic: y forward, multiply, y inverse in one kernel
                 dim3 grid((g.Cx + tx - 1) / tx, 1);
                 c->kt.begin(KT_MID);
-                k_gen_mid<<<grid, 256, bytes, st>>>(g, c->plan[1], c->specA, c->khat, 1, tx);
+                k_gen_mid<<<grid, 256, bytes, st>>>(g, c->plan[1], c->specA, kh, 1, tx);
                 c->kt.end(KT_MID);
             } else {
                 // very long y lines (four tile buffers do not fit): three launches through specB
@@ -345,7 +350,7 @@ mm_status launch_eval(mm_ctx* c, const EpiParams& ep)
                 c->kt.end(KT_FWD_Y);
                 c->kt.begin(KT_MID);
                 dim3 gm((g.Cx + 255) / 256, g.Py);
-                ff::k_mul2d<<<gm, 256, 0, st>>>(g, c->specB, c->khat);
+                ff::k_mul2d<<<gm, 256, 0, st>>>(g, c->specB, kh);
                 c->kt.end(KT_MID);
                 c->kt.begin(KT_INV_Y);
                 k_gen_y<1><<<grid, 256, bytes, st>>>(g, c->plan[1], c->specB, c->specA, ty);
@@ -353,7 +358,7 @@ mm_status launch_eval(mm_ctx* c, const EpiParams& ep)
             }
         } else {
             c->kt.begin(KT_MID);
-            k_gen_mul1d<<<(g.Cx + 127) / 128, 128, 0, st>>>(g, c->specA, c->khat);
+            k_gen_mul1d<<<(g.Cx + 127) / 128, 128, 0, st>>>(g, c->specA, kh);
             c->kt.end(KT_MID);
         }
     }
@@ -391,6 +396,26 @@ mm_status launch_eval(mm_ctx* c, const EpiParams& ep)
     return MM_OK;
 }
 
+__global__ void k_khat_exchange(Geom g, const float* __restrict__ khat, float* __restrict__ out, float wx, float wy,
+                                float wz);
+
+// (re)build khat_ex = khat + exchange stencil when the material asks for the paper's variant
+mm_status refresh_khat_ex(mm_ctx* c)
+{
+    if (!(c->has_mat && c->has_demag && c->mat.exchange_in_kernel && c->mat.demag)) return MM_OK;
+    const Geom& g = c->g;
+    const size_t nK = (size_t)6 * g.Cz * g.Cy * g.CxK;
+    if (!c->khat_ex) CUDA_TRY(c, cudaMalloc(&c->khat_ex, nK * sizeof(float)));
+    const double Ms = c->mat.Ms;
+    const int ext[3] = { g.Nx, g.Ny, g.Nz };
+    float w[3];
+    for (int a = 0; a < 3; ++a)
+        w[a] = ext[a] > 1 ? (float)(2.0 * c->mat.Aex / (MU0 * Ms * Ms * c->cell[a] * c->cell[a])) : 0.f;
+    k_khat_exchange<<<148 * 8, 256, 0, c->stream>>>(g, c->khat, c->khat_ex, w[0], w[1], w[2]);
+    CUDA_TRY(c, cudaGetLastError());
+    return MM_OK;
+}
+
 mm_status check_ready(mm_ctx* c)
 {
     if (!c) return MM_EINVAL;
@@ -421,6 +446,30 @@ __global__ void k_normalise(size_t n, const float* __restrict__ src, float* __re
         const float x = src[i], y = src[i + n], z = src[i + 2 * n];
         const float s = rsqrtf(x * x + y * y + z * z);
         dst[i] = x * s; dst[i + n] = y * s; dst[i + 2 * n] = z * s;
+    }
+}
+
+// K-hat with the exchange stencil added to its diagonal: in k space the 6-neighbour stencil
+// is sum_a w_a (2 cos(2 pi k_a / P_a) - 2); the convolution carries the factor 1/(Px Py Pz) of K-hat.
+__global__ void k_khat_exchange(Geom g, const float* __restrict__ khat, float* __restrict__ out, float wx, float wy,
+                                float wz)
+{
+    const size_t nC = (size_t)g.CxK * g.Cy * g.Cz;
+    const float norm = 1.0f / ((float)g.Px * (float)g.Py * (float)g.Pz);
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < 6 * nC; i += (size_t)gridDim.x * blockDim.x) {
+        const size_t r = i % nC;
+        const int comp = (int)(i / nC);
+        float v = khat[i];
+        if (comp < 3) {
+            const int kx = (int)(r % g.CxK), ky = (int)((r / g.CxK) % g.Cy), kz = (int)(r / ((size_t)g.CxK * g.Cy));
+            if (kx < g.Cx) {
+                const float ex = wx * (2.0f * cospif(2.0f * kx / (float)g.Px) - 2.0f) +
+                                 wy * (2.0f * cospif(2.0f * ky / (float)g.Py) - 2.0f) +
+                                 wz * (2.0f * cospif(2.0f * kz / (float)g.Pz) - 2.0f);
+                v += norm * ex;
+            }
+        }
+        out[i] = v;
     }
 }
 
@@ -578,7 +627,7 @@ mm_status mm_create(mm_ctx** out, const int grid[3], const double cellsize[3], c
     c->gstream = nullptr;
     c->gev[0] = c->gev[1] = nullptr;
     c->use_graph = getenv("MM_GRAPH") ? atoi(getenv("MM_GRAPH")) : 1;
-    c->khat = nullptr; c->specA = c->specB = nullptr;
+    c->khat = nullptr; c->khat_ex = nullptr; c->specA = c->specB = nullptr;
     for (int a = 0; a < 3; ++a) c->tw[a] = nullptr;
     for (int i = 0; i < 7; ++i) c->kb[i] = nullptr;
     c->ms[0] = c->ms[1] = c->mtmp = nullptr;
@@ -611,7 +660,7 @@ mm_status mm_set_material(mm_ctx* c, const mm_material* mat)
     c->mat = *mat;
     c->has_mat = true;
     c->k0_valid = false;
-    return MM_OK;
+    return refresh_khat_ex(c);
 }
 
 mm_status mm_demag_init(mm_ctx* c)
@@ -676,7 +725,7 @@ mm_status mm_demag_init(mm_ctx* c)
     std::string ferr;
     if (!fast_plan_init(c->fp, g, &ferr)) return fail(c, MM_ECUDA, ferr);
     c->has_demag = true;
-    return MM_OK;
+    return refresh_khat_ex(c);
 }
 
 static mm_status eval_to(mm_ctx* c, const float* m_dev, float* out, int mode, uint64_t step, double dt_th)
@@ -1202,6 +1251,7 @@ void mm_destroy(mm_ctx* c)
 {
     if (!c) return;
     cudaFree(c->khat);
+    cudaFree(c->khat_ex);
     cudaFree(c->specA);
     cudaFree(c->specB);
     for (int a = 0; a < 3; ++a) cudaFree(c->tw[a]);

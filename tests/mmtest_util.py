@@ -12,7 +12,8 @@ def oracle_material(matd):
                         seed=matd["seed"], j=tuple(matd["j"]), P=matd["P"], xi=matd["xi"],
                         stt_literal_eq7=bool(matd["stt_literal_eq7"]), K1=matd.get("K1", 0.0), K2=matd.get("K2", 0.0),
                         anis_c1=tuple(matd.get("anis_c1", (1.0, 0.0, 0.0))),
-                        anis_c2=tuple(matd.get("anis_c2", (0.0, 1.0, 0.0))))
+                        anis_c2=tuple(matd.get("anis_c2", (0.0, 1.0, 0.0))),
+                        exchange_in_kernel=bool(matd.get("exchange_in_kernel", False)))
 
 
 def oracle_problem(wl, demag="fft"):

@@ -605,3 +605,29 @@ def test_cubic_anisotropy_matches_oracle(grid, fast):
     sim.steps_fixed(md, "rk4", 5e-14, 5)
     assert np.abs(md.double().cpu().numpy() - mo).max() <= TOL_M
     sim.close(); sim2.close()
+
+
+@pytest.mark.parametrize("grid,pbc,fast", [((24, 10, 6), (0, 0, 0), 0), ((64, 32, 32), (0, 0, 0), 63),
+                                           ((16, 12, 1), (2, 2, 0), 0), ((32, 32, 32), (0, 1, 0), 63)])
+def test_exchange_inside_the_kernel_variant(grid, pbc, fast):
+    """SURVEY 8(f) row f-2, PAPER.md:85 (reading A3'): the exchange stencil rides on the convolution
+    kernel; H_eff changes only at open faces (by a field parallel to m), the torque not at all."""
+    wl = util.small(grid, (3e-9, 4e-9, 5e-9), pbc, exchange_in_kernel=True)
+    wl0 = util.small(grid, (3e-9, 4e-9, 5e-9), pbc)
+    m = wlm.initial_m(wl)
+    m64 = m.astype(np.float64)
+    pb = util.oracle_problem(wl)
+    sim = util.gpu_sim(wl, fast=fast)
+    md = util.to_dev(m)
+    H = sim.heff(md)
+    _cmp(H, pb.heff(m64), TOL_H)
+    _cmp(sim.torque(md), pb.torque(m64), TOL_H)
+    _cmp(sim.demag_field(md), pb.demag_field(m64), TOL_H)          # the pure magnetostatic field is unchanged
+    sim0 = util.gpu_sim(wl0, fast=fast)
+    T0, T1 = sim0.torque(md).double(), sim.torque(md).double()
+    assert float((T0 - T1).abs().max()) <= 5e-5 * float(T0.abs().max())
+    if tuple(pbc) == (0, 0, 0):
+        d = (H - sim0.heff(md)).double()
+        assert float(d[:, 1:-1, 1:-1, 1:-1].abs().max()) <= 2e-5 * float(H.abs().max())   # interior: same field
+        assert float(d.abs().max()) > 1e-2 * float(H.abs().max())                           # faces: not
+    sim.close(); sim0.close()
