@@ -448,7 +448,17 @@ k_epi4(Geom g, const float* __restrict__ hms, EpiParams ep)
         }
     }
     unsigned int red = 0u;
-    if (active) {
+    // no neighbour is needed when the exchange rides on the convolution kernel and no current flows
+    const bool need_nb = ep.wex[0] != 0.f || ep.wex[1] != 0.f || ep.wex[2] != 0.f || ep.stt;
+    if (active && !need_nb) {
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            ldv<4>(hms + idx + c * n, h[c]);
+#pragma unroll
+            for (int u = 0; u < 4; ++u) D[c][u] = 0.f;
+        }
+        red = __float_as_uint(epilogue_finish_v<4>(ep, idx, n, m, h, D)) & 0x7fffffffu;
+    } else if (active) {
         const int ym = y > 0 ? y - 1 : (g.pery ? g.Ny - 1 : y);
         const int yp = y + 1 < g.Ny ? y + 1 : (g.pery ? 0 : y);
         const int zm = z > 0 ? z - 1 : (g.perz ? g.Nz - 1 : z);
