@@ -97,6 +97,7 @@ class Material:
     anis_c1: tuple = (1.0, 0.0, 0.0)   # first two cubic axes; the third is c1 x c2 (reading A14)
     anis_c2: tuple = (0.0, 1.0, 0.0)
     exchange_in_kernel: bool = False   # exchange added to the convolution kernel (reading A3')
+    geometry: bool = False          # cells with m = 0 are empty (staircase shapes, reading A15)
 
 
 # --------------------------------------------------------------------------
@@ -295,6 +296,34 @@ def exchange_field(m, mat: Material, grid, cell, pbc=(0, 0, 0)) -> np.ndarray:
     return H
 
 
+def _shifted(m, a, sgn, n, periodic):
+    """m_(i + sgn e_a) with the cell itself where that neighbour does not exist (open face)."""
+    if periodic:
+        return np.roll(m, -sgn, axis=a)
+    idx = np.arange(n)
+    return np.take(m, np.clip(idx + sgn, 0, n - 1), axis=a)
+
+
+def exchange_field_geometry(m, mat: Material, grid, cell, pbc=(0, 0, 0)) -> np.ndarray:
+    """Eq. (3) on a staircase shape (reading A15): cells with m = 0 are empty.  An empty
+    neighbour counts as a missing one (free boundary, as reading A3: it contributes zero), and an empty
+    cell has no exchange field."""
+    H = np.zeros_like(m, dtype=np.float64)
+    if mat.Aex == 0.0:
+        return H
+    pref = 2.0 * mat.Aex / (MU0 * mat.Ms)
+    full = (np.sum(m * m, axis=0, keepdims=True) > 0.0)
+    for a, comp in ((3, 0), (2, 1), (1, 2)):
+        n, d = grid[comp], cell[comp]
+        if n == 1:
+            continue
+        for sgn in (1, -1):
+            nb = _shifted(m, a, sgn, n, pbc[comp] > 0)
+            nb_full = _shifted(full, a, sgn, n, pbc[comp] > 0)
+            H += pref * np.where(nb_full & full, nb - m, 0.0) / d ** 2
+    return H
+
+
 def exchange_field_in_kernel(m, mat: Material, grid, cell, pbc=(0, 0, 0)) -> np.ndarray:
     """The paper's own variant (reading A3'): the exchange stencil is added to the
     magnetostatic kernel, so at an open face the zero padding of the convolution makes a missing
@@ -468,7 +497,9 @@ class Problem:
         """H_eff = H_ms + H_ex + H_an + H_ext + H_th  (PAPER.md:59), in A/m."""
         m = np.asarray(m, dtype=np.float64)
         H = self.demag_field(m)
-        if self.mat.exchange_in_kernel:
+        if self.mat.geometry:
+            H = H + exchange_field_geometry(m, self.mat, self.grid, self.cell, self.pbc)
+        elif self.mat.exchange_in_kernel:
             H = H + exchange_field_in_kernel(m, self.mat, self.grid, self.cell, self.pbc)
         else:
             H = H + exchange_field(m, self.mat, self.grid, self.cell, self.pbc)
@@ -504,6 +535,9 @@ def j_dot_grad_m(m, mat: Material, grid, cell, pbc) -> np.ndarray:
             idx = np.arange(n)
             up = np.take(m, np.minimum(idx + 1, n - 1), axis=a_m)
             dn = np.take(m, np.maximum(idx - 1, 0), axis=a_m)
+        if mat.geometry:          # reading A15: an empty neighbour is replaced by the cell itself
+            up = np.where(np.sum(up * up, axis=0, keepdims=True) > 0.0, up, m)
+            dn = np.where(np.sum(dn * dn, axis=0, keepdims=True) > 0.0, dn, m)
         out += ja * (up - dn) / (2.0 * cell[comp])
     return out
 
@@ -579,7 +613,9 @@ TABLEAUX = {
 
 
 def _normalise(m):
-    return m / np.sqrt(np.sum(m * m, axis=0, keepdims=True))
+    """Unit vectors; the zero vector of an empty cell (reading A15) stays zero."""
+    n = np.sqrt(np.sum(m * m, axis=0, keepdims=True))
+    return np.where(n > 0.0, m / np.where(n > 0.0, n, 1.0), 0.0)
 
 
 def rk4_step(f, m, dt):

@@ -188,6 +188,41 @@ def test_exchange_in_kernel_variant_differs_only_at_open_faces_and_gives_the_sam
     assert np.allclose(conv[:, :grid[2], :grid[1], :grid[0]], Hk, rtol=0, atol=1e-8 * np.abs(Hk).max())
 
 
+def test_exchange_on_a_staircase_shape():
+    """Reading A15.  Pins: (i) no empty cell: the plain stencil; (ii) an L-shaped sample
+    against plain Python loops over cell pairs; (iii) uniform m on any shape: zero; (iv) empty cells get
+    no field, and normalisation leaves them empty."""
+    rng = np.random.default_rng(4)
+    grid, cell = (5, 4, 3), (3e-9, 4e-9, 5e-9)
+    mat = orc.Material(Ms=8e5, Aex=1.3e-11, geometry=True)
+    m = rng.standard_normal((3, grid[2], grid[1], grid[0]))
+    m /= np.sqrt((m * m).sum(0))
+    assert np.allclose(orc.exchange_field_geometry(m, mat, grid, cell), orc.exchange_field(m, mat, grid, cell))
+    shape = np.ones((grid[2], grid[1], grid[0]), dtype=bool)
+    shape[:, 2:, 3:] = False                       # cut a corner out: L shape
+    shape[1, 1, 1] = False                         # and a hole
+    mg = m * shape[None]
+    H = orc.exchange_field_geometry(mg, mat, grid, cell)
+    pref = 2 * mat.Aex / (orc.MU0 * mat.Ms)
+    ref = np.zeros_like(mg)
+    for z in range(grid[2]):
+        for y in range(grid[1]):
+            for x in range(grid[0]):
+                if not shape[z, y, x]:
+                    continue
+                for dz, dy, dx, d in ((0, 0, 1, cell[0]), (0, 0, -1, cell[0]), (0, 1, 0, cell[1]), (0, -1, 0, cell[1]),
+                                      (1, 0, 0, cell[2]), (-1, 0, 0, cell[2])):
+                    zz, yy, xx = z + dz, y + dy, x + dx
+                    if 0 <= zz < grid[2] and 0 <= yy < grid[1] and 0 <= xx < grid[0] and shape[zz, yy, xx]:
+                        ref[:, z, y, x] += pref * (mg[:, zz, yy, xx] - mg[:, z, y, x]) / d ** 2
+    assert np.allclose(H, ref, rtol=0, atol=1e-9 * np.abs(ref).max())
+    assert np.all(H[:, ~shape] == 0.0)
+    mu = np.zeros_like(m); mu[0] = 1.0
+    assert np.abs(orc.exchange_field_geometry(mu * shape[None], mat, grid, cell)).max() == 0.0
+    nrm = orc._normalise(1.7 * mg)
+    assert np.all(nrm[:, ~shape] == 0.0) and np.allclose((nrm * nrm).sum(0)[shape], 1.0)
+
+
 def test_anisotropy_special_cases():
     mat = orc.Material(Ms=1.1e6, Ku=5e5, anis_u=(0.0, 0.0, 2.0))
     m = np.zeros((3, 1, 1, 2))
