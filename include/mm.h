@@ -78,6 +78,8 @@ typedef struct {
     int exchange_in_kernel; /* 1: the paper's variant (reading A3'): the exchange stencil is added
                        * to the convolution kernel, so a missing neighbour at an open face counts as m = 0;
                        * 0 (default): stencil in the epilogue, free boundary (reading A3).  Needs demag = 1. */
+    int geometry;     /* 1: cells whose m is the zero vector are empty (staircase shapes; reading
+                       * A15): no exchange / current coupling to them, they stay empty.  0 (default).      */
     double anis_c1[3], anis_c2[3]; /* first two cubic axes; c2 is made orthogonal to c1, c3 = c1 x c2
                        * (reading A14); ignored if K1 == K2 == 0                                 */
 } mm_material;

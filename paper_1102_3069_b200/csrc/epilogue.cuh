@@ -201,7 +201,8 @@ __device__ __forceinline__ float epilogue_finish_v(const EpiParams& p, size_t id
         if (p.normalise) {
 #pragma unroll
             for (int u = 0; u < V; ++u) {
-                const float s = rsqrtf(r[0][u] * r[0][u] + r[1][u] * r[1][u] + r[2][u] * r[2][u]);
+                const float q = r[0][u] * r[0][u] + r[1][u] * r[1][u] + r[2][u] * r[2][u];
+                const float s = q > 0.f ? rsqrtf(q) : 0.f;        // an empty cell stays empty (reading A15)
                 r[0][u] *= s; r[1][u] *= s; r[2][u] *= s;
             }
         }
@@ -286,11 +287,17 @@ __device__ __forceinline__ float epilogue_cell(const Geom& g, const EpiParams& p
             else if (per[a]) ip = idx - (size_t)(ext[a] - 1) * str[a];
             if (pos[a] > 0) im = idx - str[a];
             else if (per[a]) im = idx + (size_t)(ext[a] - 1) * str[a];
+            float mp[3] = { mi[ip], mi[ip + n], mi[ip + 2 * n] };
+            float mm_[3] = { mi[im], mi[im + n], mi[im + 2 * n] };
+            if (p.geometry) {     // reading A15: an empty neighbour is a missing one; an empty cell has no field
+                const bool full = m[0] * m[0] + m[1] * m[1] + m[2] * m[2] > 0.f;
+                if (!full || !(mp[0] * mp[0] + mp[1] * mp[1] + mp[2] * mp[2] > 0.f)) { mp[0] = m[0]; mp[1] = m[1]; mp[2] = m[2]; }
+                if (!full || !(mm_[0] * mm_[0] + mm_[1] * mm_[1] + mm_[2] * mm_[2] > 0.f)) { mm_[0] = m[0]; mm_[1] = m[1]; mm_[2] = m[2]; }
+            }
 #pragma unroll
             for (int c = 0; c < 3; ++c) {
-                const float mp = mi[ip + c * n], mm_ = mi[im + c * n];
-                h[c] += p.wex[a] * ((mp - m[c]) + (mm_ - m[c]));
-                D[c] += p.cj[a] * (mp - mm_);
+                h[c] += p.wex[a] * ((mp[c] - m[c]) + (mm_[c] - m[c]));
+                D[c] += p.cj[a] * (mp[c] - mm_[c]);
             }
         }
     }
@@ -404,6 +411,23 @@ __device__ __forceinline__ void block_max_atomic(unsigned int b, unsigned int* t
         for (int o = 16; o > 0; o >>= 1) b = max(b, __shfl_xor_sync(0xffffffffu, b, o));
         if (lane == 0 && b != 0u) atomicMax(target, b);
     }
+}
+
+// a6-a10 as a streaming kernel, one thread per cell (any Nx; staircase geometry, reading A15): the per-cell
+// tail of the generic path on the H_ms field the inverse x pass has left.
+__global__ void __launch_bounds__(256)
+k_epi1(Geom g, const float* __restrict__ hms, EpiParams ep)
+{
+    const size_t n = (size_t)g.Nx * g.Ny * g.Nz;
+    size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    unsigned int red = 0u;
+    if (i < n) {
+        const int x = (int)(i % g.Nx);
+        const size_t yz = i / g.Nx;
+        const int y = (int)(yz % g.Ny), z = (int)(yz / g.Ny);
+        red = __float_as_uint(epilogue_cell(g, ep, x, y, z, hms[i], hms[i + n], hms[i + 2 * n])) & 0x7fffffffu;
+    }
+    if (ep.do_err) block_max_atomic(red, ep.maxbits);
 }
 
 // ---------------------------------------------------------------------------------------------

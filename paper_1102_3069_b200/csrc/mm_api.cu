@@ -215,6 +215,7 @@ void fill_material(const mm_ctx* c, EpiParams& p, uint64_t step, double dt_therm
         p.u[a] = un > 0 ? (float)(u[a] / un) : 0.f;
         p.hext[a] = (float)(M.Bext[a] / (MU0 * Ms));
     }
+    p.geometry = M.geometry ? 1 : 0;
     p.cubic = (M.K1 != 0.0 || M.K2 != 0.0) ? 1 : 0;
     if (p.cubic) {
         // reading A14: c1 normalised, c2 orthogonalised against c1, c3 = c1 x c2
@@ -364,7 +365,7 @@ mm_status launch_eval(mm_ctx* c, const EpiParams& ep)
     }
     // a5-a10
     bool done = false;
-    if (ep.demag && (c->fast & FAST_SPLIT) && (fp.ok_x || fp.ok_xr) && g.Nx % 4 == 0) {
+    if (ep.demag && (c->fast & FAST_SPLIT) && (fp.ok_x || fp.ok_xr) && (g.Nx % 4 == 0 || ep.geometry)) {
         // split variant: inverse x pass -> H_ms field, then the streaming per-cell tail
         c->kt.begin(KT_INV_X);
         if (ep.mode == EPI_HMS) {
@@ -376,14 +377,15 @@ mm_status launch_eval(mm_ctx* c, const EpiParams& ep)
             if (done) {
                 const size_t quads = ncell(g) / 4;
                 c->kt.begin(KT_EPI);
-                k_epi4<<<(unsigned)((quads + 255) / 256), 256, 0, st>>>(g, c->hfield, ep);
+                if (ep.geometry) k_epi1<<<(unsigned)((ncell(g) + 255) / 256), 256, 0, st>>>(g, c->hfield, ep);
+                else k_epi4<<<(unsigned)((quads + 255) / 256), 256, 0, st>>>(g, c->hfield, ep);
                 c->kt.end(KT_EPI);
             }
         }
     }
     if (!done) {
         c->kt.begin(KT_INV_X);
-        if (!(ep.demag && (c->fast & FAST_INV_X) && fast_inv_x(fp, g, st, c->specA, ep))) {
+        if (!(ep.demag && !ep.geometry && (c->fast & FAST_INV_X) && fast_inv_x(fp, g, st, c->specA, ep))) {
             const int tx = pick_tx(g.Px, 2, 3, &bytes);
             if (!tx) return fail(c, MM_EUNSUPPORTED, "x line too long for the shared-memory tile");
             const int npy = (g.Ny + 1) / 2;
@@ -444,7 +446,8 @@ __global__ void k_normalise(size_t n, const float* __restrict__ src, float* __re
 {
     for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
         const float x = src[i], y = src[i + n], z = src[i + 2 * n];
-        const float s = rsqrtf(x * x + y * y + z * z);
+        const float q = x * x + y * y + z * z;
+        const float s = q > 0.f ? rsqrtf(q) : 0.f;
         dst[i] = x * s; dst[i + n] = y * s; dst[i + 2 * n] = z * s;
     }
 }

@@ -32,7 +32,7 @@ class Material(C.Structure):
                 ("Ku", C.c_double), ("anis_u", C.c_double * 3), ("Bext", C.c_double * 3),
                 ("T", C.c_double), ("seed", C.c_uint64), ("j", C.c_double * 3), ("P", C.c_double),
                 ("xi", C.c_double), ("stt_literal_eq7", C.c_int), ("demag", C.c_int),
-                ("K1", C.c_double), ("K2", C.c_double), ("exchange_in_kernel", C.c_int),
+                ("K1", C.c_double), ("K2", C.c_double), ("exchange_in_kernel", C.c_int), ("geometry", C.c_int),
                 ("anis_c1", C.c_double * 3), ("anis_c2", C.c_double * 3)]
 
     @classmethod
@@ -49,6 +49,7 @@ class Material(C.Structure):
         m.demag = int(bool(demag))
         m.K1 = d.get("K1", 0.0); m.K2 = d.get("K2", 0.0)
         m.exchange_in_kernel = int(bool(d.get("exchange_in_kernel", False)))
+        m.geometry = int(bool(d.get("geometry", False)))
         m.anis_c1 = (C.c_double * 3)(*d.get("anis_c1", (1.0, 0.0, 0.0)))
         m.anis_c2 = (C.c_double * 3)(*d.get("anis_c2", (0.0, 1.0, 0.0)))
         return m

@@ -78,7 +78,7 @@ def _mat(**kw):
     d = dict(Ms=8e5, Aex=1.3e-11, alpha=0.5, gamma0=2.211e5, Ku=0.0, anis_u=(0.0, 0.0, 1.0),
              Bext=(0.0, 0.0, 0.0), T=0.0, seed=0, j=(0.0, 0.0, 0.0), P=0.0, xi=0.0,
              stt_literal_eq7=False, K1=0.0, K2=0.0, anis_c1=(1.0, 0.0, 0.0), anis_c2=(0.0, 1.0, 0.0),
-             exchange_in_kernel=False)
+             exchange_in_kernel=False, geometry=False)
     d.update(kw)
     return d
 

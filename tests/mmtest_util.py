@@ -13,7 +13,8 @@ def oracle_material(matd):
                         stt_literal_eq7=bool(matd["stt_literal_eq7"]), K1=matd.get("K1", 0.0), K2=matd.get("K2", 0.0),
                         anis_c1=tuple(matd.get("anis_c1", (1.0, 0.0, 0.0))),
                         anis_c2=tuple(matd.get("anis_c2", (0.0, 1.0, 0.0))),
-                        exchange_in_kernel=bool(matd.get("exchange_in_kernel", False)))
+                        exchange_in_kernel=bool(matd.get("exchange_in_kernel", False)),
+                        geometry=bool(matd.get("geometry", False)))
 
 
 def oracle_problem(wl, demag="fft"):

@@ -631,3 +631,29 @@ def test_exchange_inside_the_kernel_variant(grid, pbc, fast):
         assert float(d[:, 1:-1, 1:-1, 1:-1].abs().max()) <= 2e-5 * float(H.abs().max())   # interior: same field
         assert float(d.abs().max()) > 1e-2 * float(H.abs().max())                           # faces: not
     sim.close(); sim0.close()
+
+
+@pytest.mark.parametrize("grid,fast", [((24, 10, 6), 0), ((64, 32, 32), 63), ((30, 12, 1), 0)])
+def test_staircase_geometry(grid, fast):
+    """SURVEY 8(f) row f-2 (reading A15): cells with m = 0 are empty."""
+    wl = util.small(grid, (3e-9, 4e-9, 5e-9), geometry=True, j=(1e12, -5e11, 0.0), P=0.5, xi=0.04, alpha=0.1)
+    m = wlm.initial_m(wl)
+    Nx, Ny, Nz = grid
+    z, y, x = np.meshgrid(np.arange(Nz), np.arange(Ny), np.arange(Nx), indexing="ij")
+    shape = ((x - Nx / 2.0) / (Nx / 2.0)) ** 2 + ((y - Ny / 2.0) / (Ny / 2.0)) ** 2 <= 1.0     # elliptic cylinder
+    shape &= ~((abs(x - Nx // 3) <= 1) & (abs(y - Ny // 2) <= 1))                                  # with a hole
+    m = m * shape[None].astype(np.float32)
+    m64 = m.astype(np.float64)
+    pb = util.oracle_problem(wl)
+    sim = util.gpu_sim(wl, fast=fast)
+    md = util.to_dev(m)
+    _cmp(sim.heff(md), pb.heff(m64), TOL_H)
+    _cmp(sim.torque(md), pb.torque(m64), TOL_H)
+    mo = m64.copy()
+    for _ in range(5):
+        mo = orc.rk4_step(pb.torque, mo, 5e-14)
+    sim.steps_fixed(md, "rk4", 5e-14, 5)
+    out = md.double().cpu().numpy()
+    assert np.abs(out - mo).max() <= TOL_M
+    assert np.all(out[:, ~shape] == 0.0) and np.isfinite(out).all()
+    sim.close()
