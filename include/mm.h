@@ -40,7 +40,7 @@ typedef enum {
     MM_ENOMEM = 2,       /* host or device allocation failed                                      */
     MM_ECUDA = 3,        /* CUDA runtime error (message in mm_last_error)                         */
     MM_ESTATE = 4,       /* call order: material / demag kernel not set                           */
-    MM_EUNSUPPORTED = 5, /* padded size not 2^a 3^b 5^c, thermal field with adaptive stepping ... */
+    MM_EUNSUPPORTED = 5, /* padded size not 2^a 3^b 5^c 7^d, thermal field with adaptive stepping */
     MM_ENUMERIC = 6      /* non-finite value met by the max-norm reduction                        */
 } mm_status;
 
@@ -93,7 +93,7 @@ typedef struct {
  *                (reading A8).
  *   cuda_stream  a cudaStream_t (e.g. torch.cuda.current_stream().cuda_stream) or NULL for the
  *                default stream.  Every kernel of this context is launched on it.
- * Errors: MM_EINVAL; MM_EUNSUPPORTED if a padded size has a prime factor other than 2, 3, 5
+ * Errors: MM_EINVAL; MM_EUNSUPPORTED if a padded size has a prime factor other than 2, 3, 5, 7
  * (PAPER.md:169-171 restricts sizes to smooth numbers); MM_ECUDA if no device; MM_ENOMEM. */
 mm_status mm_create(mm_ctx** out, const int grid[3], const double cellsize[3], const int pbc[3],
                     void* cuda_stream);

@@ -338,7 +338,7 @@ void tensor_at(const double cell[3], const int grid[3], const int pbc[3], size_t
 }
 
 // ---------------------------------------------------------------------------------------------
-// host FFT (fp64, Stockham, any mix of radices 2, 3, 5)
+// host FFT (fp64, Stockham, any mix of radices 2, 3, 5, 7)
 // ---------------------------------------------------------------------------------------------
 typedef std::complex<double> cd;
 
@@ -349,7 +349,7 @@ struct HostFFT {
     explicit HostFFT(int n_) : n(n_)
     {
         int m = n;
-        for (int p : { 5, 3, 2 })
+        for (int p : { 7, 5, 3, 2 })
             while (m % p == 0) { radices.push_back(p); m /= p; }
         tw.resize(n);
         for (int q = 0; q < n; ++q) {
@@ -373,7 +373,7 @@ struct HostFFT {
             const int m = n / R;
             for (int j = 0; j < m; ++j) {
                 const int k = j % ns;
-                cd v[5];
+                cd v[7];
                 for (int r = 0; r < R; ++r) v[r] = in[j + r * m] * tw[(size_t)r * k * (n / (ns * R)) % n];
                 const int j0 = (j / ns) * ns * R + k;
                 for (int s = 0; s < R; ++s) {
@@ -391,7 +391,7 @@ struct HostFFT {
 
 static bool smooth235(int n)
 {
-    for (int p : { 2, 3, 5 })
+    for (int p : { 2, 3, 5, 7 })
         while (n % p == 0) n /= p;
     return n == 1;
 }
@@ -444,7 +444,7 @@ int build_khat(const double cell[3], const int grid[3], const int pbc[3], float*
         per[a] = pbc[a] > 0;
         P[a] = per[a] ? grid[a] : (grid[a] > 1 ? 2 * grid[a] : 1);
         if (!smooth235(P[a])) {
-            if (err) *err = "padded size has a prime factor other than 2, 3, 5";
+            if (err) *err = "padded size has a prime factor other than 2, 3, 5, 7";
             return 5;
         }
         E[a] = octant_extent(grid[a], per[a]);

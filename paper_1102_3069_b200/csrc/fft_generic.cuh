@@ -72,6 +72,35 @@ __device__ __forceinline__ void bfly5(float2* v)
     v[3] = csub(a2, b2);
 }
 
+// radix 7 (PAPER.md:171 lists sizes 2^n x {1, 3, 5, 7}): X_k = v0 + sum_j t_j cos(2 pi j k / 7) + SGN i sum_j d_j sin(...),
+// t_j = v_j + v_(7-j), d_j = v_j - v_(7-j), j = 1..3
+template <int SGN>
+__device__ __forceinline__ void bfly7(float2* v)
+{
+    const float C[3] = { 0.62348980185873353053f, -0.22252093395631440429f, -0.90096886790241912624f };
+    const float S[3] = { 0.78183148246802980871f, 0.97492791218182360702f, 0.43388373911755812048f };
+    float2 t[3], d[3];
+#pragma unroll
+    for (int j = 0; j < 3; ++j) { t[j] = cadd(v[j + 1], v[6 - j]); d[j] = csub(v[j + 1], v[6 - j]); }
+    const float2 v0 = v[0];
+    v[0] = cadd(v0, cadd(t[0], cadd(t[1], t[2])));
+#pragma unroll
+    for (int k = 1; k <= 3; ++k) {
+        float2 a = v0, b = make_float2(0.f, 0.f);
+#pragma unroll
+        for (int j = 1; j <= 3; ++j) {
+            const int q = (j * k) % 7;                    // cos(2 pi q / 7), sin(2 pi q / 7) from q in 1..3 by symmetry
+            const float c = q <= 3 ? C[q - 1] : C[6 - q];
+            const float s = q <= 3 ? S[q - 1] : -S[6 - q];
+            a.x += c * t[j - 1].x; a.y += c * t[j - 1].y;
+            b.x += s * d[j - 1].x; b.y += s * d[j - 1].y;
+        }
+        const float2 ib = cmuli<SGN>(b);
+        v[k] = cadd(a, ib);
+        v[7 - k] = csub(a, ib);
+    }
+}
+
 // One Stockham pass of radix R: in -> out.
 template <int R, int SGN>
 __device__ __forceinline__ void stockham_pass(const float2* __restrict__ in, float2* __restrict__ out,
@@ -98,6 +127,7 @@ __device__ __forceinline__ void stockham_pass(const float2* __restrict__ in, flo
         if (R == 3) bfly3<SGN>(v);
         if (R == 4) bfly4<SGN>(v);
         if (R == 5) bfly5<SGN>(v);
+        if (R == 7) bfly7<SGN>(v);
         const int j0 = (j / ns) * ns * R + k;
 #pragma unroll
         for (int s = 0; s < R; ++s) out[(j0 + s * ns) * TXP + c] = v[s];
@@ -116,7 +146,8 @@ __device__ float2* tile_fft(float2* a, float2* b, const FftPlan& pl, int TXP, in
         if (R == 4) stockham_pass<4, SGN>(a, b, pl.L, ns, TXP, ncol, pl.tw);
         else if (R == 2) stockham_pass<2, SGN>(a, b, pl.L, ns, TXP, ncol, pl.tw);
         else if (R == 3) stockham_pass<3, SGN>(a, b, pl.L, ns, TXP, ncol, pl.tw);
-        else stockham_pass<5, SGN>(a, b, pl.L, ns, TXP, ncol, pl.tw);
+        else if (R == 5) stockham_pass<5, SGN>(a, b, pl.L, ns, TXP, ncol, pl.tw);
+        else stockham_pass<7, SGN>(a, b, pl.L, ns, TXP, ncol, pl.tw);
         ns *= R;
         float2* t = a; a = b; b = t;
         __syncthreads();

@@ -110,7 +110,7 @@ Tableau make_tableau(mm_method m)
 
 bool smooth235(int n)
 {
-    for (int p : { 2, 3, 5 })
+    for (int p : { 2, 3, 5, 7 })
         while (n % p == 0) n /= p;
     return n == 1;
 }
@@ -181,6 +181,7 @@ void make_plan(FftPlan& pl, int L)
     while (m % 2 == 0) { pl.rad[pl.nrad++] = 2; m /= 2; }
     while (m % 3 == 0) { pl.rad[pl.nrad++] = 3; m /= 3; }
     while (m % 5 == 0) { pl.rad[pl.nrad++] = 5; m /= 5; }
+    while (m % 7 == 0) { pl.rad[pl.nrad++] = 7; m /= 7; }
 }
 
 // largest column count from {16, 8, 4, 2, 1} (times `mult`, plus one pad column) whose tile fits
@@ -603,7 +604,7 @@ mm_status mm_create(mm_ctx** out, const int grid[3], const double cellsize[3], c
     for (int a = 0; a < 3; ++a) {
         P[a] = pbc[a] > 0 ? grid[a] : (grid[a] > 1 ? 2 * grid[a] : 1);
         if (!smooth235(P[a]))
-            return fail(nullptr, MM_EUNSUPPORTED, "padded size has a prime factor other than 2, 3, 5");
+            return fail(nullptr, MM_EUNSUPPORTED, "padded size has a prime factor other than 2, 3, 5, 7");
     }
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) {

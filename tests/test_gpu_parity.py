@@ -28,6 +28,8 @@ GRIDS = [
     ((1, 1, 1), (5e-9, 5e-9, 5e-9), (0, 0, 0)),          # macrospin
     ((1, 8, 2), (5e-9, 4e-9, 3e-9), (0, 0, 0)),          # one cell along x
     ((64, 48, 2), (3e-9, 3e-9, 3e-9), (0, 0, 0)),        # several tiles per pass
+    ((28, 14, 7), (3e-9, 4e-9, 5e-9), (0, 0, 0)),        # radix 7 (56, 28, 14)
+    ((49, 7, 1), (3e-9, 3e-9, 3e-9), (1, 1, 0)),         # 49 = 7 * 7 periodic, no padding
 ]
 
 

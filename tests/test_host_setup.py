@@ -42,7 +42,7 @@ def test_create_without_device_fails_loudly(mm):
 def test_unsupported_size_is_reported(mm):
     L = mm.lib()
     ctx = ctypes.c_void_p()
-    st = L.mm_create(ctypes.byref(ctx), (ctypes.c_int * 3)(7, 4, 1), (ctypes.c_double * 3)(1, 1, 1),
+    st = L.mm_create(ctypes.byref(ctx), (ctypes.c_int * 3)(11, 4, 1), (ctypes.c_double * 3)(1, 1, 1),
                      (ctypes.c_int * 3)(0, 0, 0), None)
     assert st == 5 and b"prime factor" in L.mm_last_error(None)
 
