@@ -264,10 +264,12 @@ k_mid(Geom g, ColTile ct, float2* __restrict__ spec, const float* __restrict__ k
 // loops over work items (16 kx columns x one ky pair {p, Py - p}) and, while it transforms one
 // line set, cp.async already brings in the next one's spectrum tile [3][Nz][16] and, once per pair,
 // the K^ octant tile [6][Cz][16], so neither load latency is exposed and the two lines of a pair
-// share one K^ fetch.  grid = min(items, 2 SMs...); block = 16 T.
+// share one K^ fetch.  The three components go through ONE exchange tile in turn (a barrier in
+// between), which keeps the footprint at 67 KB and the registers at 168: 3 blocks = 12 warps per SM.
+// grid = resident blocks; block = 16 T.
 // ---------------------------------------------------------------------------------------------
 template <int T, int E, bool PER>
-__global__ void __launch_bounds__(16 * T, (T * E <= 128) ? 2 : 1)
+__global__ void __launch_bounds__(16 * T, (T * E <= 128) ? 3 : 1)
 k_mid_p(Geom g, ColTile ct, float2* __restrict__ spec, const float* __restrict__ khat,
         const float2* __restrict__ tw)
 {
@@ -278,7 +280,7 @@ k_mid_p(Geom g, ColTile ct, float2* __restrict__ spec, const float* __restrict__
     constexpr int CZ = L / 2 + 1;              // == g.Cz
     constexpr int NT = 16 * T;
     float2* xb = ff_smem;
-    float2* ib = xb + 3 * LB;                   // [3][NZ][16]
+    float2* ib = xb + LB;                       // one exchange tile, used by the components in turn
     float* kb = reinterpret_cast<float*>(ib + 3 * NZ * 16);     // [6][CZ][16]
     const int tid = threadIdx.x, c = tid & 15, t = tid >> 4;
     const int ntx = (ct.ncol + 15) >> 4;
@@ -333,8 +335,10 @@ k_mid_p(Geom g, ColTile ct, float2* __restrict__ spec, const float* __restrict__
             else if (qn < nitem) issue_in(qn % ntx, qn / ntx);
             cp_async_commit();
 #pragma unroll
-            for (int comp = 0; comp < 3; ++comp)
-                fft_line<T, E, -1, !PER>(v[comp], xb + comp * LB + c, 16, t, tw, SyncBlock());
+            for (int comp = 0; comp < 3; ++comp) {
+                if (comp) __syncthreads();
+                fft_line<T, E, -1, !PER>(v[comp], xb + c, 16, t, tw, SyncBlock());
+            }
             cp_async_wait<1>();
             __syncthreads();                    // K^ tile of this pair has landed
 #pragma unroll
@@ -356,8 +360,10 @@ k_mid_p(Geom g, ColTile ct, float2* __restrict__ spec, const float* __restrict__
             if (h + 1 == nh && qn < nitem) issue_k(qn % ntx, qn / ntx);
             cp_async_commit();
 #pragma unroll
-            for (int comp = 0; comp < 3; ++comp)
-                fft_line<T, E, 1, false>(v[comp], xb + comp * LB + c, 16, t, tw, SyncBlock());
+            for (int comp = 0; comp < 3; ++comp) {
+                if (comp) __syncthreads();
+                fft_line<T, E, 1, false>(v[comp], xb + c, 16, t, tw, SyncBlock());
+            }
             if (valid) {
                 float2* __restrict__ base = spec + (size_t)other * ct.b_row + col;
 #pragma unroll

@@ -158,11 +158,12 @@ bool launch_mid3(const FastPlan& fp, const Geom& g, cudaStream_t st, const ColTi
     if (fp.mid_pipe) {
         constexpr int L = T * E;
         constexpr int NZ = PER ? L : L / 2;
-        const size_t pb = (size_t)3 * T * (E + 1) * 16 * sizeof(float2) + (size_t)3 * NZ * 16 * sizeof(float2) +
+        constexpr int NXB = 1;           // one exchange tile, used by the three components in turn
+        const size_t pb = (size_t)NXB * T * (E + 1) * 16 * sizeof(float2) + (size_t)3 * NZ * 16 * sizeof(float2) +
                           (size_t)6 * (L / 2 + 1) * 16 * sizeof(float);
         if (pb <= 227 * 1024) {
             const int nitem = ((ct.ncol + 15) / 16) * (g.Py / 2 + 1);
-            const int per_sm = (T * E <= 128) ? 2 : 1;
+            const int per_sm = (T * E <= 128) ? 3 : 1;
             const int grid = nitem < fp.nsm * per_sm ? nitem : fp.nsm * per_sm;
             static bool oncep = ensure_smem(k_mid_p<T, E, PER>, pb);
             if (!oncep) return false;
