@@ -276,7 +276,9 @@ def main():
     # ---- device-resident timing ----
     sampler = ClockSampler(local)          # samples from the warm-up to the end of the e2e region
     sampler.start()
-    sim.steps_fixed(md, method, dt, max(3, args.warmup))
+    # warm-up: at least 4 steps in one call, so that the graph-replay path of mm_steps_fixed (its stream,
+    # events and first capture) is initialised outside the timed region
+    sim.steps_fixed(md, method, dt, max(4, args.warmup))
     barrier()
     # the timed region: the plain product call, no per-pass instrumentation
     l0 = sim.launch_count()
@@ -362,7 +364,7 @@ def main():
                          f"by cell count"}
 
     out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
-           "warmup": max(3, args.warmup), "ms_per_step": sec / args.steps * 1e3, "higher_is_better": True,
+           "warmup": max(4, args.warmup), "ms_per_step": sec / args.steps * 1e3, "higher_is_better": True,
            "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
            "config": {"workload": f"{wl.name}: {wl.grid[0]}x{wl.grid[1]}x{wl.grid[2]} cells, pbc {tuple(wl.pbc)}, "
                                   f"'{wl.init}' state (seed {wl.seed}), RK4 dt={dt:g} s, 1 step = 4 fused evaluations",
