@@ -276,6 +276,9 @@ def main():
     # ---- device-resident timing ----
     sampler = ClockSampler(local)          # samples from the warm-up to the end of the e2e region
     sampler.start()
+    t_wait = time.perf_counter()           # let nvidia-smi finish its own start-up before anything is timed
+    while len(sampler.rows) < 2 and time.perf_counter() - t_wait < 5.0:
+        time.sleep(0.05)
     # warm-up: at least 4 steps in one call, so that the graph-replay path of mm_steps_fixed (its stream,
     # events and first capture) is initialised outside the timed region
     sim.steps_fixed(md, method, dt, max(4, args.warmup))
