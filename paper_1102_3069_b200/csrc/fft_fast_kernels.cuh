@@ -76,6 +76,202 @@ template <int N>
 __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;\n" ::"n"(N) : "memory"); }
 
 // ---------------------------------------------------------------------------------------------
+// a1 / a5, software-pipelined forms of k_fwd_x / k_inv_x_h (same arithmetic, same thread layout): the
+// rows of the NEXT pair are staged by cp.async into the slot's exchange buffer -- free between the
+// read-back of the exchange and the next first register FFT -- while the second register FFT, the
+// separation shuffles and the stores of the current pair run.  Needs 16-byte aligned rows (Nx % 4 == 0).
+// ---------------------------------------------------------------------------------------------
+template <int T, int E, bool PER>
+__global__ void __launch_bounds__(128)
+k_fwd_x_p(Geom g, const float* __restrict__ m, float2* __restrict__ specA, const float2* __restrict__ tw)
+{
+    constexpr int L = T * E;
+    constexpr int LB = T * (E + 1);
+    constexpr int NIN = PER ? E : E / 2;
+    constexpr int NXC = PER ? L : L / 2;       // == g.Nx
+    const int t = threadIdx.x % T;
+    const int slot = threadIdx.x / T;
+    const int nslot = 128 / T;
+    float2* sb = ff_smem + slot * LB;
+    float* sf = reinterpret_cast<float*>(sb);  // staged rows: [2][NXC] floats
+    const int npy = (g.Ny + 1) >> 1;
+    const int npair = 3 * g.Nz * npy;
+    const unsigned lane = threadIdx.x & 31;
+    const unsigned src = lane - t + ((T - t) % T);
+    const int stride = gridDim.x * nslot;
+
+    auto issue = [&](int pb) {
+        const int pp = pb + slot < npair ? pb + slot : npair - 1;
+        const int cz = pp / npy, y0 = 2 * (pp - cz * npy);
+        const bool two = y0 + 1 < g.Ny;
+        const float* __restrict__ r0 = m + ((size_t)cz * g.Ny + y0) * g.Nx;
+        for (int u = t; u < NXC / 2; u += T) {
+            const int row = u / (NXC / 4), q = u - row * (NXC / 4);
+            const bool ok = row == 0 || two;
+            cp_async16(sf + row * NXC + 4 * q, ok ? r0 + (size_t)row * g.Nx + 4 * q : m, ok ? 16 : 0);
+        }
+    };
+
+    int pb = blockIdx.x * nslot;
+    if (pb < npair) issue(pb);
+    cp_async_commit();
+    for (; pb < npair; pb += stride) {
+        const bool act = pb + slot < npair;
+        const int pp = act ? pb + slot : npair - 1;
+        const int cz = pp / npy, y0 = 2 * (pp - cz * npy);
+        const bool two = y0 + 1 < g.Ny;
+        cp_async_wait<0>();
+        __syncwarp();
+        float2 v[E];
+#pragma unroll
+        for (int j = 0; j < NIN; ++j) v[j] = make_float2(sf[t + T * j], sf[NXC + t + T * j]);
+        __syncwarp();                           // the region now serves as the exchange buffer
+        if constexpr (!PER) fft_reg_half<E, -1>(v);
+        else fft_reg<E, -1>(v);
+#pragma unroll
+        for (int k2 = 1; k2 < E; ++k2) v[k2] = cmul(v[k2], __ldg(tw + k2 * T + t));
+#pragma unroll
+        for (int k2 = 0; k2 < E; ++k2) sb[t * (E + 1) + k2] = v[k2];
+        __syncwarp();
+        float2 u[E / T][T];
+#pragma unroll
+        for (int q = 0; q < E / T; ++q)
+#pragma unroll
+            for (int n1 = 0; n1 < T; ++n1) u[q][n1] = sb[n1 * (E + 1) + t + T * q];
+        __syncwarp();                           // exchange read back: stage the next pair
+        if (pb + stride < npair) issue(pb + stride);
+        cp_async_commit();
+#pragma unroll
+        for (int q = 0; q < E / T; ++q) {
+            fft_reg<T, -1>(u[q]);
+#pragma unroll
+            for (int k1 = 0; k1 < T; ++k1) v[q + (E / T) * k1] = u[q][k1];
+        }
+        float2* __restrict__ o0 = specA + ((size_t)cz * g.Ny + y0) * g.CxS;
+        float2* __restrict__ o1 = o0 + g.CxS;
+#pragma unroll
+        for (int j = 0; j < E / 2; ++j) {
+            float2 p;
+            p.x = __shfl_sync(0xffffffffu, v[E - 1 - j].x, src);
+            p.y = __shfl_sync(0xffffffffu, v[E - 1 - j].y, src);
+            if (t == 0) p = v[(E - j) % E];
+            const float2 z = v[j];
+            if (act) o0[t + T * j] = make_float2(0.5f * (z.x + p.x), 0.5f * (z.y - p.y));
+            if (act && two) o1[t + T * j] = make_float2(0.5f * (z.y + p.y), 0.5f * (p.x - z.x));
+        }
+        if (t == 0 && act) {
+            o0[L / 2] = make_float2(v[E / 2].x, 0.f);
+            if (two) o1[L / 2] = make_float2(v[E / 2].y, 0.f);
+        }
+    }
+    cp_async_wait<0>();
+}
+
+template <int T, int E, bool PER>
+__global__ void __launch_bounds__(128)
+k_inv_x_h_p(Geom g, const float2* __restrict__ specA, const float2* __restrict__ tw, float* __restrict__ out,
+            float scale)
+{
+    constexpr int L = T * E;
+    constexpr int LB = T * (E + 1);
+    constexpr int NOUT = PER ? E : E / 2;
+    constexpr int CX = L / 2 + 1;               // == g.Cx
+    constexpr int CXP = L / 2 + 2;              // second staged row starts 16-byte aligned
+    static_assert(2 * CXP <= LB, "staged rows must fit the exchange buffer");
+    const int t = threadIdx.x % T;
+    const int slot = threadIdx.x / T;
+    const int nslot = 128 / T;
+    float2* sb = ff_smem + slot * LB;
+    const int npy = (g.Ny + 1) >> 1;
+    const int npair = 3 * g.Nz * npy;
+    const unsigned lane = threadIdx.x & 31;
+    const unsigned srcl = lane - t + ((T - t) % T);
+    const int stride = gridDim.x * nslot;
+
+    auto issue = [&](int pb) {
+        const int pp = pb + slot < npair ? pb + slot : npair - 1;
+        const int cz = pp / npy, y0 = 2 * (pp - cz * npy);
+        const bool two = y0 + 1 < g.Ny;
+        const float2* __restrict__ a0 = specA + ((size_t)cz * g.Ny + y0) * g.CxS;
+        for (int u = t; u < CXP; u += T) {       // CXP / 2 units of two complex values per row
+            const int row = u / (CXP / 2), q = u - row * (CXP / 2);
+            const bool ok = row == 0 || two;
+            const int nb = !ok ? 0 : (2 * q + 2 <= CX ? 16 : 8);
+            cp_async16(sb + row * CXP + 2 * q, ok ? a0 + (size_t)row * g.CxS + 2 * q : specA, nb);
+        }
+    };
+
+    int pb = blockIdx.x * nslot;
+    if (pb < npair) issue(pb);
+    cp_async_commit();
+    for (; pb < npair; pb += stride) {
+        const bool act = pb + slot < npair;
+        const int pp = act ? pb + slot : npair - 1;
+        const int cz = pp / npy, y0 = 2 * (pp - cz * npy);
+        const bool two = y0 + 1 < g.Ny;
+        cp_async_wait<0>();
+        __syncwarp();
+        float2 v[E];
+#pragma unroll
+        for (int j = 0; j < E / 2; ++j) {
+            const float2 A = sb[t + T * j], B = sb[CXP + t + T * j];
+            v[j] = make_float2(A.x - B.y, A.y + B.x);
+            v[E - 1 - j] = make_float2(A.x + B.y, B.x - A.y);
+        }
+        float2 nyq = make_float2(0.f, 0.f);
+        if (t == 0) {
+            const float2 A = sb[L / 2], B = sb[CXP + L / 2];
+            nyq = make_float2(A.x - B.y, A.y + B.x);
+        }
+        __syncwarp();                           // the region now serves as the exchange buffer
+        float2 own[E / 2];
+#pragma unroll
+        for (int j = 0; j < E / 2; ++j) own[j] = v[E - 1 - j];
+#pragma unroll
+        for (int j = E / 2; j < E; ++j) {
+            float2 p;
+            p.x = __shfl_sync(0xffffffffu, v[j].x, srcl);
+            p.y = __shfl_sync(0xffffffffu, v[j].y, srcl);
+            v[j] = p;
+        }
+        if (t == 0) {
+            v[E / 2] = nyq;
+#pragma unroll
+            for (int j = E / 2 + 1; j < E; ++j) v[j] = own[E - j];
+        }
+        fft_reg<E, 1>(v);
+#pragma unroll
+        for (int k2 = 1; k2 < E; ++k2) v[k2] = cmul(v[k2], cconj(__ldg(tw + k2 * T + t)));
+#pragma unroll
+        for (int k2 = 0; k2 < E; ++k2) sb[t * (E + 1) + k2] = v[k2];
+        __syncwarp();
+        float2 u[E / T][T];
+#pragma unroll
+        for (int q = 0; q < E / T; ++q)
+#pragma unroll
+            for (int n1 = 0; n1 < T; ++n1) u[q][n1] = sb[n1 * (E + 1) + t + T * q];
+        __syncwarp();                           // exchange read back: stage the next pair
+        if (pb + stride < npair) issue(pb + stride);
+        cp_async_commit();
+#pragma unroll
+        for (int q = 0; q < E / T; ++q) {
+            fft_reg<T, 1>(u[q]);
+#pragma unroll
+            for (int k1 = 0; k1 < T; ++k1) v[q + (E / T) * k1] = u[q][k1];
+        }
+        float* __restrict__ o0 = out + ((size_t)cz * g.Ny + y0) * g.Nx;
+        if (act) {
+#pragma unroll
+            for (int j = 0; j < NOUT; ++j) {
+                o0[t + T * j] = scale * v[j].x;
+                if (two) o0[g.Nx + t + T * j] = scale * v[j].y;
+            }
+        }
+    }
+    cp_async_wait<0>();
+}
+
+// ---------------------------------------------------------------------------------------------
 // Where the columns of a y / last-axis pass live.  The whole-array mode uses the layouts of
 // mm_common.cuh (row stride CxS); the chunked mode works on `ncol`
 // kx columns starting at kx0, with the y-padded spectrum in a compact chunk buffer [3][Nz][Py][W]

@@ -12,6 +12,7 @@ struct FastPlan {
     float2* twx;                         // ok_xr: exp(-i pi k / Lc), k < Lc = Px / 2
     float2* tw[3];                       // per axis: tw[k2 * T + t] = exp(-2 pi i t k2 / L)
     int nsm;                             // SM count (persistent grids)
+    int x_pipe;                          // x passes, cp.async-pipelined forms: bit 0 forward (default), bit 1 inverse (env MM_X_PIPE)
     int mid_pipe;                        // last-axis pass: persistent cp.async-pipelined kernel (env MM_MID_PIPE)
     int chunk_w, nstream;                // chunked a2-a4: columns per chunk (0 = whole-array passes), streams
     cudaStream_t stream[4];
@@ -75,6 +76,13 @@ bool launch_fwd_x(const FastPlan& fp, const Geom& g, cudaStream_t st, const floa
     const int npair = 3 * g.Nz * ((g.Ny + 1) / 2);
     const int want = (npair + nslot - 1) / nslot;
     const int grid = want < fp.nsm * 8 ? want : fp.nsm * 8;
+    if ((fp.x_pipe & 1) && g.Nx % 4 == 0) {
+        static bool oncep = ensure_smem(k_fwd_x_p<T, E, PER>, bytes);
+        if (!oncep) return false;
+        const int gridp = want < fp.nsm * 4 ? want : fp.nsm * 4;      // resident blocks: the loop is pipelined
+        k_fwd_x_p<T, E, PER><<<gridp, 128, bytes, st>>>(g, m, specA, fp.tw[0]);
+        return true;
+    }
     k_fwd_x<T, E, PER><<<grid, 128, bytes, st>>>(g, m, specA, fp.tw[0]);
     return true;
 }
@@ -104,6 +112,13 @@ bool launch_inv_x_h(const FastPlan& fp, const Geom& g, cudaStream_t st, const fl
     const int npair = 3 * g.Nz * ((g.Ny + 1) / 2);
     const int want = (npair + nslot - 1) / nslot;
     const int grid = want < fp.nsm * 8 ? want : fp.nsm * 8;
+    if ((fp.x_pipe & 2) && g.CxS % 2 == 0) {      // measured slower than the plain form on B200: off by default
+        static bool oncep = ensure_smem(k_inv_x_h_p<T, E, PER>, bytes);
+        if (!oncep) return false;
+        const int gridp = want < fp.nsm * 4 ? want : fp.nsm * 4;
+        k_inv_x_h_p<T, E, PER><<<gridp, 128, bytes, st>>>(g, specA, fp.tw[0], out, scale);
+        return true;
+    }
     k_inv_x_h<T, E, PER><<<grid, 128, bytes, st>>>(g, specA, fp.tw[0], out, scale);
     return true;
 }
@@ -347,6 +362,7 @@ inline bool fast_plan_init(FastPlan& fp, const Geom& g, std::string* err)
     // B200 at 512x512x64 they give bit-identical results and cut DRAM traffic, but no time, because the
     // y and last-axis passes are bound by instruction issue, not by HBM (profiles/).
     fp.chunk_w = 0;
+    fp.x_pipe = getenv("MM_X_PIPE") ? atoi(getenv("MM_X_PIPE")) : 1;
     fp.mid_pipe = getenv("MM_MID_PIPE") ? atoi(getenv("MM_MID_PIPE")) : 1;
     fp.nstream = 3;
     if (getenv("MM_CHUNK_W")) fp.chunk_w = atoi(getenv("MM_CHUNK_W"));
