@@ -19,6 +19,8 @@
  *  - All device work is enqueued on the CUDA stream given to mm_create.  mm_heff / mm_torque /
  *    mm_stage are asynchronous with respect to the host; mm_step synchronises the stream once, at its
  *    end, to return dt / err / accepted.
+ *  - A context belongs to the CUDA device that is current when mm_create is called; that device must be
+ *    current for every later call on the context (one process per GPU is the intended use).
  *  - There is no CPU fallback, no cuFFT and no tensor-core path inside the library: every hot-path
  *    step runs in hand-written sm_100a kernels.  Without a CUDA device mm_create fails with MM_ECUDA.
  */

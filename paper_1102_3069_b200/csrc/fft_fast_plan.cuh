@@ -66,19 +66,33 @@ inline bool ensure_smem(K kern, size_t bytes)
     return cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes) == cudaSuccess;
 }
 
+// the dynamic shared-memory limit is a per-device attribute of a kernel: set it once per (kernel, device)
+#define MM_MAX_DEV 64
+template <class K>
+inline bool ensure_smem_dev(K kern, size_t bytes, bool (&done)[MM_MAX_DEV])
+{
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= MM_MAX_DEV) return ensure_smem(kern, bytes);
+    if (!done[dev]) {
+        if (!ensure_smem(kern, bytes)) return false;
+        done[dev] = true;
+    }
+    return true;
+}
+
 template <int T, int E, bool PER>
 bool launch_fwd_x(const FastPlan& fp, const Geom& g, cudaStream_t st, const float* m, float2* specA)
 {
     const size_t bytes = (size_t)(128 / T) * T * (E + 1) * sizeof(float2);
-    static bool once = ensure_smem(k_fwd_x<T, E, PER>, bytes);
-    if (!once) return false;
+    static bool once[MM_MAX_DEV] = {};
+    if (!ensure_smem_dev(k_fwd_x<T, E, PER>, bytes, once)) return false;
     const int nslot = 128 / T;
     const int npair = 3 * g.Nz * ((g.Ny + 1) / 2);
     const int want = (npair + nslot - 1) / nslot;
     const int grid = want < fp.nsm * 8 ? want : fp.nsm * 8;
     if ((fp.x_pipe & 1) && g.Nx % 4 == 0) {
-        static bool oncep = ensure_smem(k_fwd_x_p<T, E, PER>, bytes);
-        if (!oncep) return false;
+        static bool oncep[MM_MAX_DEV] = {};
+        if (!ensure_smem_dev(k_fwd_x_p<T, E, PER>, bytes, oncep)) return false;
         const int gridp = want < fp.nsm * 4 ? want : fp.nsm * 4;      // resident blocks: the loop is pipelined
         k_fwd_x_p<T, E, PER><<<gridp, 128, bytes, st>>>(g, m, specA, fp.tw[0]);
         return true;
@@ -92,8 +106,8 @@ bool launch_inv_x(const FastPlan& fp, const Geom& g, cudaStream_t st, const floa
 {
     constexpr int NX = PER ? T * E : T * E / 2;
     const size_t bytes = (size_t)(128 / T) * (T * (E + 1) + 2 * NX) * sizeof(float2);
-    static bool once = ensure_smem(k_inv_x<T, E, PER>, bytes);
-    if (!once) return false;
+    static bool once[MM_MAX_DEV] = {};
+    if (!ensure_smem_dev(k_inv_x<T, E, PER>, bytes, once)) return false;
     const int nslot = 128 / T;
     const int npair = g.Nz * ((g.Ny + 1) / 2);
     const int want = (npair + nslot - 1) / nslot;
@@ -106,15 +120,15 @@ template <int T, int E, bool PER>
 bool launch_inv_x_h(const FastPlan& fp, const Geom& g, cudaStream_t st, const float2* specA, float* out, float scale)
 {
     const size_t bytes = (size_t)(128 / T) * T * (E + 1) * sizeof(float2);
-    static bool once = ensure_smem(k_inv_x_h<T, E, PER>, bytes);
-    if (!once) return false;
+    static bool once[MM_MAX_DEV] = {};
+    if (!ensure_smem_dev(k_inv_x_h<T, E, PER>, bytes, once)) return false;
     const int nslot = 128 / T;
     const int npair = 3 * g.Nz * ((g.Ny + 1) / 2);
     const int want = (npair + nslot - 1) / nslot;
     const int grid = want < fp.nsm * 8 ? want : fp.nsm * 8;
     if ((fp.x_pipe & 2) && g.CxS % 2 == 0) {      // measured slower than the plain form on B200: off by default
-        static bool oncep = ensure_smem(k_inv_x_h_p<T, E, PER>, bytes);
-        if (!oncep) return false;
+        static bool oncep[MM_MAX_DEV] = {};
+        if (!ensure_smem_dev(k_inv_x_h_p<T, E, PER>, bytes, oncep)) return false;
         const int gridp = want < fp.nsm * 4 ? want : fp.nsm * 4;
         k_inv_x_h_p<T, E, PER><<<gridp, 128, bytes, st>>>(g, specA, fp.tw[0], out, scale);
         return true;
@@ -127,8 +141,8 @@ template <int T, int E, bool PER>
 bool launch_fwd_x_r(const FastPlan& fp, const Geom& g, cudaStream_t st, const float* m, float2* specA)
 {
     const size_t bytes = (size_t)(128 / T) * T * (E + 1) * sizeof(float2);
-    static bool once = ensure_smem(k_fwd_x_r<T, E, PER>, bytes);
-    if (!once) return false;
+    static bool once[MM_MAX_DEV] = {};
+    if (!ensure_smem_dev(k_fwd_x_r<T, E, PER>, bytes, once)) return false;
     const int nslot = 128 / T;
     const int want = (3 * g.Nz * g.Ny + nslot - 1) / nslot;
     const int grid = want < fp.nsm * 8 ? want : fp.nsm * 8;
@@ -141,8 +155,8 @@ bool launch_inv_x_h_r(const FastPlan& fp, const Geom& g, cudaStream_t st, const 
                       float scale)
 {
     const size_t bytes = (size_t)(128 / T) * T * (E + 1) * sizeof(float2);
-    static bool once = ensure_smem(k_inv_x_h_r<T, E, PER>, bytes);
-    if (!once) return false;
+    static bool once[MM_MAX_DEV] = {};
+    if (!ensure_smem_dev(k_inv_x_h_r<T, E, PER>, bytes, once)) return false;
     const int nslot = 128 / T;
     const int want = (3 * g.Nz * g.Ny + nslot - 1) / nslot;
     const int grid = want < fp.nsm * 8 ? want : fp.nsm * 8;
@@ -154,8 +168,8 @@ template <int T, int E, int SGN, bool PER>
 bool launch_y(const FastPlan& fp, const Geom& g, cudaStream_t st, const ColTile& ct, float2* a, float2* b)
 {
     const size_t bytes = (size_t)T * (E + 1) * 8 * sizeof(float2);
-    static bool oncep = ensure_smem(k_y_p<T, E, SGN, PER>, bytes);
-    if (!oncep) return false;
+    static bool oncep[MM_MAX_DEV] = {};
+    if (!ensure_smem_dev(k_y_p<T, E, SGN, PER>, bytes, oncep)) return false;
     const int ntile = ((ct.ncol + 7) / 8) * 3 * g.Nz;
     int per_sm = (int)((227 * 1024) / (bytes + 1024));
     const int cap = 2048 / (8 * T) < ((T == 32) ? 2 : 8) ? 2048 / (8 * T) : ((T == 32) ? 2 : 8);
@@ -180,8 +194,8 @@ bool launch_mid3(const FastPlan& fp, const Geom& g, cudaStream_t st, const ColTi
             const int nitem = ((ct.ncol + 15) / 16) * (g.Py / 2 + 1);
             const int per_sm = (T * E <= 128) ? 3 : 1;
             const int grid = nitem < fp.nsm * per_sm ? nitem : fp.nsm * per_sm;
-            static bool oncep = ensure_smem(k_mid_p<T, E, PER>, pb);
-            if (!oncep) return false;
+            static bool oncep[MM_MAX_DEV] = {};
+            if (!ensure_smem_dev(k_mid_p<T, E, PER>, pb, oncep)) return false;
             k_mid_p<T, E, PER><<<grid, 16 * T, pb, st>>>(g, ct, specB, khat, fp.tw[2]);
             return true;
         }
@@ -189,8 +203,8 @@ bool launch_mid3(const FastPlan& fp, const Geom& g, cudaStream_t st, const ColTi
     const size_t bytes = (size_t)3 * T * (E + 1) * 16 * sizeof(float2);
     constexpr int MINB = (T * E <= 128) ? 2 : 1;
     dim3 grid((ct.ncol + 15) / 16, 2 * (g.Py / 2 + 1));
-    static bool once = ensure_smem(k_mid<T, E, PER, true, MINB>, bytes);
-    if (!once) return false;
+    static bool once[MM_MAX_DEV] = {};
+    if (!ensure_smem_dev(k_mid<T, E, PER, true, MINB>, bytes, once)) return false;
     k_mid<T, E, PER, true, MINB><<<grid, 16 * T, bytes, st>>>(g, ct, specB, khat, fp.tw[2], 2);
     return true;
 }
