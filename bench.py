@@ -217,6 +217,60 @@ def run_sweep(args):
                       "data": "synthetic", "higher_is_better": False, "n_gpus": 1, "sweep": rows}))
 
 
+def run_cufft_compare(args):
+    """the same magnetostatic convolution through the FFT LIBRARY (torch.fft = cuFFT): pad, 3D
+    R2C, multiply by the full half-spectrum kernel, C2R, crop.  A bench-only comparison (north_star: cuFFT never
+    on the product path); it also cross-checks the result against the library's own kernels."""
+    import torch
+    import paper_1102_3069_b200 as mm
+    from paper_1102_3069_b200 import workloads as wlm
+    torch.cuda.set_device(0)
+    wl = workload(args.config)
+    Nx, Ny, Nz = wl.grid
+    sim = mm.Sim(wl.grid, wl.cell, wl.pbc, wl.mat)
+    P, Cs = sim.padded_size()
+    md = torch.from_numpy(wlm.initial_m(wl)).cuda()
+    # full half-spectrum kernel from the stored octant (even / odd symmetry of each component)
+    kz = torch.arange(P[2], device="cuda"); ky = torch.arange(P[1], device="cuda")
+    fz = torch.where(2 * kz > P[2], P[2] - kz, kz); sz = torch.where(2 * kz > P[2], -1.0, 1.0)
+    fy = torch.where(2 * ky > P[1], P[1] - ky, ky); sy = torch.where(2 * ky > P[1], -1.0, 1.0)
+    K = []
+    for comp, (py, pz) in enumerate(((0, 0), (0, 0), (0, 0), (1, 0), (0, 1), (1, 1))):
+        o = torch.from_numpy(sim.get_demag_kernel(comp)).cuda()
+        full = o[fz][:, fy]
+        if py: full = full * sy[None, :, None]
+        if pz: full = full * sz[:, None, None]
+        K.append(full.contiguous())
+    Ms = wl.mat["Ms"]
+    scale = float(P[0] * P[1] * P[2])          # K-hat carries 1/(Px Py Pz); irfftn normalises again
+
+    def conv(m):
+        M = torch.fft.rfftn(m, s=(P[2], P[1], P[0]), dim=(1, 2, 3))
+        H = torch.stack((K[0] * M[0] + K[3] * M[1] + K[4] * M[2],
+                         K[3] * M[0] + K[1] * M[1] + K[5] * M[2],
+                         K[4] * M[0] + K[5] * M[1] + K[2] * M[2]))
+        return torch.fft.irfftn(H, s=(P[2], P[1], P[0]), dim=(1, 2, 3))[:, :Nz, :Ny, :Nx] * (Ms * scale)
+
+    ref = sim.demag_field(md)
+    out = conv(md)
+    err = float((out - ref).abs().max() / ref.abs().max())
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    for f in (conv, lambda m: sim.demag_field(m, out=ref)):
+        f(md); f(md)
+    res = {}
+    for name, f in (("cufft_torch", conv), ("ours_demag_field", lambda m: sim.demag_field(m, out=ref))):
+        torch.cuda.synchronize(); e0.record()
+        for _ in range(args.steps):
+            f(md)
+        e1.record(); torch.cuda.synchronize()
+        res[name] = e0.elapsed_time(e1) / args.steps
+    print(json.dumps({"metric": "magnetostatic convolution, ms per call", "config": {"workload": wl.name},
+                      "cufft_torch_ms": res["cufft_torch"], "ours_demag_field_ms": res["ours_demag_field"],
+                      "max_rel_difference": err, "dtype": "f32", "data": "synthetic", "n_gpus": 1,
+                      "note": "torch.fft (cuFFT) with materialised padding and full half-spectrum kernel; bench-only"}))
+    sim.close()
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -230,12 +284,15 @@ def main():
     ap.add_argument("--fast", type=int, default=-1, help="bit mask for mm_set_fast_path (default: all)")
     ap.add_argument("--exchange-in-kernel", action="store_true",
                     help="the paper's variant (PAPER.md:85): exchange stencil inside the convolution kernel")
+    ap.add_argument("--cufft", action="store_true", help="bench-only comparison with the FFT library (torch.fft)")
     ap.add_argument("--sweep", action="store_true", help="Euler-step time on N^2 / N^3 grids (Table 1 shape)")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
     if args.sweep:
         return run_sweep(args)
+    if args.cufft:
+        return run_cufft_compare(args)
 
     import numpy as np
     import torch
