@@ -15,12 +15,16 @@
  *    data_ptr()); pointers named *_host are HOST pointers.  The library never frees, reallocates or
  *    keeps caller memory beyond the call (asynchronous calls keep it until the stream reaches them).
  *  - The context owns the transformed kernel K-hat, FFT workspaces, twiddle tables, Runge-Kutta
- *    buffers and device scalars.  Nothing is allocated on the device after mm_demag_init.
+ *    buffers and device scalars.  Nothing is allocated on the device after mm_demag_init, with one
+ *    exception: the first mm_set_material that asks for exchange_in_kernel allocates a second copy of
+ *    K-hat (kept until mm_destroy).
  *  - All device work is enqueued on the CUDA stream given to mm_create.  mm_heff / mm_torque /
- *    mm_stage are asynchronous with respect to the host; mm_step synchronises the stream once, at its
+ *    mm_demag_field / mm_fused_eval are asynchronous with respect to the host; mm_step synchronises the stream once, at its
  *    end, to return dt / err / accepted.
  *  - A context belongs to the CUDA device that is current when mm_create is called; that device must be
  *    current for every later call on the context (one process per GPU is the intended use).
+ *  - A context has no hidden global state: the library reads no environment variable; tuning switches are
+ *    per-context options (mm_set_option).
  *  - There is no CPU fallback, no cuFFT and no tensor-core path inside the library: every hot-path
  *    step runs in hand-written sm_100a kernels.  Without a CUDA device mm_create fails with MM_ECUDA.
  */
@@ -222,6 +226,20 @@ mm_status mm_demag_khat_host(const double cellsize[3], const int grid[3], const 
 /* mm_padded_size -- padded FFT sizes P[3] and the octant extents C[3] = P/2 + 1 of this context. */
 mm_status mm_padded_size(const mm_ctx* ctx, int P_out[3], int C_out[3]);
 
+/* mm_padded_size_of -- the same rule (reading A9: 2 N open, N periodic, 1 for a one-cell axis) for a grid
+ * without a context; HOST only, needs no device.  MM_EUNSUPPORTED if a padded size is not 2^a 3^b 5^c 7^d. */
+mm_status mm_padded_size_of(const int grid[3], const int pbc[3], int P_out[3], int C_out[3]);
+
+/* mm_set_option -- per-context tuning switches (integers; defaults are the measured best on B200):
+ *   "graph"          1 (default): mm_steps_fixed replays a captured CUDA graph of one step; 0: plain launches
+ *   "x_pipe"         bit 0: forward x pass in its cp.async-pipelined form (default 1); bit 1: inverse x pass too
+ *   "mid_pipe"       1 (default): persistent, pipelined last-axis pass; 0: one block per line set
+ *   "chunk_w"        > 0: run the y / last-axis passes in L2-resident chunks of that many kx columns (multiple
+ *                    of 16; default 0 = whole-array passes); "chunk_streams" 1..4 streams for them (default 3).
+ *                    These two must be set BEFORE mm_demag_init (MM_ESTATE afterwards).
+ * Results do not depend on any option (tested bit for bit).  Errors: MM_EINVAL (unknown key, bad value). */
+mm_status mm_set_option(mm_ctx* ctx, const char* key, int value);
+
 /* mm_launch_count -- number of kernels this context has launched so far (bench.py "gpu_launches"). */
 uint64_t mm_launch_count(const mm_ctx* ctx);
 
@@ -238,7 +256,7 @@ mm_status mm_kernel_times(mm_ctx* ctx, double sec_out[7], uint64_t count_out[7])
  * when the grid allows (1 forward x, 2 the y passes, 4 last axis + K-hat multiply, 8 inverse x +
  * fused epilogue, 16 the split last pass: inverse x to an H_ms field, then a streaming per-cell
  * kernel; 16 wins over 8; 32 allows the L2-resident kx chunks of the y / last-axis passes when the
- * environment variable MM_CHUNK_W asks for them); a negative value (and the default) enables all, 0
+ * option "chunk_w" asks for them); a negative value (and the default) enables all, 0
  * forces the generic shared-memory
  * radix-2/3/4/5 kernels.  Both families use the same layouts, so tests compare them pass by pass. */
 mm_status mm_set_fast_path(mm_ctx* ctx, int enable);

@@ -12,8 +12,8 @@ struct FastPlan {
     float2* twx;                         // ok_xr: exp(-i pi k / Lc), k < Lc = Px / 2
     float2* tw[3];                       // per axis: tw[k2 * T + t] = exp(-2 pi i t k2 / L)
     int nsm;                             // SM count (persistent grids)
-    int x_pipe;                          // x passes, cp.async-pipelined forms: bit 0 forward (default), bit 1 inverse (env MM_X_PIPE)
-    int mid_pipe;                        // last-axis pass: persistent cp.async-pipelined kernel (env MM_MID_PIPE)
+    int x_pipe;                          // x passes, cp.async-pipelined forms: bit 0 forward (default), bit 1 inverse (option "x_pipe")
+    int mid_pipe;                        // last-axis pass: persistent pipelined kernel (option "mid_pipe")
     int chunk_w, nstream;                // chunked a2-a4: columns per chunk (0 = whole-array passes), streams
     cudaStream_t stream[4];
     cudaEvent_t ev_fork, ev_join[4];
@@ -371,16 +371,10 @@ inline bool fast_plan_init(FastPlan& fp, const Geom& g, std::string* err)
     fp.ok_y = g.Py > 1 && ff::split(g.Py, &T, &E);
     fp.ok_mid3 = g.Pz > 1 && g.Py > 1 && ff::split(g.Pz, &T, &E) && E <= 16;
     fp.ok_mul2 = g.Pz == 1 && fp.ok_y;
-    fp.nsm = 148;
-    // L2-resident chunks (env MM_CHUNK_W = columns per chunk, multiple of 16): off by default -- measured on
-    // B200 at 512x512x64 they give bit-identical results and cut DRAM traffic, but no time, because the
-    // y and last-axis passes are bound by instruction issue, not by HBM (profiles/).
-    fp.chunk_w = 0;
-    fp.x_pipe = getenv("MM_X_PIPE") ? atoi(getenv("MM_X_PIPE")) : 1;
-    fp.mid_pipe = getenv("MM_MID_PIPE") ? atoi(getenv("MM_MID_PIPE")) : 1;
-    fp.nstream = 3;
-    if (getenv("MM_CHUNK_W")) fp.chunk_w = atoi(getenv("MM_CHUNK_W"));
-    if (getenv("MM_CHUNK_STREAMS")) fp.nstream = atoi(getenv("MM_CHUNK_STREAMS"));
+    // fp.x_pipe, fp.mid_pipe, fp.chunk_w, fp.nstream come from the context (mm_set_option; defaults set by
+    // mm_create).  L2-resident chunks (chunk_w = columns per chunk, multiple of 16) are off by default:
+    // measured on B200 at 512x512x64 they give bit-identical results and cut DRAM traffic, but no time,
+    // because the y and last-axis passes are bound by instruction issue, not by HBM (profiles/).
     if (fp.chunk_w % 16 != 0 || fp.chunk_w < 0 || !(fp.ok_y && fp.ok_mid3)) fp.chunk_w = 0;
     if (fp.nstream < 1) fp.nstream = 1;
     if (fp.nstream > 4) fp.nstream = 4;
@@ -400,8 +394,11 @@ inline bool fast_plan_init(FastPlan& fp, const Geom& g, std::string* err)
             return false;
         }
     }
-    cudaGetDevice(&dev);
-    cudaDeviceGetAttribute(&fp.nsm, cudaDevAttrMultiProcessorCount, dev);
+    if (cudaGetDevice(&dev) != cudaSuccess ||
+        cudaDeviceGetAttribute(&fp.nsm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || fp.nsm < 1) {
+        if (err) *err = "fast plan: cannot read the SM count of the current device";
+        return false;
+    }
     const int P[3] = { fp.ok_xr ? g.Px / 2 : g.Px, g.Py, g.Pz };
     if (fp.ok_xr) {
         const int Lc = g.Px / 2;

@@ -129,7 +129,10 @@ struct mm_ctx {
     int fast;
     cudaStream_t gstream;   // the context's own stream for graph capture / replay (created on first use)
     cudaEvent_t gev[2];
-    int use_graph;    // mm_steps_fixed may replay a captured step (env MM_GRAPH=0 switches it off)
+    cudaGraphExec_t gexec;  // instantiated graph of one fixed step, reused while its key below holds
+    int g_method; double g_dt; float* g_m; uint64_t g_epoch, g_per;
+    uint64_t epoch;   // bumped by mm_set_material / mm_set_option / mm_set_fast_path
+    int use_graph;    // mm_steps_fixed may replay a captured step (option "graph" = 0 switches it off)
     // device
     float* khat;      // demag kernel octant
     float* khat_ex;   // khat + exchange stencil on the diagonal (exchange_in_kernel), built at mm_set_material
@@ -414,7 +417,7 @@ mm_status refresh_khat_ex(mm_ctx* c)
     float w[3];
     for (int a = 0; a < 3; ++a)
         w[a] = ext[a] > 1 ? (float)(2.0 * c->mat.Aex / (MU0 * Ms * Ms * c->cell[a] * c->cell[a])) : 0.f;
-    k_khat_exchange<<<148 * 8, 256, 0, c->stream>>>(g, c->khat, c->khat_ex, w[0], w[1], w[2]);
+    k_khat_exchange<<<c->fp.nsm * 8, 256, 0, c->stream>>>(g, c->khat, c->khat_ex, w[0], w[1], w[2]);
     CUDA_TRY(c, cudaGetLastError());
     return MM_OK;
 }
@@ -553,11 +556,15 @@ mm_status enqueue_step(mm_ctx* c, float* m_dev, mm_method method, const Tableau&
     CUDA_TRY(c, cudaMemsetAsync(c->maxbits, 0, sizeof(unsigned int), c->stream));
     const uint64_t step = c->step_index;
     int s0 = 0;
-    if (tab.fsal && c->k0_valid && c->k0_method == (int)method) {
+    // a method without the FSAL property overwrites kb[0] with its own first stage: the saved one is gone
+    if (!tab.fsal) c->k0_valid = false;
+    // with a thermal field the saved stage carries the previous step's draw (reading A6: one draw per
+    // step, held over that step's own stages): evaluate k_1 afresh
+    if (tab.fsal && c->k0_valid && c->k0_method == (int)method && !(c->mat.T > 0)) {
         // k_1 of this step is the last stage of the previous accepted step: skip the evaluation
         const double dtr = dev_dt ? 1.0 : dt * gamma0_of(c) * c->mat.Ms;
         c->kt.begin(KT_OTHER);
-        k_combine<<<148 * 8, 256, 0, c->stream>>>(n, m_dev, c->ms[0], 1, (float)(dtr * tab.A[1][0]), 0.f,
+        k_combine<<<c->fp.nsm * 8, 256, 0, c->stream>>>(n, m_dev, c->ms[0], 1, (float)(dtr * tab.A[1][0]), 0.f,
                                                   c->kb[0], c->kb[0], dev_dt ? &c->ctl->dtr : nullptr);
         c->kt.end(KT_OTHER);
         s0 = 1;
@@ -601,11 +608,8 @@ mm_status mm_create(mm_ctx** out, const int grid[3], const double cellsize[3], c
         if (pbc[a] < 0) return fail(nullptr, MM_EINVAL, "pbc must be >= 0");
     }
     int P[3];
-    for (int a = 0; a < 3; ++a) {
-        P[a] = pbc[a] > 0 ? grid[a] : (grid[a] > 1 ? 2 * grid[a] : 1);
-        if (!smooth235(P[a]))
-            return fail(nullptr, MM_EUNSUPPORTED, "padded size has a prime factor other than 2, 3, 5, 7");
-    }
+    if (mm_padded_size_of(grid, pbc, P, nullptr) != MM_OK)
+        return fail(nullptr, MM_EUNSUPPORTED, "padded size has a prime factor other than 2, 3, 5, 7");
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) {
         cudaGetLastError();
@@ -630,7 +634,9 @@ mm_status mm_create(mm_ctx** out, const int grid[3], const double cellsize[3], c
     c->fast = FAST_ALL;
     c->gstream = nullptr;
     c->gev[0] = c->gev[1] = nullptr;
-    c->use_graph = getenv("MM_GRAPH") ? atoi(getenv("MM_GRAPH")) : 1;
+    c->use_graph = 1;
+    c->gexec = nullptr; c->g_method = -1; c->g_dt = 0.0; c->g_m = nullptr; c->g_epoch = 0; c->g_per = 0;
+    c->epoch = 1;
     c->khat = nullptr; c->khat_ex = nullptr; c->specA = c->specB = nullptr;
     for (int a = 0; a < 3; ++a) c->tw[a] = nullptr;
     for (int i = 0; i < 7; ++i) c->kb[i] = nullptr;
@@ -644,6 +650,13 @@ mm_status mm_create(mm_ctx** out, const int grid[3], const double cellsize[3], c
     c->k0_valid = false;
     c->k0_method = -1;
     std::memset(&c->fp, 0, sizeof(c->fp));
+    {
+        int dev = 0;
+        c->fp.nsm = 0;
+        if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&c->fp.nsm, cudaDevAttrMultiProcessorCount, dev);
+        if (c->fp.nsm < 1) c->fp.nsm = 1;
+    }
+    c->fp.x_pipe = 1; c->fp.mid_pipe = 1; c->fp.chunk_w = 0; c->fp.nstream = 3;     // mm_set_option defaults
     *out = c;
     return MM_OK;
 }
@@ -663,14 +676,43 @@ mm_status mm_set_material(mm_ctx* c, const mm_material* mat)
     }
     c->mat = *mat;
     c->has_mat = true;
+    c->epoch++;
     c->k0_valid = false;
     return refresh_khat_ex(c);
 }
+
+// everything mm_demag_init allocates; pointers are reset so that the call can be repeated after a failure
+static void free_workspaces(mm_ctx* c)
+{
+    auto fr = [](auto*& p) { if (p) cudaFree(p); p = nullptr; };
+    fr(c->khat); fr(c->khat_ex); fr(c->specA); fr(c->specB);
+    for (int a = 0; a < 3; ++a) fr(c->tw[a]);
+    for (int i = 0; i < 7; ++i) fr(c->kb[i]);
+    fr(c->ms[0]); fr(c->ms[1]); fr(c->mtmp); fr(c->mhost); fr(c->hfield);
+    fr(c->maxbits); fr(c->ctl); fr(c->ctl_scratch); fr(c->step_dev);
+    fast_plan_destroy(c->fp);
+}
+
+static mm_status demag_init_impl(mm_ctx* c);
 
 mm_status mm_demag_init(mm_ctx* c)
 {
     if (!c) return MM_EINVAL;
     if (c->has_demag) return MM_OK;
+    mm_status s = demag_init_impl(c);
+    // the set-up copies and memsets run on the legacy default stream, the kernels of this context on the
+    // caller's stream (possibly non-blocking): order everything before returning (the call is blocking)
+    if (s == MM_OK && cudaDeviceSynchronize() != cudaSuccess) s = fail(c, MM_ECUDA, "mm_demag_init: device synchronisation failed");
+    if (s != MM_OK) {
+        c->has_demag = false;
+        free_workspaces(c);
+        cudaGetLastError();
+    }
+    return s;
+}
+
+static mm_status demag_init_impl(mm_ctx* c)
+{
     const Geom& g = c->g;
     const int grid[3] = { g.Nx, g.Ny, g.Nz };
     const size_t nC = (size_t)g.Cx * g.Cy * g.Cz;
@@ -847,30 +889,37 @@ static mm_status steps_fixed_impl(mm_ctx* c, float* m_dev, mm_method method, con
             cudaMemcpyAsync(c->step_dev, &si, sizeof(si), cudaMemcpyHostToDevice, c->stream);
             cudaStreamSynchronize(c->stream);              // `si` is a stack variable
         }
-        if ((s = one_step()) != MM_OK) { c->step_on_device = false; return s; }   // also sets kernel attributes outside the capture
-        done = 1;
-        cudaGraph_t graph = nullptr;
-        cudaGraphExec_t exec = nullptr;
-        const uint64_t l0 = c->kt.launches;
-        if (cudaStreamBeginCapture(c->stream, cudaStreamCaptureModeThreadLocal) == cudaSuccess) {
-            const mm_status sc = one_step();
-            const cudaError_t ec = cudaStreamEndCapture(c->stream, &graph);
-            if (sc == MM_OK && ec == cudaSuccess && graph &&
-                cudaGraphInstantiate(&exec, graph, 0) == cudaSuccess) {
-                const uint64_t per = c->kt.launches - l0;
-                c->kt.launches = l0;
-                c->step_index--;                           // the captured step has not run yet
-                for (; done < n; ++done) {
-                    if (cudaGraphLaunch(exec, c->stream) != cudaSuccess) break;
-                    c->kt.launches += per;
-                    c->step_index++;
+        // the instantiated graph of one step is kept in the context and reused while everything baked into
+        // its kernel arguments is unchanged: method, dt, the state pointer, material / options (epoch)
+        const bool hit = c->gexec && c->g_method == (int)method && c->g_dt == dt && c->g_m == m_dev &&
+                         c->g_epoch == c->epoch;
+        if (!hit) {
+            if (c->gexec) { cudaGraphExecDestroy(c->gexec); c->gexec = nullptr; }
+            if ((s = one_step()) != MM_OK) { c->step_on_device = false; return s; }   // also sets kernel attributes outside the capture
+            done = 1;
+            cudaGraph_t graph = nullptr;
+            const uint64_t l0 = c->kt.launches;
+            if (n > 1 && cudaStreamBeginCapture(c->stream, cudaStreamCaptureModeThreadLocal) == cudaSuccess) {
+                const mm_status sc = one_step();
+                const cudaError_t ec = cudaStreamEndCapture(c->stream, &graph);
+                if (sc == MM_OK && ec == cudaSuccess && graph &&
+                    cudaGraphInstantiate(&c->gexec, graph, 0) == cudaSuccess) {
+                    c->g_method = (int)method; c->g_dt = dt; c->g_m = m_dev; c->g_epoch = c->epoch;
+                    c->g_per = c->kt.launches - l0;
+                } else {
+                    c->gexec = nullptr;
                 }
-            } else {
                 c->kt.launches = l0;
-                c->step_index--;
+                c->step_index--;                           // the captured step has not run
+                if (graph) cudaGraphDestroy(graph);
             }
-            if (exec) cudaGraphExecDestroy(exec);
-            if (graph) cudaGraphDestroy(graph);
+        }
+        if (c->gexec) {
+            for (; done < n; ++done) {
+                if (cudaGraphLaunch(c->gexec, c->stream) != cudaSuccess) break;
+                c->kt.launches += c->g_per;
+                c->step_index++;
+            }
         }
         cudaGetLastError();                                // a refused capture must not surface later
         if (c->step_on_device) {
@@ -986,7 +1035,7 @@ mm_status mm_steps_adaptive(mm_ctx* c, float* m_dev, mm_method method, int ntria
         if (s != MM_OK) return s;
         k_step_control<<<1, 1, 0, c->stream>>>(c->ctl, c->maxbits);
         const bool fs = tab.fsal;
-        k_step_commit<<<148 * 8, 256, 0, c->stream>>>(n4, (const float4*)newstate, (float4*)m_dev,
+        k_step_commit<<<c->fp.nsm * 8, 256, 0, c->stream>>>(n4, (const float4*)newstate, (float4*)m_dev,
                                                        fs ? (const float4*)c->kb[tab.S - 1] : nullptr,
                                                        fs ? (float4*)c->kb[0] : nullptr, c->ctl);
         c->kt.launches += 2;
@@ -1054,12 +1103,12 @@ mm_status mm_steps_maxdm(mm_ctx* c, float* m_dev, mm_method method, double max_d
         k_maxdm_dt<<<1, 1, 0, c->stream>>>(c->ctl, c->maxbits, max_dm);
         c->kt.launches++;
         if (tab.S == 1) {
-            k_combine<<<148 * 8, 256, 0, c->stream>>>(ncl, m_dev, c->mtmp, 1, (float)tab.b[0], 0.f, c->kb[0], c->kb[0],
+            k_combine<<<c->fp.nsm * 8, 256, 0, c->stream>>>(ncl, m_dev, c->mtmp, 1, (float)tab.b[0], 0.f, c->kb[0], c->kb[0],
                                                       &c->ctl->dtr);
-            k_normalise<<<148 * 8, 256, 0, c->stream>>>(ncl, c->mtmp, m_dev);
+            k_normalise<<<c->fp.nsm * 8, 256, 0, c->stream>>>(ncl, c->mtmp, m_dev);
             c->kt.launches += 2;
         } else {
-            k_combine<<<148 * 8, 256, 0, c->stream>>>(ncl, m_dev, c->ms[0], 1, (float)tab.A[1][0], 0.f, c->kb[0],
+            k_combine<<<c->fp.nsm * 8, 256, 0, c->stream>>>(ncl, m_dev, c->ms[0], 1, (float)tab.A[1][0], 0.f, c->kb[0],
                                                       c->kb[0], &c->ctl->dtr);
             c->kt.launches++;
             for (int st = 1; st < tab.S; ++st)
@@ -1103,7 +1152,7 @@ mm_status mm_average(mm_ctx* c, const float* field_dev, double avg_host[3])
     double* acc = reinterpret_cast<double*>(c->ctl_scratch);
     CUDA_TRY(c, cudaMemsetAsync(acc, 0, 3 * sizeof(double), c->stream));
     const size_t n = ncell(c->g);
-    k_average<<<148 * 4, 256, 0, c->stream>>>(n, field_dev, acc);
+    k_average<<<c->fp.nsm * 4, 256, 0, c->stream>>>(n, field_dev, acc);
     c->kt.launches++;
     double h[3];
     CUDA_TRY(c, cudaMemcpyAsync(h, acc, sizeof(h), cudaMemcpyDeviceToHost, c->stream));
@@ -1199,11 +1248,10 @@ mm_status mm_demag_khat_host(const double cellsize[3], const int grid[3], const 
                              size_t n)
 {
     if (!cellsize || !grid || !pbc || !out_host) return MM_EINVAL;
-    size_t nC = 1;
-    for (int a = 0; a < 3; ++a) {
-        const int P = pbc[a] > 0 ? grid[a] : (grid[a] > 1 ? 2 * grid[a] : 1);
-        nC *= (size_t)(P / 2 + 1);
-    }
+    int Cs[3];
+    const mm_status ps = mm_padded_size_of(grid, pbc, nullptr, Cs);
+    if (ps != MM_OK) return ps;
+    const size_t nC = (size_t)Cs[0] * Cs[1] * Cs[2];
     if (n < 6 * nC) return MM_EINVAL;
     std::string err;
     return (mm_status)mmh::build_khat(cellsize, grid, pbc, out_host, &err);
@@ -1217,12 +1265,45 @@ mm_status mm_padded_size(const mm_ctx* c, int P_out[3], int C_out[3])
     return MM_OK;
 }
 
+mm_status mm_padded_size_of(const int grid[3], const int pbc[3], int P_out[3], int C_out[3])
+{
+    if (!grid || !pbc) return MM_EINVAL;
+    for (int a = 0; a < 3; ++a) {
+        if (grid[a] < 1 || pbc[a] < 0) return MM_EINVAL;
+        const int P = pbc[a] > 0 ? grid[a] : (grid[a] > 1 ? 2 * grid[a] : 1);
+        if (!smooth235(P)) return MM_EUNSUPPORTED;
+        if (P_out) P_out[a] = P;
+        if (C_out) C_out[a] = P / 2 + 1;
+    }
+    return MM_OK;
+}
+
+mm_status mm_set_option(mm_ctx* c, const char* key, int value)
+{
+    if (!c || !key) return MM_EINVAL;
+    const std::string k(key);
+    c->epoch++;
+    if (k == "graph") { c->use_graph = value != 0; return MM_OK; }
+    if (k == "x_pipe") { c->fp.x_pipe = value & 3; return MM_OK; }
+    if (k == "mid_pipe") { c->fp.mid_pipe = value; return MM_OK; }
+    if (k == "chunk_w" || k == "chunk_streams") {
+        // the chunk streams and the slot layout are fixed when the workspaces are made
+        if (c->has_demag) return fail(c, MM_ESTATE, "option " + k + " must be set before mm_demag_init");
+        if (value < 0) return fail(c, MM_EINVAL, "option " + k + " must be >= 0");
+        if (k == "chunk_w") c->fp.chunk_w = value;
+        else c->fp.nstream = value;
+        return MM_OK;
+    }
+    return fail(c, MM_EINVAL, "unknown option '" + k + "'");
+}
+
 uint64_t mm_launch_count(const mm_ctx* c) { return c ? c->kt.launches : 0; }
 
 mm_status mm_set_fast_path(mm_ctx* c, int enable)
 {
     if (!c) return MM_EINVAL;
     c->fast = enable < 0 ? FAST_ALL : (enable & FAST_ALL);
+    c->epoch++;
     return MM_OK;
 }
 
@@ -1234,10 +1315,10 @@ mm_status mm_copy_bandwidth(mm_ctx* c, const void* src_dev, void* dst_dev, size_
     CUDA_TRY(c, cudaEventCreate(&e0));
     CUDA_TRY(c, cudaEventCreate(&e1));
     const size_t n4 = nbytes / 16;
-    k_copy4<<<148 * 16, 512, 0, c->stream>>>((const float4*)src_dev, (float4*)dst_dev, n4);
+    k_copy4<<<c->fp.nsm * 16, 512, 0, c->stream>>>((const float4*)src_dev, (float4*)dst_dev, n4);
     CUDA_TRY(c, cudaEventRecord(e0, c->stream));
     for (int i = 0; i < reps; ++i)
-        k_copy4<<<148 * 16, 512, 0, c->stream>>>((const float4*)src_dev, (float4*)dst_dev, n4);
+        k_copy4<<<c->fp.nsm * 16, 512, 0, c->stream>>>((const float4*)src_dev, (float4*)dst_dev, n4);
     CUDA_TRY(c, cudaEventRecord(e1, c->stream));
     CUDA_TRY(c, cudaEventSynchronize(e1));
     float ms = 0.f;
@@ -1254,29 +1335,15 @@ const char* mm_last_error(const mm_ctx* c) { return c ? c->err.c_str() : g_creat
 void mm_destroy(mm_ctx* c)
 {
     if (!c) return;
-    cudaFree(c->khat);
-    cudaFree(c->khat_ex);
-    cudaFree(c->specA);
-    cudaFree(c->specB);
-    for (int a = 0; a < 3; ++a) cudaFree(c->tw[a]);
-    for (int i = 0; i < 7; ++i) cudaFree(c->kb[i]);
-    cudaFree(c->ms[0]);
-    cudaFree(c->ms[1]);
-    cudaFree(c->mtmp);
-    cudaFree(c->mhost);
-    cudaFree(c->hfield);
+    free_workspaces(c);
     for (int k = 0; k < KT_N; ++k) {
         for (int i = 0; i < c->kt.cap[k]; ++i) cudaEventDestroy(c->kt.ev[k][i]);
         delete[] c->kt.ev[k];
     }
-    cudaFree(c->maxbits);
-    cudaFree(c->ctl);
-    cudaFree(c->ctl_scratch);
-    cudaFree(c->step_dev);
+    if (c->gexec) cudaGraphExecDestroy(c->gexec);
     if (c->gstream) cudaStreamDestroy(c->gstream);
     for (int i = 0; i < 2; ++i)
         if (c->gev[i]) cudaEventDestroy(c->gev[i]);
-    fast_plan_destroy(c->fp);
     delete c;
 }
 

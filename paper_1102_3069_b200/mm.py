@@ -87,6 +87,8 @@ def lib():
         L.mm_demag_tensor_host.argtypes = [d3, i3, i3, C.c_size_t, vp, vp]
         L.mm_demag_khat_host.argtypes = [d3, i3, i3, vp, C.c_size_t]
         L.mm_padded_size.argtypes = [vp, i3, i3]
+        L.mm_padded_size_of.argtypes = [i3, i3, i3, i3]
+        L.mm_set_option.argtypes = [vp, C.c_char_p, C.c_int]
         L.mm_launch_count.argtypes = [vp]
         L.mm_launch_count.restype = C.c_uint64
         L.mm_set_fast_path.argtypes = [vp, C.c_int]
@@ -120,8 +122,10 @@ def demag_tensor_host(cell, grid, pbc, offsets) -> np.ndarray:
 
 def demag_khat_host(cell, grid, pbc) -> np.ndarray:
     """mm_demag_khat_host: K-hat octant, shape (6, Cz, Cy, Cx) float32, as uploaded by mm_demag_init."""
-    P = [int(n) if p > 0 else (2 * int(n) if n > 1 else 1) for n, p in zip(grid, pbc)]
-    Cs = [p // 2 + 1 for p in P]
+    P, Cs = (C.c_int * 3)(), (C.c_int * 3)()
+    st = lib().mm_padded_size_of(_i3(grid), _i3(pbc), P, Cs)
+    if st != MM_OK:
+        raise MMError(st, "mm_padded_size_of")
     out = np.zeros((6, Cs[2], Cs[1], Cs[0]), dtype=np.float32)
     st = lib().mm_demag_khat_host(_d3(cell), _i3(grid), _i3(pbc), out.ctypes.data_as(C.c_void_p), out.size)
     if st != MM_OK:
@@ -132,7 +136,8 @@ def demag_khat_host(cell, grid, pbc) -> np.ndarray:
 class Sim:
     """One mm_ctx.  Fields are torch CUDA float32 tensors of shape (3, Nz, Ny, Nx)."""
 
-    def __init__(self, grid, cell, pbc=(0, 0, 0), mat=None, demag=True, stream=None, demag_init=True):
+    def __init__(self, grid, cell, pbc=(0, 0, 0), mat=None, demag=True, stream=None, demag_init=True,
+                 options=None):
         import torch
         self.torch = torch
         self.L = lib()
@@ -148,6 +153,8 @@ class Sim:
         st = self.L.mm_create(C.byref(self.ctx), _i3(grid), _d3(cell), _i3(pbc), sp)
         if st != MM_OK:
             raise MMError(st, self.L.mm_last_error(None).decode())
+        for k, v in (options or {}).items():
+            self.set_option(k, v)
         if mat is not None:
             self.set_material(mat, demag)
         if demag_init:
@@ -164,6 +171,9 @@ class Sim:
     def set_material(self, mat, demag=True):
         m = mat if isinstance(mat, Material) else Material.from_dict(mat, demag)
         self._chk(self.L.mm_set_material(self.ctx, C.byref(m)))
+
+    def set_option(self, key, value):
+        self._chk(self.L.mm_set_option(self.ctx, key.encode(), int(value)))
 
     def demag_init(self):
         self._chk(self.L.mm_demag_init(self.ctx))

@@ -21,9 +21,9 @@ def oracle_problem(wl, demag="fft"):
     return orc.Problem(wl.grid, wl.cell, wl.pbc, oracle_material(wl.mat), demag=demag)
 
 
-def gpu_sim(wl, demag=True, fast=True):
+def gpu_sim(wl, demag=True, fast=True, options=None):
     import paper_1102_3069_b200 as mm
-    sim = mm.Sim(wl.grid, wl.cell, wl.pbc, wl.mat, demag=demag)
+    sim = mm.Sim(wl.grid, wl.cell, wl.pbc, wl.mat, demag=demag, options=options)
     sim.set_fast_path(fast)
     return sim
 

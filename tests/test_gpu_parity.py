@@ -317,13 +317,11 @@ def test_fast_path_rk4_and_rkdp_steps_match_generic():
 
 
 @pytest.mark.parametrize("grid,pbc", [((64, 32, 64), (0, 0, 0)), ((128, 32, 32), (0, 0, 1))])
-def test_chunked_l2_resident_passes_match_whole_array_passes(grid, pbc, monkeypatch):
+def test_chunked_l2_resident_passes_match_whole_array_passes(grid, pbc):
     """a2-a4 in kx chunks through a compact buffer (several streams) against the whole-array passes."""
-    monkeypatch.setenv("MM_CHUNK_W", "16")
-    monkeypatch.setenv("MM_CHUNK_STREAMS", "3")
     wl = util.small(grid, (3e-9, 3e-9, 3e-9), pbc)
     m = wlm.initial_m(wl)
-    sim = util.gpu_sim(wl, fast=31)
+    sim = util.gpu_sim(wl, fast=31, options={"chunk_w": 16, "chunk_streams": 3})
     md = util.to_dev(m)
     H0 = sim.demag_field(md).double()
     T0 = sim.torque(md).double()
@@ -425,14 +423,13 @@ def test_full_size_headline_grid_local_terms_and_torque():
 
 
 @pytest.mark.parametrize("method", ["rk1", "rk4"])
-def test_graph_replayed_steps_equal_plain_launches(method, monkeypatch):
+def test_graph_replayed_steps_equal_plain_launches(method):
     """mm_steps_fixed replays a captured step for the fixed-step, non-FSAL methods: same bits as plain launches."""
     wl = util.small((32, 32, 1), (4e-9, 4e-9, 4e-9), alpha=0.5)
     m = wlm.initial_m(wl)
     out = []
-    for flag in ("1", "0"):
-        monkeypatch.setenv("MM_GRAPH", flag)
-        sim = util.gpu_sim(wl)
+    for flag in (1, 0):
+        sim = util.gpu_sim(wl, options={"graph": flag})
         md = util.to_dev(m)
         t, _ = sim.steps_fixed(md, method, 1e-13, 25)
         l0 = sim.launch_count()
@@ -505,6 +502,51 @@ def test_remaining_tableaux_follow_the_oracle(method):
     sim.close()
 
 
+@pytest.mark.parametrize("fsal", ["rkdp", "rk23"])
+def test_saved_first_stage_is_dropped_when_another_method_runs_in_between(fsal):
+    """FSAL step, then fixed steps of a method that overwrites the first-stage buffer, then FSAL again: the
+    saved k_1 belongs to an older state and must not be reused (the oracle evaluates k_1 afresh)."""
+    wl = util.small((24, 10, 6), init="tilted", alpha=0.05, Bext=(-0.0246, 0.0043, 0.0))
+    m = wlm.initial_m(wl)
+    pb = util.oracle_problem(wl)
+    dt = 6e-14
+    mo = m.astype(np.float64)
+    mo, _, _ = orc.rk_step(pb.torque, mo, dt, fsal)
+    for _ in range(3):
+        mo = orc.rk4_step(pb.torque, mo, dt)
+    mo, err_o, _ = orc.rk_step(pb.torque, mo, dt, fsal)          # k_1 evaluated on the current state
+    for inner in ("fixed", "step"):
+        sim = util.gpu_sim(wl)
+        md = util.to_dev(m)
+        sim.steps_fixed(md, fsal, dt, 1)
+        if inner == "fixed":
+            sim.steps_fixed(md, "rk4", dt, 3)
+        else:
+            for _ in range(3):
+                sim.step(md, "rk4", dt)
+        _, err_g = sim.steps_fixed(md, fsal, dt, 1)
+        assert np.abs(md.double().cpu().numpy() - mo).max() <= 2e-6
+        assert abs(err_g - err_o) <= 0.02 * err_o + 1e-9
+        sim.close()
+
+
+def test_fixed_step_fsal_method_with_thermal_field_redraws_per_step():
+    """Reading A6: one draw per step, held over that step's own stages -- the first stage of step n+1 is
+    evaluated with draw n+1, so the last stage of step n (draw n) cannot be reused when T > 0."""
+    wl = util.small((16, 12, 1), (4e-9, 4e-9, 2e-9), (2, 2, 0), init="xnoise", alpha=0.1, T=300.0, seed=3)
+    m = wlm.initial_m(wl)
+    pb = util.oracle_problem(wl)
+    dt, n = 5e-14, 4
+    mo = m.astype(np.float64)
+    for i in range(n):
+        mo, _, _ = orc.rk_step(lambda x: pb.torque(x, step=i, dt_thermal=dt), mo, dt, "rk23")
+    sim = util.gpu_sim(wl)
+    md = util.to_dev(m)
+    sim.steps_fixed(md, "rk23", dt, n)
+    assert np.abs(md.double().cpu().numpy() - mo).max() <= TOL_M
+    sim.close()
+
+
 def test_cash_karp_adaptive_run_matches_the_oracle_controller():
     wl = util.small((24, 10, 6), init="tilted", alpha=0.02, Bext=(-0.0246, 0.0043, 0.0), Ku=0.0)
     m = wlm.initial_m(wl)
@@ -561,15 +603,14 @@ def test_average_magnetisation():
     sim.close()
 
 
-def test_graph_replay_with_thermal_field_draws_per_step(monkeypatch):
+def test_graph_replay_with_thermal_field_draws_per_step():
     """With a thermal field the step index that selects the draw is advanced on the device during the
     replay: same bits as plain launches, and as the oracle's per-step draws (reading A6)."""
     wl = util.small((16, 12, 1), (4e-9, 4e-9, 2e-9), (2, 2, 0), init="xnoise", alpha=0.1, T=300.0, seed=3)
     m = wlm.initial_m(wl)
     out = []
-    for flag in ("1", "0"):
-        monkeypatch.setenv("MM_GRAPH", flag)
-        sim = util.gpu_sim(wl)
+    for flag in (1, 0):
+        sim = util.gpu_sim(wl, options={"graph": flag})
         md = util.to_dev(m)
         sim.steps_fixed(md, "rk4", 5e-14, 8)
         sim.steps_fixed(md, "rk4", 5e-14, 6)          # continues at step index 8

@@ -538,3 +538,79 @@ def test_heff_is_the_sum_of_its_terms():
              + orc.anisotropy_field(m, mat) + orc.zeeman_field(m, mat)
              + orc.thermal_field(mat, grid, cell, 3, 1e-13))
     assert np.allclose(H, parts, rtol=1e-12, atol=1e-6)
+
+
+# ---------------------------------------------------------------- round-2 pins ("parity unpinned")
+def test_current_gradient_on_a_staircase_shape():
+    """j_dot_grad_m with geometry=True (reading A15): an empty or missing neighbour is
+    replaced by the cell itself.  Pinned against plain Python loops on the L shape with a hole of
+    test_exchange_on_a_staircase_shape; `zero instead of the cell itself` or a wrong axis fails."""
+    rng = np.random.default_rng(11)
+    grid, cell = (5, 4, 3), (3e-9, 4e-9, 5e-9)
+    shape = np.ones((grid[2], grid[1], grid[0]), dtype=bool)
+    shape[:, 2:, 3:] = False
+    shape[1, 1, 1] = False
+    m = rng.standard_normal((3, grid[2], grid[1], grid[0]))
+    m /= np.sqrt((m * m).sum(0))
+    mg = m * shape[None]
+    j = (1.5e12, -0.7e12, 0.4e12)
+    mat = orc.Material(Ms=8e5, j=j, P=0.5, xi=0.04, geometry=True)
+    D = orc.j_dot_grad_m(mg, mat, grid, cell, (0, 0, 0))
+    ref = np.zeros_like(mg)
+    steps = ((0, 0, 1), (0, 1, 0), (1, 0, 0))            # (dz, dy, dx) of axis x, y, z
+    for z in range(grid[2]):
+        for y in range(grid[1]):
+            for x in range(grid[0]):
+                if not shape[z, y, x]:
+                    continue
+                for a, (dz, dy, dx) in enumerate(steps):
+                    def at(s):
+                        zz, yy, xx = z + s * dz, y + s * dy, x + s * dx
+                        inside = 0 <= zz < grid[2] and 0 <= yy < grid[1] and 0 <= xx < grid[0]
+                        return mg[:, zz, yy, xx] if inside and shape[zz, yy, xx] else mg[:, z, y, x]
+                    ref[:, z, y, x] += j[a] * (at(+1) - at(-1)) / (2.0 * cell[a])
+    occupied = np.broadcast_to(shape[None], mg.shape)
+    assert np.allclose(D[occupied], ref[occupied], rtol=0, atol=1e-12 * np.abs(ref).max())
+    # without empty cells the geometry branch is the plain rule
+    mat0 = orc.Material(Ms=8e5, j=j, P=0.5, xi=0.04)
+    assert np.allclose(orc.j_dot_grad_m(m, mat, grid, cell, (0, 0, 0)), orc.j_dot_grad_m(m, mat0, grid, cell, (0, 0, 0)))
+
+
+def test_average_m_against_a_hand_sum():
+    """<m> is the arithmetic mean per component over cells: `sum` instead of `mean`, or an
+    average over the wrong axis, fails on this non-symmetric 2 x 1 x 3 state."""
+    m = np.zeros((3, 3, 1, 2))
+    vals = [(1.0, 0.0, 0.0), (0.0, 1.0, 0.0), (0.6, 0.0, 0.8), (0.0, -0.6, 0.8), (0.0, 0.0, -1.0), (1.0, 0.0, 0.0)]
+    for i, v in enumerate(vals):
+        m[:, i // 2, 0, i % 2] = v
+    want = (np.array([2.6, 0.4, 0.6]) / 6.0)
+    assert np.allclose(orc.average_m(m), want, rtol=0, atol=1e-15)
+
+
+def test_max_dm_step_length_takes_the_largest_cell():
+    """dt = max_dm / max_i |dm/dt(i)|: with two uncoupled cells of different torque the larger
+    one sets the step (a mean, a minimum or a per-component maximum fails)."""
+    def f(m):
+        k = np.zeros_like(m)
+        k[:, 0, 0, 0] = (3.0, 4.0, 0.0)          # |k| = 5
+        k[:, 0, 0, 1] = (1.0, 2.0, 2.0)          # |k| = 3
+        k[:, 0, 0, 2] = (0.0, 0.0, 4.5)          # largest single component, |k| = 4.5
+        return k
+    m = np.zeros((3, 1, 1, 3)); m[2] = 1.0
+    dt, k = orc.max_dm_step_length(f, m, 0.02)
+    assert math.isclose(dt, 0.02 / 5.0, rel_tol=1e-15) and np.array_equal(k, f(m))
+
+
+def test_thermal_eta_word_to_component_map_is_the_documented_convention():
+    """Any map from the four Philox words to three N(0,1) numbers is a correct thermal field; which word
+    feeds which component is a convention (reading A6).  This pins the documented one on one cell:
+    eta = (r1 cos th1, r1 sin th1, r2 cos th2), u1 from word 0, th1 from word 1, u2 from word 2, th2 from
+    word 3, counter = (cell, 0, step, 0)."""
+    grid, seed, step = (3, 2, 2), 0x1234567, 7
+    eta = orc.thermal_eta(grid, seed, step)
+    cellidx = (1 * 2 + 1) * 3 + 2                  # z = 1, y = 1, x = 2
+    w = [int(v) for v in orc.philox4x32_10(cellidx, 0, step, 0, seed & 0xFFFFFFFF, seed >> 32)]
+    r1 = math.sqrt(-2.0 * math.log((w[0] + 1) / 2 ** 32)); th1 = 2 * math.pi * w[1] / 2 ** 32
+    r2 = math.sqrt(-2.0 * math.log((w[2] + 1) / 2 ** 32)); th2 = 2 * math.pi * w[3] / 2 ** 32
+    want = (r1 * math.cos(th1), r1 * math.sin(th1), r2 * math.cos(th2))
+    assert np.allclose(eta[:, 1, 1, 2], want, rtol=1e-13, atol=1e-15)

@@ -150,3 +150,31 @@ def test_thin_film_limit_nzz_tends_to_one():
     # and the self term of a very flat cell
     n = orc.tensor_at([[0, 0, 0]], (1000.0, 1000.0, 1.0))[0]
     assert n[2] > 0.995 and n[0] < 0.0025
+
+
+def _golden_rows():
+    import os
+    rows = []
+    with open(os.path.join(os.path.dirname(__file__), "golden", "tensor_near_field_survey.txt")) as f:
+        for line in f:
+            if line.startswith("#") or not line.strip():
+                continue
+            w = line.split()
+            rows.append((w[0], tuple(float(v) for v in w[1:4]), tuple(int(v) for v in w[4:7]),
+                         [None if v == "-" else float(v) for v in w[7:13]]))
+    return rows
+
+
+def test_printed_near_field_and_self_term_values():
+    """SURVEY.md:443-444 pins P5 (near field of unit cubes) and P6 (self terms of the configs' cells),
+    "[survey-computed]" there, stored in tests/golden/tensor_near_field_survey.txt.  The values are
+    printed to 12-15 digits; a wrong sign, a swapped component or a dropped term of f or g fails here."""
+    rows = _golden_rows()
+    assert sum(r[0] == "P5" for r in rows) == 5 and sum(r[0] == "P6" for r in rows) == 3
+    for kind, cell, off, want in rows:
+        got = orc.tensor_at([list(off)], cell)[0]
+        for c in range(6):
+            if want[c] is None:
+                assert abs(got[c]) <= 1e-15          # off-diagonal self terms vanish by symmetry
+            else:
+                assert abs(got[c] - want[c]) <= 2e-12, (kind, cell, off, c)   # printed to >= 12 digits
