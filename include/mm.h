@@ -233,7 +233,8 @@ mm_status mm_padded_size_of(const int grid[3], const int pbc[3], int P_out[3], i
 /* mm_set_option -- per-context tuning switches (integers; defaults are the measured best on B200):
  *   "graph"          1 (default): mm_steps_fixed replays a captured CUDA graph of one step; 0: plain launches
  *   "x_pipe"         bit 0: forward x pass in its cp.async-pipelined form (default 1); bit 1: inverse x pass too
- *   "mid_pipe"       1 (default): persistent, pipelined last-axis pass; 0: one block per line set
+ *   "mid_pipe"       last-axis pass: 2 (default) persistent, TMA tile loads, packed f32x2 codelets (padded z
+ *                    length 128; other lengths take 1); 1: persistent, cp.async-pipelined; 0: one block per line set
  *   "chunk_w"        > 0: run the y / last-axis passes in L2-resident chunks of that many kx columns (multiple
  *                    of 16; default 0 = whole-array passes); "chunk_streams" 1..4 streams for them (default 3).
  *                    These two must be set BEFORE mm_demag_init (MM_ESTATE afterwards).

@@ -850,4 +850,5 @@ k_inv_x_h_r(Geom g, const float2* __restrict__ specA, const float2* __restrict__
 }  // namespace ff
 }  // namespace mm
 
+#include "fft_packed.cuh"
 #include "fft_fast_plan.cuh"

@@ -14,6 +14,11 @@ struct FastPlan {
     int nsm;                             // SM count (persistent grids)
     int x_pipe;                          // x passes, cp.async-pipelined forms: bit 0 forward (default), bit 1 inverse (option "x_pipe")
     int mid_pipe;                        // last-axis pass: persistent pipelined kernel (option "mid_pipe")
+    // last-axis pass through TMA tiles and sibling-packed codelets (pk::k_mid_t; mid_pipe >= 2, Pz = 128)
+    bool ok_mid_t, has_kex_map;
+    CUtensorMap map_spec, map_k, map_kex;  // specB [3][Nz][Py][2 CxS] floats; K-hat / K-hat + exchange [6][Cz][Cy][CxK]
+    const float* k_ptr;                  // the K-hat array map_k describes (map_kex: any other)
+    float4* twp;                         // pk::k_mid_t twiddles
     int chunk_w, nstream;                // chunked a2-a4: columns per chunk (0 = whole-array passes), streams
     cudaStream_t stream[4];
     cudaEvent_t ev_fork, ev_join[4];
@@ -180,10 +185,30 @@ bool launch_y(const FastPlan& fp, const Geom& g, cudaStream_t st, const ColTile&
     return true;
 }
 
+template <bool PER>
+bool launch_mid_t(const FastPlan& fp, const Geom& g, cudaStream_t st, float2* specB, const float* khat)
+{
+    using M = pk::MidT<PER>;
+    static bool once[MM_MAX_DEV] = {};
+    if (!ensure_smem_dev(pk::k_mid_t<PER>, M::SMEM_BYTES, once)) return false;
+    const int nitem = ((g.Cx + 15) / 16) * (g.Py / 2 + 1);
+    const int per_sm = PER ? 2 : 3;
+    const int grid = nitem < fp.nsm * per_sm ? nitem : fp.nsm * per_sm;
+    pk::k_mid_t<PER><<<grid, 128, M::SMEM_BYTES, st>>>(fp.map_spec, khat == fp.k_ptr ? fp.map_k : fp.map_kex, g, specB,
+                                                        fp.twp);
+    return true;
+}
+
 template <int T, int E, bool PER>
 bool launch_mid3(const FastPlan& fp, const Geom& g, cudaStream_t st, const ColTile& ct, float2* specB,
                  const float* khat)
 {
+    if constexpr (T * E == 128) {
+        // whole-array tiles only: the tensor maps describe specB and K-hat as laid out in mm_common.cuh
+        if (fp.mid_pipe >= 2 && fp.ok_mid_t && ct.kx0 == 0 && ct.ncol == g.Cx && ct.b_row == (size_t)g.CxS &&
+            (khat == fp.k_ptr || fp.has_kex_map))
+            return launch_mid_t<PER>(fp, g, st, specB, khat);
+    }
     if (fp.mid_pipe) {
         constexpr int L = T * E;
         constexpr int NZ = PER ? L : L / 2;
@@ -431,8 +456,87 @@ inline bool fast_plan_init(FastPlan& fp, const Geom& g, std::string* err)
     return true;
 }
 
+// ---- TMA tensor maps (cuTensorMapEncodeTiled, fetched through the runtime: libcuda is not linked) ----
+typedef CUresult (*mm_encode_tiled_fn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                       const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                       CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+inline mm_encode_tiled_fn tensor_map_encoder()
+{
+    static mm_encode_tiled_fn fn = nullptr;
+    if (!fn) {
+        void* p = nullptr;
+        cudaDriverEntryPointQueryResult qr;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &qr) == cudaSuccess &&
+            qr == cudaDriverEntryPointSuccess)
+            fn = reinterpret_cast<mm_encode_tiled_fn>(p);
+        else
+            cudaGetLastError();
+    }
+    return fn;
+}
+
+// 4D float32 map: dims[0] is the contiguous one; stride_bytes[i] = byte stride of dims[i + 1]; out-of-range reads give 0
+inline bool make_map4(CUtensorMap* m, const void* base, const cuuint64_t dims[4], const cuuint64_t stride_bytes[3],
+                      const cuuint32_t box[4])
+{
+    mm_encode_tiled_fn enc = tensor_map_encoder();
+    if (!enc) return false;
+    const cuuint32_t es[4] = { 1, 1, 1, 1 };
+    return enc(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, const_cast<void*>(base), dims, stride_bytes, box, es,
+               CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+               CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
+// K-hat octant [6][Cz][Cy][CxK] seen as (kx, ky, kz >> 1, component, kz & 1): a box of all kz lands in shared
+// memory as [parity][component][kz >> 1][16].  Row kz = Cz (parity 1 of the last pair when Cz is odd) is
+// addressed but never used: the K-hat allocations carry one spare plane (mm_api.cu).
+inline bool khat_map(CUtensorMap* m, const Geom& g, const float* khat)
+{
+    mm_encode_tiled_fn enc = tensor_map_encoder();
+    if (!enc) return false;
+    const cuuint64_t row = (cuuint64_t)g.CxK * 4, plane = row * g.Cy;
+    const cuuint32_t ch = (cuuint32_t)(g.Cz / 2 + 1);
+    const cuuint64_t dims[5] = { (cuuint64_t)g.CxK, (cuuint64_t)g.Cy, ch, 6, 2 };
+    const cuuint64_t sb[4] = { row, 2 * plane, plane * g.Cz, plane };
+    const cuuint32_t box[5] = { 16, 1, ch, 6, 2 };
+    const cuuint32_t es[5] = { 1, 1, 1, 1, 1 };
+    return enc(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 5, const_cast<float*>(khat), dims, sb, box, es,
+               CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+               CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
+// called by mm_demag_init once specB and K-hat exist; failure only switches pk::k_mid_t off
+inline void fast_plan_maps(FastPlan& fp, const Geom& g, const float2* specB, const float* khat)
+{
+    fp.ok_mid_t = false;
+    fp.has_kex_map = false;
+    fp.k_ptr = khat;
+    if (!(fp.ok_mid3 && g.Pz == 128 && specB && khat)) return;
+    const cuuint64_t dims[4] = { (cuuint64_t)2 * g.CxS, (cuuint64_t)g.Py, (cuuint64_t)g.Nz, 3 };
+    const cuuint64_t sb[3] = { (cuuint64_t)g.CxS * 8, (cuuint64_t)g.CxS * g.Py * 8, (cuuint64_t)g.CxS * g.Py * g.Nz * 8 };
+    const cuuint32_t box[4] = { 32, 1, (cuuint32_t)g.Nz, 3 };
+    if (!make_map4(&fp.map_spec, specB, dims, sb, box) || !khat_map(&fp.map_k, g, khat)) return;
+    std::vector<float4> tw(64);
+    for (int a = 0; a < 8; ++a)
+        for (int b = 0; b < 8; ++b) {
+            const long double w = 2.0L * 3.14159265358979323846264338327950288L / 128.0L;
+            const long double p0 = w * (a * 2 * b), p1 = w * (a * (2 * b + 1));
+            tw[a * 8 + b] = make_float4((float)cosl(p0), (float)cosl(p1), (float)sinl(p0), (float)sinl(p1));
+        }
+    if (cudaMalloc(&fp.twp, tw.size() * sizeof(float4)) != cudaSuccess ||
+        cudaMemcpy(fp.twp, tw.data(), tw.size() * sizeof(float4), cudaMemcpyHostToDevice) != cudaSuccess) {
+        cudaGetLastError();
+        return;
+    }
+    fp.ok_mid_t = true;
+}
+
 inline void fast_plan_destroy(FastPlan& fp)
 {
+    cudaFree(fp.twp);
+    fp.twp = nullptr;
+    fp.ok_mid_t = false;
     for (int a = 0; a < 3; ++a) { cudaFree(fp.tw[a]); fp.tw[a] = nullptr; }
     cudaFree(fp.twx);
     fp.twx = nullptr;

@@ -411,7 +411,11 @@ mm_status refresh_khat_ex(mm_ctx* c)
     if (!(c->has_mat && c->has_demag && c->mat.exchange_in_kernel && c->mat.demag)) return MM_OK;
     const Geom& g = c->g;
     const size_t nK = (size_t)6 * g.Cz * g.Cy * g.CxK;
-    if (!c->khat_ex) CUDA_TRY(c, cudaMalloc(&c->khat_ex, nK * sizeof(float)));
+    if (!c->khat_ex) {
+        CUDA_TRY(c, cudaMalloc(&c->khat_ex, (nK + (size_t)g.Cy * g.CxK) * sizeof(float)));
+        CUDA_TRY(c, cudaMemsetAsync(c->khat_ex + nK, 0, (size_t)g.Cy * g.CxK * sizeof(float), c->stream));
+        c->fp.has_kex_map = c->fp.ok_mid_t && khat_map(&c->fp.map_kex, g, c->khat_ex);
+    }
     const double Ms = c->mat.Ms;
     const int ext[3] = { g.Nx, g.Ny, g.Nz };
     float w[3];
@@ -656,7 +660,7 @@ mm_status mm_create(mm_ctx** out, const int grid[3], const double cellsize[3], c
         if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&c->fp.nsm, cudaDevAttrMultiProcessorCount, dev);
         if (c->fp.nsm < 1) c->fp.nsm = 1;
     }
-    c->fp.x_pipe = 1; c->fp.mid_pipe = 1; c->fp.chunk_w = 0; c->fp.nstream = 3;     // mm_set_option defaults
+    c->fp.x_pipe = 1; c->fp.mid_pipe = 2; c->fp.chunk_w = 0; c->fp.nstream = 3;     // mm_set_option defaults
     *out = c;
     return MM_OK;
 }
@@ -726,8 +730,9 @@ static mm_status demag_init_impl(mm_ctx* c)
     const int rc = mmh::build_khat(c->cell, grid, c->pbc, kh.data(), &err);
     if (rc != 0) return fail(c, (mm_status)rc, err);
     const size_t nrow = (size_t)6 * g.Cz * g.Cy;         // device rows are padded to CxK floats (zeros)
-    CUDA_TRY(c, cudaMalloc(&c->khat, nrow * g.CxK * sizeof(float)));
-    CUDA_TRY(c, cudaMemset(c->khat, 0, nrow * g.CxK * sizeof(float)));
+    // one spare kz plane at the end: the even / odd kz view of the TMA map addresses row kz = Cz (never used)
+    CUDA_TRY(c, cudaMalloc(&c->khat, (nrow + g.Cy) * g.CxK * sizeof(float)));
+    CUDA_TRY(c, cudaMemset(c->khat, 0, (nrow + g.Cy) * g.CxK * sizeof(float)));
     CUDA_TRY(c, cudaMemcpy2D(c->khat, g.CxK * sizeof(float), kh.data(), g.Cx * sizeof(float), g.Cx * sizeof(float),
                              nrow, cudaMemcpyHostToDevice));
     const size_t nA = (size_t)3 * g.Nz * g.Ny * g.CxS;
@@ -770,6 +775,7 @@ static mm_status demag_init_impl(mm_ctx* c)
     if ((s = set_smem(c, k_gen_inv_x)) != MM_OK) return s;
     std::string ferr;
     if (!fast_plan_init(c->fp, g, &ferr)) return fail(c, MM_ECUDA, ferr);
+    fast_plan_maps(c->fp, g, c->specB, c->khat);
     c->has_demag = true;
     return refresh_khat_ex(c);
 }

@@ -262,6 +262,7 @@ FAST_GRIDS = [
     ((768, 24, 2), (3e-9, 3e-9, 3e-9), (0, 0, 0)),      # x = 1536 through the half-length real transform
     ((1024, 16, 2), (3e-9, 3e-9, 3e-9), (0, 0, 0)),     # x = 2048, same
     ((1536, 8, 1), (3e-9, 3e-9, 3e-9), (1, 0, 0)),      # x = 1536 periodic (no padding)
+    ((32, 40, 128), (3e-9, 3e-9, 3e-9), (0, 0, 1)),     # periodic z of length 128 (no padding), ragged kx tile
 ]
 
 
