@@ -361,6 +361,7 @@ def main():
                     help="the paper's variant (PAPER.md:85): exchange stencil inside the convolution kernel")
     ap.add_argument("--cufft", action="store_true", help="bench-only comparison with the FFT library (torch.fft)")
     ap.add_argument("--sweep", action="store_true", help="Euler-step time on N^2 / N^3 grids (Table 1 shape)")
+    ap.add_argument("--opt", action="append", default=[], help="mm_set_option KEY=VALUE (may repeat)")
     ap.add_argument("--dry", action="store_true", help="multi-process plumbing only, no GPU (CPU test hook)")
     args = ap.parse_args()
     if args.impl == "reference":
@@ -395,7 +396,8 @@ def main():
     N = wl.grid[0] * wl.grid[1] * wl.grid[2]
     m0 = torch.from_numpy(wlm.initial_m(wl))
     t0 = time.perf_counter()
-    sim = mm.Sim(wl.grid, wl.cell, wl.pbc, wl.mat)
+    opts = {kv.split('=')[0]: int(kv.split('=')[1]) for kv in args.opt}
+    sim = mm.Sim(wl.grid, wl.cell, wl.pbc, wl.mat, options=opts)
     setup_s = time.perf_counter() - t0
     if args.generic:
         sim.set_fast_path(0)

@@ -16,6 +16,7 @@ struct FastPlan {
     int mid_pipe;                        // last-axis pass: persistent pipelined kernel (option "mid_pipe")
     // last-axis pass through TMA tiles and sibling-packed codelets (pk::k_mid_t; mid_pipe >= 2, Pz = 128)
     bool ok_mid_t, has_kex_map;
+    int mid_cols;                        // kx columns per work item of pk::k_mid_t
     CUtensorMap map_spec, map_k, map_kex;  // specB [3][Nz][Py][2 CxS] floats; K-hat / K-hat + exchange [6][Cz][Cy][CxK]
     const float* k_ptr;                  // the K-hat array map_k describes (map_kex: any other)
     float4* twp;                         // pk::k_mid_t twiddles
@@ -185,17 +186,17 @@ bool launch_y(const FastPlan& fp, const Geom& g, cudaStream_t st, const ColTile&
     return true;
 }
 
-template <bool PER>
+template <bool PER, int C>
 bool launch_mid_t(const FastPlan& fp, const Geom& g, cudaStream_t st, float2* specB, const float* khat)
 {
-    using M = pk::MidT<PER>;
+    using M = pk::MidT<PER, C>;
     static bool once[MM_MAX_DEV] = {};
-    if (!ensure_smem_dev(pk::k_mid_t<PER>, M::SMEM_BYTES, once)) return false;
-    const int nitem = ((g.Cx + 15) / 16) * (g.Py / 2 + 1);
-    const int per_sm = PER ? 2 : 3;
+    if (!ensure_smem_dev(pk::k_mid_t<PER, C>, M::SMEM_BYTES, once)) return false;
+    const int nitem = ((g.Cx + C - 1) / C) * (g.Py / 2 + 1);
+    const int per_sm = (PER ? 2 : 3) * (16 / C);
     const int grid = nitem < fp.nsm * per_sm ? nitem : fp.nsm * per_sm;
-    pk::k_mid_t<PER><<<grid, 128, M::SMEM_BYTES, st>>>(fp.map_spec, khat == fp.k_ptr ? fp.map_k : fp.map_kex, g, specB,
-                                                        fp.twp);
+    pk::k_mid_t<PER, C><<<grid, 8 * C, M::SMEM_BYTES, st>>>(fp.map_spec, khat == fp.k_ptr ? fp.map_k : fp.map_kex, g,
+                                                             specB, fp.twp);
     return true;
 }
 
@@ -207,7 +208,7 @@ bool launch_mid3(const FastPlan& fp, const Geom& g, cudaStream_t st, const ColTi
         // whole-array tiles only: the tensor maps describe specB and K-hat as laid out in mm_common.cuh
         if (fp.mid_pipe >= 2 && fp.ok_mid_t && ct.kx0 == 0 && ct.ncol == g.Cx && ct.b_row == (size_t)g.CxS &&
             (khat == fp.k_ptr || fp.has_kex_map))
-            return launch_mid_t<PER>(fp, g, st, specB, khat);
+            return launch_mid_t<PER, 16>(fp, g, st, specB, khat);
     }
     if (fp.mid_pipe) {
         constexpr int L = T * E;
@@ -491,7 +492,7 @@ inline bool make_map4(CUtensorMap* m, const void* base, const cuuint64_t dims[4]
 // K-hat octant [6][Cz][Cy][CxK] seen as (kx, ky, kz >> 1, component, kz & 1): a box of all kz lands in shared
 // memory as [parity][component][kz >> 1][16].  Row kz = Cz (parity 1 of the last pair when Cz is odd) is
 // addressed but never used: the K-hat allocations carry one spare plane (mm_api.cu).
-inline bool khat_map(CUtensorMap* m, const Geom& g, const float* khat)
+inline bool khat_map(CUtensorMap* m, const Geom& g, const float* khat, int cols)
 {
     mm_encode_tiled_fn enc = tensor_map_encoder();
     if (!enc) return false;
@@ -499,7 +500,7 @@ inline bool khat_map(CUtensorMap* m, const Geom& g, const float* khat)
     const cuuint32_t ch = (cuuint32_t)(g.Cz / 2 + 1);
     const cuuint64_t dims[5] = { (cuuint64_t)g.CxK, (cuuint64_t)g.Cy, ch, 6, 2 };
     const cuuint64_t sb[4] = { row, 2 * plane, plane * g.Cz, plane };
-    const cuuint32_t box[5] = { 16, 1, ch, 6, 2 };
+    const cuuint32_t box[5] = { (cuuint32_t)cols, 1, ch, 6, 2 };
     const cuuint32_t es[5] = { 1, 1, 1, 1, 1 };
     return enc(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 5, const_cast<float*>(khat), dims, sb, box, es,
                CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
@@ -515,8 +516,9 @@ inline void fast_plan_maps(FastPlan& fp, const Geom& g, const float2* specB, con
     if (!(fp.ok_mid3 && g.Pz == 128 && specB && khat)) return;
     const cuuint64_t dims[4] = { (cuuint64_t)2 * g.CxS, (cuuint64_t)g.Py, (cuuint64_t)g.Nz, 3 };
     const cuuint64_t sb[3] = { (cuuint64_t)g.CxS * 8, (cuuint64_t)g.CxS * g.Py * 8, (cuuint64_t)g.CxS * g.Py * g.Nz * 8 };
-    const cuuint32_t box[4] = { 32, 1, (cuuint32_t)g.Nz, 3 };
-    if (!make_map4(&fp.map_spec, specB, dims, sb, box) || !khat_map(&fp.map_k, g, khat)) return;
+    fp.mid_cols = 16;       // 8-column items (6 blocks per SM) were measured: 0.84 ms against 0.49 ms
+    const cuuint32_t box[4] = { (cuuint32_t)(2 * fp.mid_cols), 1, (cuuint32_t)g.Nz, 3 };
+    if (!make_map4(&fp.map_spec, specB, dims, sb, box) || !khat_map(&fp.map_k, g, khat, fp.mid_cols)) return;
     std::vector<float4> tw(64);
     for (int a = 0; a < 8; ++a)
         for (int b = 0; b < 8; ++b) {

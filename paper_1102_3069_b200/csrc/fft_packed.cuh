@@ -165,32 +165,34 @@ __device__ __forceinline__ void tma_prefetch_desc(const CUtensorMap* map)
 // ---------------------------------------------------------------------------------------------
 extern __shared__ __align__(1024) unsigned char pk_smem[];
 
-template <bool PER>
+template <bool PER, int C>
 struct MidT {
     static constexpr int T = 8, E = 16, L = 128;
     static constexpr int NZ = PER ? L : L / 2;
     static constexpr int CZ = L / 2 + 1;
     static constexpr int NIO = PER ? E : E / 2;
-    static constexpr unsigned XB_BYTES = 8 * 8 * 16 * 16;
-    static constexpr unsigned IB_BYTES = 3 * NZ * 16 * 8;
+    static constexpr int RS = 8 * C + (C == 8 ? 8 : 0);   // exchange row stride (float2): rows t, t + 1 on different bank halves
+    static constexpr int XP = 8 * RS;                     // float2 per exchange plane (re pairs | im pairs)
+    static constexpr unsigned XB_BYTES = 2 * XP * 8;
+    static constexpr unsigned IB_BYTES = 3 * NZ * C * 8;
     static constexpr int CH = CZ / 2 + 1;          // rows of one kz-parity half of the K^ tile
-    static constexpr unsigned KB_BYTES = 2 * 6 * CH * 16 * 4;
+    static constexpr unsigned KB_BYTES = 2 * 6 * CH * C * 4;
     static constexpr unsigned SMEM_BYTES = XB_BYTES + IB_BYTES + KB_BYTES + 64;
 };
 
-template <bool PER>
-__global__ void __launch_bounds__(128, PER ? 2 : 3)
+template <bool PER, int C>
+__global__ void __launch_bounds__(8 * C, (PER ? 2 : 3) * (16 / C))
 k_mid_t(const __grid_constant__ CUtensorMap map_s, const __grid_constant__ CUtensorMap map_k, Geom g,
         float2* __restrict__ spec, const float4* __restrict__ twp)
 {
-    using M = MidT<PER>;
+    using M = MidT<PER, C>;
     constexpr int NZ = M::NZ, CH = M::CH, NIO = M::NIO, L = M::L;
     float2* xb = reinterpret_cast<float2*>(pk_smem);         // exchange tile: plane of re pairs, plane of im pairs
     const float2* ib = reinterpret_cast<const float2*>(pk_smem + M::XB_BYTES);
     const float* kb = reinterpret_cast<const float*>(pk_smem + M::XB_BYTES + M::IB_BYTES);
     unsigned long long* bar = reinterpret_cast<unsigned long long*>(pk_smem + M::XB_BYTES + M::IB_BYTES + M::KB_BYTES);
-    const int tid = threadIdx.x, c = tid & 15, t = tid >> 4;
-    const int ntx = (g.Cx + 15) >> 4;
+    const int tid = threadIdx.x, c = tid % C, t = tid / C;
+    const int ntx = (g.Cx + C - 1) / C;
     const int nitem = ntx * (g.Py / 2 + 1);
     const size_t rstride = (size_t)g.Py * g.CxS, cstride = (size_t)g.Nz * rstride, step8 = 8 * rstride;
 
@@ -204,23 +206,23 @@ k_mid_t(const __grid_constant__ CUtensorMap map_s, const __grid_constant__ CUten
     __syncthreads();
     auto issue_in = [&](int bx, int other) {
         mbar_expect_tx(bar, M::IB_BYTES);
-        tma_load_4d(const_cast<float2*>(ib), &map_s, bar, 32 * bx, other, 0, 0);
+        tma_load_4d(const_cast<float2*>(ib), &map_s, bar, 2 * C * bx, other, 0, 0);
     };
     auto issue_k = [&](int bx, int p) {
         mbar_expect_tx(bar + 1, M::KB_BYTES);
-        tma_load_5d(const_cast<float*>(kb), &map_k, bar + 1, 16 * bx, p, 0, 0, 0);
+        tma_load_5d(const_cast<float*>(kb), &map_k, bar + 1, C * bx, p, 0, 0, 0);
     };
     int q = blockIdx.x;
     if (tid == 0 && q < nitem) { issue_k(q % ntx, q / ntx); issue_in(q % ntx, q / ntx); }
     unsigned par_in = 0, par_k = 0;
     // per-thread bases of the exchange tile (writer row t / reader column t) and of the K^ tile
-    constexpr int XP = 8 * 8 * 16;               // float2 per plane
-    float2* xw = xb + (t * 8) * 16 + c;          // + k * 16      : entry (row t, column k); + XP: im pair
-    float2* xr = xb + t * 16 + c;                // + n * 8 * 16  : entry (row n, column t)
+    constexpr int XP = M::XP, RS = M::RS;
+    float2* xw = xb + t * RS + c;                // + k * C   : entry (row t, column k); + XP: im pair
+    float2* xr = xb + t * C + c;                 // + n * RS  : entry (row n, column t)
     // K^ tile [parity of kz][component][kz >> 1][16]: a warp's two thread rows t, t + 1 then read rows 64 bytes
     // apart (no bank conflict); direct rows kz = 2t + 16 k1 (+1), mirrored rows 128 - kz
-    const float* kd = kb + c + 16 * t;
-    const float* km = kb + c - 16 * t;
+    const float* kd = kb + c + C * t;
+    const float* km = kb + c - C * t;
     const float4* twf = twp + t * 8;             // forward: row t
     const float4* twi = twp + t;                 // inverse: column t (stride 8)
 
@@ -229,7 +231,7 @@ k_mid_t(const __grid_constant__ CUtensorMap map_s, const __grid_constant__ CUten
         const int mir = (g.Py - p) % g.Py;
         const int nh = mir == p ? 1 : 2;
         const int qn = q + gridDim.x;
-        const int col = bx * 16 + c;
+        const int col = bx * C + c;
         const bool valid = col < g.Cx;
         for (int h = 0; h < nh; ++h) {
             const int other = h ? mir : p;
@@ -241,16 +243,17 @@ k_mid_t(const __grid_constant__ CUtensorMap map_s, const __grid_constant__ CUten
 #pragma unroll
             for (int comp = 0; comp < 3; ++comp)
 #pragma unroll
-                for (int j = 0; j < NIO; ++j) x[comp][j] = ib[(comp * NZ + t + 8 * j) * 16 + c];
+                for (int j = 0; j < NIO; ++j) x[comp][j] = ib[(comp * NZ + t + 8 * j) * C + c];
             __syncthreads();                     // the spectrum tile is in registers: refill it
             if (tid == 0) {
                 if (h + 1 < nh) issue_in(bx, mir);
                 else if (qn < nitem) issue_in(qn % ntx, qn / ntx);
             }
             // ---------------- forward ----------------
-#pragma unroll
-            for (int comp = 0; comp < 3; ++comp) {
-                P2 A[8];
+            // Software-pipelined over the components: the read-back of component c is issued, then the first
+            // register FFT of component c + 1 runs while it lands, and the second register FFT of component c
+            // runs after the next exchange write -- shared-memory and FP phases of one warp interleave.
+            auto fwd_first = [&](int comp, P2 (&A)[8]) {
 #pragma unroll
                 for (int n = 0; n < 8; ++n) {
                     float2 a, d;
@@ -270,21 +273,35 @@ k_mid_t(const __grid_constant__ CUtensorMap map_s, const __grid_constant__ CUten
                 }
                 fft8<-1>(A);                     // A[k] lanes: Y[2k], Y[2k+1]
 #pragma unroll
-                for (int k = 1; k < 8; ++k) A[k] = ptwiddle<false>(A[k], __ldg(twf + k));
-                {   // k = 0: lane 0 has angle 0
-                    const float4 w = __ldg(twf);
-                    A[0] = ptwiddle<false>(A[0], w);
-                }
-                if (comp) __syncthreads();       // the previous component's read-back is done
+                for (int k = 0; k < 8; ++k) A[k] = ptwiddle<false>(A[k], __ldg(twf + k));
+            };
+            auto put_rows = [&](const P2 (&A)[8]) {      // entry (row t, column k)
 #pragma unroll
-                for (int k = 0; k < 8; ++k) { xw[k * 16] = A[k].re; xw[XP + k * 16] = A[k].im; }
+                for (int k = 0; k < 8; ++k) { xw[k * C] = A[k].re; xw[XP + k * C] = A[k].im; }
+            };
+            auto get_cols = [&](P2 (&B)[8]) {            // entry (row n, column t)
+#pragma unroll
+                for (int n = 0; n < 8; ++n) { B[n].re = xr[n * RS]; B[n].im = xr[XP + n * RS]; }
+            };
+            {
+                P2 A[8];
+                fwd_first(0, A);
+                put_rows(A);
                 __syncthreads();
-#pragma unroll
-                for (int n = 0; n < 8; ++n) {
-                    V[comp][n].re = xr[n * 128];
-                    V[comp][n].im = xr[XP + n * 128];
-                }
-                fft8<-1>(V[comp]);               // V[comp][k1] lanes: kz = 2t + 16 k1, 2t + 1 + 16 k1
+                get_cols(V[0]);
+                fwd_first(1, A);
+                __syncthreads();                 // component 0 has been read back by every thread
+                put_rows(A);
+                fft8<-1>(V[0]);                  // V[comp][k1] lanes: kz = 2t + 16 k1, 2t + 1 + 16 k1
+                __syncthreads();
+                get_cols(V[1]);
+                fwd_first(2, A);
+                __syncthreads();
+                put_rows(A);
+                fft8<-1>(V[1]);
+                __syncthreads();
+                get_cols(V[2]);
+                fft8<-1>(V[2]);
             }
             // ---------------- multiply ----------------
             if (h == 0) { mbar_wait(bar + 1, par_k); par_k ^= 1u; }
@@ -296,11 +313,11 @@ k_mid_t(const __grid_constant__ CUtensorMap map_s, const __grid_constant__ CUten
                     if (k1 < 4) {
 #pragma unroll
                         for (int i = 0; i < 6; ++i)
-                            kk[i] = make_float2(kd[(i * CH + 8 * k1) * 16], kd[((6 + i) * CH + 8 * k1) * 16]);
+                            kk[i] = make_float2(kd[(i * CH + 8 * k1) * C], kd[((6 + i) * CH + 8 * k1) * C]);
                     } else {
 #pragma unroll
                         for (int i = 0; i < 6; ++i)
-                            kk[i] = make_float2(km[(i * CH + L / 2 - 8 * k1) * 16], km[((6 + i) * CH + L / 2 - 1 - 8 * k1) * 16]);
+                            kk[i] = make_float2(km[(i * CH + L / 2 - 8 * k1) * C], km[((6 + i) * CH + L / 2 - 1 - 8 * k1) * C]);
                     }
                     float2 kxy = mul2(kk[3], so2), kxz = kk[4], kyz = mul2(kk[5], so2);
                     if (k1 >= 4) {
@@ -323,23 +340,23 @@ k_mid_t(const __grid_constant__ CUtensorMap map_s, const __grid_constant__ CUten
             // ---------------- inverse ----------------
             // rows t, t + 8, ... of this column: pointer increments instead of 64-bit multiplies per store
             float2* __restrict__ op = spec + (size_t)other * g.CxS + col + (size_t)t * rstride;
-#pragma unroll
-            for (int comp = 0; comp < 3; ++comp) {
+            auto inv_first = [&](int comp) {
                 fft8<1>(V[comp]);                // V[comp][n2] lanes: k2 = 2t, 2t + 1
 #pragma unroll
                 for (int n = 0; n < 8; ++n) V[comp][n] = ptwiddle<true>(V[comp][n], __ldg(twi + n * 8));
-                if (comp) __syncthreads();
+            };
+            auto put_cols = [&](const P2 (&B)[8]) {
 #pragma unroll
-                for (int n = 0; n < 8; ++n) { xr[n * 128] = V[comp][n].re; xr[XP + n * 128] = V[comp][n].im; }
-                __syncthreads();
-                P2 R[8];
+                for (int n = 0; n < 8; ++n) { xr[n * RS] = B[n].re; xr[XP + n * RS] = B[n].im; }
+            };
+            auto get_rows = [&](P2 (&R)[8]) {
 #pragma unroll
-                for (int k = 0; k < 8; ++k) {
-                    R[k].re = xw[k * 16];
-                    R[k].im = xw[XP + k * 16];
-                }
+                for (int k = 0; k < 8; ++k) { R[k].re = xw[k * C]; R[k].im = xw[XP + k * C]; }
+            };
+            auto inv_last = [&](P2 (&R)[8], int comp) {
                 fft8<1>(R);                      // R[n1] lanes: E[n1] (even k2), O[n1] (odd k2)
                 // x[n1] = E + w O, x[n1 + 8] = E - w O, w = exp(+2 pi i n1 / 16); row = t + 8 n1
+                float2 o[NIO];
 #pragma unroll
                 for (int n = 0; n < 8; ++n) {
                     const float er = R[n].re.x, ei = R[n].im.x, pr = R[n].re.y, pi = R[n].im.y;
@@ -351,13 +368,34 @@ k_mid_t(const __grid_constant__ CUtensorMap map_s, const __grid_constant__ CUten
                         wr = fmaf(-pi, sn, pr * cs);
                         wi = fmaf(pr, sn, pi * cs);
                     }
-                    if (valid) {
-                        *op = make_float2(er + wr, ei + wi);
-                        if (PER) op[step8 * 8] = make_float2(er - wr, ei - wi);
-                    }
-                    op += step8;
+                    o[n] = make_float2(er + wr, ei + wi);
+                    if (PER) o[n + 8] = make_float2(er - wr, ei - wi);
                 }
-                op += cstride - 8 * step8;
+                if (valid) {
+                    float2* __restrict__ oc = op + comp * cstride;
+#pragma unroll
+                    for (int n = 0; n < NIO; ++n) oc[n * step8] = o[n];
+                }
+            };
+            {
+                P2 R[8];
+                inv_first(0);
+                put_cols(V[0]);
+                __syncthreads();
+                get_rows(R);
+                inv_first(1);
+                __syncthreads();
+                put_cols(V[1]);
+                inv_last(R, 0);
+                __syncthreads();
+                get_rows(R);
+                inv_first(2);
+                __syncthreads();
+                put_cols(V[2]);
+                inv_last(R, 1);
+                __syncthreads();
+                get_rows(R);
+                inv_last(R, 2);
             }
         }
     }

@@ -414,7 +414,7 @@ mm_status refresh_khat_ex(mm_ctx* c)
     if (!c->khat_ex) {
         CUDA_TRY(c, cudaMalloc(&c->khat_ex, (nK + (size_t)g.Cy * g.CxK) * sizeof(float)));
         CUDA_TRY(c, cudaMemsetAsync(c->khat_ex + nK, 0, (size_t)g.Cy * g.CxK * sizeof(float), c->stream));
-        c->fp.has_kex_map = c->fp.ok_mid_t && khat_map(&c->fp.map_kex, g, c->khat_ex);
+        c->fp.has_kex_map = c->fp.ok_mid_t && khat_map(&c->fp.map_kex, g, c->khat_ex, c->fp.mid_cols);
     }
     const double Ms = c->mat.Ms;
     const int ext[3] = { g.Nx, g.Ny, g.Nz };
@@ -660,7 +660,7 @@ mm_status mm_create(mm_ctx** out, const int grid[3], const double cellsize[3], c
         if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&c->fp.nsm, cudaDevAttrMultiProcessorCount, dev);
         if (c->fp.nsm < 1) c->fp.nsm = 1;
     }
-    c->fp.x_pipe = 1; c->fp.mid_pipe = 2; c->fp.chunk_w = 0; c->fp.nstream = 3;     // mm_set_option defaults
+    c->fp.x_pipe = 1; c->fp.mid_pipe = 2; c->fp.mid_cols = 16; c->fp.chunk_w = 0; c->fp.nstream = 3;     // mm_set_option defaults
     *out = c;
     return MM_OK;
 }
