@@ -10,7 +10,7 @@ import sys
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
-LIB = os.path.join(HERE, "libmm_b200.so")
+LIB = os.environ.get("MM_B200_LIB") or os.path.join(HERE, "libmm_b200.so")
 SOURCES = ["mm_api.cu", "demag_host.cpp"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "-split-compile", "0",
               "-Xcompiler", "-fPIC,-fopenmp,-O2", "-shared", "-lgomp"]

@@ -12,7 +12,7 @@ import os
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-_LIBPATH = os.path.join(_HERE, "libmm_b200.so")
+_LIBPATH = os.environ.get("MM_B200_LIB") or os.path.join(_HERE, "libmm_b200.so")      # override: A/B builds
 
 MM_OK = 0
 STATUS = {0: "MM_OK", 1: "MM_EINVAL", 2: "MM_ENOMEM", 3: "MM_ECUDA", 4: "MM_ESTATE",
