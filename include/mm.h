@@ -268,6 +268,64 @@ mm_status mm_set_fast_path(mm_ctx* ctx, int enable);
 mm_status mm_copy_bandwidth(mm_ctx* ctx, const void* src_dev, void* dst_dev, size_t nbytes,
                             int reps, double* sec_out);
 
+
+/* ---- multi-GPU slab decomposition ("multi-GPU ... efficient communication") ----
+ * One process per GPU.  Rank r owns the planes z0 <= z < z1 of every field (all x, y) and, for the transform
+ * along z, the columns kx0 <= kx < kx1 of the half spectrum (all ky, all z).  One evaluation is
+ *   mm_dist_forward   a1, a2 on the slab; the y pass writes straight into the exchange layout
+ *   all-to-all #1     slab buffer -> pencil buffer   (done by the CALLER: NCCL, or copies in a test)
+ *   mm_dist_mid       a3 on the pencil (full z lines, this rank's K-hat columns)
+ *   all-to-all #2     pencil buffer -> slab buffer
+ *   halo exchange     plane z0 to rank r-1, plane z1-1 to rank r+1 (m only, one plane each way)
+ *   mm_dist_backward  a4, a5 and the per-cell tail a6-a8 on the slab
+ * The library does no communication itself: it exposes the two device buffers and, per (peer, component), the
+ * contiguous segment that travels, so that each all-to-all is a list of contiguous sends and receives with no
+ * pack or unpack kernel.  DESIGN.md section 10 has the layouts and the byte counts. */
+typedef struct {
+    int rank, nranks;
+    int z0, z1;   /* planes owned                                                                  */
+    int kx0, kx1; /* columns of the half spectrum (0 .. Px/2) owned for the z pass; multiples of 16 */
+} mm_slab;
+
+/* mm_slab_partition -- the partition rule, HOST only (no device, no context): planes in contiguous balanced
+ * ranges, columns in contiguous ranges of whole 16-column tiles.  Errors: MM_EINVAL (nranks < 1, rank out of range,
+ * more ranks than planes or than column tiles), MM_EUNSUPPORTED (padded size not 2^a 3^b 5^c 7^d). */
+mm_status mm_slab_partition(const int grid[3], const int pbc[3], int nranks, int rank, mm_slab* out);
+
+/* mm_create_dist -- context of one rank: `grid` is the GLOBAL grid; fields passed to the mm_dist_* calls are the
+ * local slab, float32 [3][z1-z0][Ny][Nx].  Needs a 3D grid whose passes all have size-specialised kernels and
+ * Nx % 4 == 0 (MM_EUNSUPPORTED otherwise).  mm_set_material and mm_demag_init follow as for mm_create
+ * (mm_demag_init builds the whole K-hat octant on the host and uploads this rank's columns). */
+mm_status mm_create_dist(mm_ctx** out, const int grid[3], const double cellsize[3], const int pbc[3],
+                         void* cuda_stream, int rank, int nranks);
+
+/* mm_dist_buffers -- the two exchange buffers (device, float2 elements, owned by the context):
+ *   slab_buf    [peer][3][z1-z0][Py][W(peer)]   W(peer) = kx1(peer) - kx0(peer) rounded up to a multiple of 8
+ *   pencil_buf  [3][Nz][Py][W(rank)]
+ * and their sizes in float2 elements. */
+mm_status mm_dist_buffers(mm_ctx* ctx, void** slab_buf_dev, size_t* slab_elems, void** pencil_buf_dev,
+                          size_t* pencil_elems);
+
+/* mm_dist_segment -- the contiguous segment exchanged with `peer` for component comp (0..2), in float2
+ * elements: all-to-all #1 sends slab_buf[slab_off .. +slab_count) to the peer and receives the peer's planes
+ * into pencil_buf[pencil_off .. +pencil_count); all-to-all #2 is the reverse. */
+mm_status mm_dist_segment(const mm_ctx* ctx, int peer, int comp, size_t* slab_off, size_t* slab_count,
+                          size_t* pencil_off, size_t* pencil_count);
+
+/* mm_slab_segment -- the same bookkeeping without a context, HOST only (the CPU tests drive a two-process
+ * all-to-all over gloo with it). */
+mm_status mm_slab_segment(const int grid[3], const int pbc[3], int nranks, int rank, int peer, int comp,
+                          size_t* slab_off, size_t* slab_count, size_t* pencil_off, size_t* pencil_count);
+
+mm_status mm_dist_forward(mm_ctx* ctx, const float* m_slab_dev);
+mm_status mm_dist_mid(mm_ctx* ctx);
+/* mm_dist_backward -- what = 0: H_ms (A/m), 1: H_eff (A/m), 2: dm/dt (1/s) into out_slab_dev.
+ *   halo_lo_dev / halo_hi_dev   float32 [3][Ny][Nx]: the plane z0-1 / z1 of m from the neighbouring rank (for a
+ *   periodic z axis the ring neighbour); NULL at an open boundary of the global grid.  Ignored for what = 0. */
+mm_status mm_dist_backward(mm_ctx* ctx, const float* m_slab_dev, const float* halo_lo_dev,
+                           const float* halo_hi_dev, float* out_slab_dev, int what, uint64_t step,
+                           double dt_for_thermal);
+
 /* mm_last_error -- message for the last non-OK status of this context ("" if none); for a NULL ctx
  * the message of the last failed mm_create on this thread. */
 const char* mm_last_error(const mm_ctx* ctx);

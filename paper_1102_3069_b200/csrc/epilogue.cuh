@@ -126,7 +126,7 @@ __device__ __forceinline__ float epilogue_finish_v(const EpiParams& p, size_t id
 #pragma unroll
         for (int u = 0; u < V; ++u) {
             float eta[3];
-            thermal_eta(p, (uint64_t)(idx + u), eta);
+            thermal_eta(p, (uint64_t)(idx + u) + p.cell0, eta);
 #pragma unroll
             for (int c = 0; c < 3; ++c) h[c][u] += p.sig_th * eta[c];
         }
@@ -489,14 +489,19 @@ k_epi4(Geom g, const float* __restrict__ hms, EpiParams ep)
         const int zp = z + 1 < g.Nz ? z + 1 : (g.perz ? 0 : z);
         const size_t iym = (size_t)z * plane + (size_t)ym * g.Nx + x, iyp = (size_t)z * plane + (size_t)yp * g.Nx + x;
         const size_t izm = (size_t)zm * plane + (size_t)y * g.Nx + x, izp = (size_t)zp * plane + (size_t)y * g.Nx + x;
+        // slab decomposition: the planes below the first and above the last local plane come from the neighbours
+        const bool lo_h = ep.zlo != nullptr && z == 0, hi_h = ep.zhi != nullptr && z == g.Nz - 1;
+        const float* __restrict__ pzm = lo_h ? ep.zlo + (size_t)y * g.Nx + x : mi + izm;
+        const float* __restrict__ pzp = hi_h ? ep.zhi + (size_t)y * g.Nx + x : mi + izp;
+        const size_t szm = lo_h ? plane : n, szp = hi_h ? plane : n;
 #pragma unroll
         for (int c = 0; c < 3; ++c) {
             float a[4], b[4], d[4], e[4];
             ldv<4>(hms + idx + c * n, h[c]);
             ldv<4>(mi + iym + c * n, a);
             ldv<4>(mi + iyp + c * n, b);
-            ldv<4>(mi + izm + c * n, d);
-            ldv<4>(mi + izp + c * n, e);
+            ldv<4>(pzm + c * szm, d);
+            ldv<4>(pzp + c * szp, e);
 #pragma unroll
             for (int u = 0; u < 4; ++u) {
                 const float mc = m[c][u];

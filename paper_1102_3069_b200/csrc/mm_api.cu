@@ -154,6 +154,14 @@ struct mm_ctx {
     bool k0_valid;
     int k0_method;
     FastPlan fp;
+    // slab decomposition (mm_dist.cuh): g holds the LOCAL planes, gmid the geometry of the z pass on the pencil
+    bool dist;
+    mm_slab slab;
+    std::vector<mm_slab> peers;
+    int gNz;
+    Geom gmid;
+    float2 *slab_buf, *pencil_buf;
+    size_t slab_elems, pencil_elems;
 };
 
 namespace {
@@ -207,7 +215,7 @@ void fill_material(const mm_ctx* c, EpiParams& p, uint64_t step, double dt_therm
     const Geom& g = c->g;
     const double Ms = M.Ms;
     const double g0 = M.gamma0 > 0 ? M.gamma0 : GAMMA0_DEFAULT;
-    const int ext[3] = { g.Nx, g.Ny, g.Nz };
+    const int ext[3] = { g.Nx, g.Ny, c->dist ? c->gNz : g.Nz };     // a slab has z neighbours even with one local plane
     p.demag = M.demag ? 1 : 0;
     const bool ex_in_k = M.exchange_in_kernel && M.demag;      // then the convolution carries the exchange field
     for (int a = 0; a < 3; ++a)
@@ -269,6 +277,7 @@ mm_status set_smem(mm_ctx* c, K kern)
 // else the generic shared-memory kernel; both use the same layouts. ----
 mm_status launch_eval(mm_ctx* c, const EpiParams& ep)
 {
+    if (c->dist) return fail(c, MM_ESTATE, "a slab context evaluates through mm_dist_forward / _mid / _backward");
     const Geom& g = c->g;
     cudaStream_t st = c->stream;
     const FastPlan& fp = c->fp;
@@ -429,6 +438,8 @@ mm_status refresh_khat_ex(mm_ctx* c)
 mm_status check_ready(mm_ctx* c)
 {
     if (!c) return MM_EINVAL;
+    if (c->dist && (c->mat.exchange_in_kernel || c->mat.geometry))
+        return fail(c, MM_EUNSUPPORTED, "slab decomposition: exchange_in_kernel and geometry are not supported");
     if (!c->has_mat) return fail(c, MM_ESTATE, "mm_set_material has not been called");
     if (!c->has_demag) return fail(c, MM_ESTATE, "mm_demag_init has not been called");
     return MM_OK;
@@ -639,6 +650,7 @@ mm_status mm_create(mm_ctx** out, const int grid[3], const double cellsize[3], c
     c->gstream = nullptr;
     c->gev[0] = c->gev[1] = nullptr;
     c->use_graph = 1;
+    c->dist = false; c->gNz = grid[2]; c->slab_buf = c->pencil_buf = nullptr; c->slab_elems = c->pencil_elems = 0;
     c->gexec = nullptr; c->g_method = -1; c->g_dt = 0.0; c->g_m = nullptr; c->g_epoch = 0; c->g_per = 0;
     c->epoch = 1;
     c->khat = nullptr; c->khat_ex = nullptr; c->specA = c->specB = nullptr;
@@ -693,7 +705,7 @@ static void free_workspaces(mm_ctx* c)
     for (int a = 0; a < 3; ++a) fr(c->tw[a]);
     for (int i = 0; i < 7; ++i) fr(c->kb[i]);
     fr(c->ms[0]); fr(c->ms[1]); fr(c->mtmp); fr(c->mhost); fr(c->hfield);
-    fr(c->maxbits); fr(c->ctl); fr(c->ctl_scratch); fr(c->step_dev);
+    fr(c->maxbits); fr(c->ctl); fr(c->ctl_scratch); fr(c->step_dev); fr(c->slab_buf); fr(c->pencil_buf);
     fast_plan_destroy(c->fp);
 }
 
@@ -718,7 +730,7 @@ mm_status mm_demag_init(mm_ctx* c)
 static mm_status demag_init_impl(mm_ctx* c)
 {
     const Geom& g = c->g;
-    const int grid[3] = { g.Nx, g.Ny, g.Nz };
+    const int grid[3] = { g.Nx, g.Ny, c->dist ? c->gNz : g.Nz };     // the kernel is that of the whole grid
     const size_t nC = (size_t)g.Cx * g.Cy * g.Cz;
     std::vector<float> kh;
     try {
@@ -730,15 +742,28 @@ static mm_status demag_init_impl(mm_ctx* c)
     const int rc = mmh::build_khat(c->cell, grid, c->pbc, kh.data(), &err);
     if (rc != 0) return fail(c, (mm_status)rc, err);
     const size_t nrow = (size_t)6 * g.Cz * g.Cy;         // device rows are padded to CxK floats (zeros)
+    // a rank of a slab decomposition keeps only the columns it transforms along z
+    const int k0 = c->dist ? c->slab.kx0 : 0, kw = c->dist ? c->slab.kx1 - c->slab.kx0 : g.Cx;
+    const size_t kstride = c->dist ? (size_t)c->gmid.CxK : (size_t)g.CxK;
     // one spare kz plane at the end: the even / odd kz view of the TMA map addresses row kz = Cz (never used)
-    CUDA_TRY(c, cudaMalloc(&c->khat, (nrow + g.Cy) * g.CxK * sizeof(float)));
-    CUDA_TRY(c, cudaMemset(c->khat, 0, (nrow + g.Cy) * g.CxK * sizeof(float)));
-    CUDA_TRY(c, cudaMemcpy2D(c->khat, g.CxK * sizeof(float), kh.data(), g.Cx * sizeof(float), g.Cx * sizeof(float),
+    CUDA_TRY(c, cudaMalloc(&c->khat, (nrow + g.Cy) * kstride * sizeof(float)));
+    CUDA_TRY(c, cudaMemset(c->khat, 0, (nrow + g.Cy) * kstride * sizeof(float)));
+    CUDA_TRY(c, cudaMemcpy2D(c->khat, kstride * sizeof(float), kh.data() + k0, g.Cx * sizeof(float), kw * sizeof(float),
                              nrow, cudaMemcpyHostToDevice));
+    if (c->dist) {
+        size_t wsum = 0;
+        for (const mm_slab& q : c->peers) wsum += (size_t)((q.kx1 - q.kx0 + 7) & ~7);
+        c->slab_elems = (size_t)3 * g.Nz * g.Py * wsum;
+        c->pencil_elems = (size_t)3 * c->gNz * g.Py * (size_t)((kw + 7) & ~7);
+        CUDA_TRY(c, cudaMalloc(&c->slab_buf, c->slab_elems * sizeof(float2)));
+        CUDA_TRY(c, cudaMalloc(&c->pencil_buf, c->pencil_elems * sizeof(float2)));
+        CUDA_TRY(c, cudaMemset(c->slab_buf, 0, c->slab_elems * sizeof(float2)));
+        CUDA_TRY(c, cudaMemset(c->pencil_buf, 0, c->pencil_elems * sizeof(float2)));
+    }
     const size_t nA = (size_t)3 * g.Nz * g.Ny * g.CxS;
     CUDA_TRY(c, cudaMalloc(&c->specA, nA * sizeof(float2)));
     CUDA_TRY(c, cudaMemset(c->specA, 0, nA * sizeof(float2)));
-    if (g.Py > 1) {
+    if (g.Py > 1 && !c->dist) {      // (a slab rank's y passes write into / read from slab_buf)
         const size_t nB = (size_t)3 * g.Nz * g.Py * g.CxS;
         CUDA_TRY(c, cudaMalloc(&c->specB, nB * sizeof(float2)));
         CUDA_TRY(c, cudaMemset(c->specB, 0, nB * sizeof(float2)));
@@ -775,7 +800,12 @@ static mm_status demag_init_impl(mm_ctx* c)
     if ((s = set_smem(c, k_gen_inv_x)) != MM_OK) return s;
     std::string ferr;
     if (!fast_plan_init(c->fp, g, &ferr)) return fail(c, MM_ECUDA, ferr);
-    fast_plan_maps(c->fp, g, c->specB, c->khat);
+    if (c->dist) {
+        if (!(c->fp.ok_x && c->fp.ok_y && c->fp.ok_mid3))
+            return fail(c, MM_EUNSUPPORTED, "mm_create_dist needs size-specialised kernels for all three padded lengths");
+    } else {
+        fast_plan_maps(c->fp, g, c->specB, c->khat);
+    }
     c->has_demag = true;
     return refresh_khat_ex(c);
 }
@@ -784,6 +814,7 @@ static mm_status eval_to(mm_ctx* c, const float* m_dev, float* out, int mode, ui
 {
     mm_status s = check_ready(c);
     if (s != MM_OK) return s;
+    if (c->dist) return fail(c, MM_ESTATE, "a slab context evaluates through mm_dist_forward / _mid / _backward");
     if (!m_dev || !out) return fail(c, MM_EINVAL, "NULL device pointer");
     EpiParams ep;
     std::memset(&ep, 0, sizeof(ep));
@@ -1233,6 +1264,7 @@ mm_status mm_get_demag_kernel(mm_ctx* c, int comp, float* host_out, size_t n)
 {
     if (!c || !host_out || comp < 0 || comp > 5) return MM_EINVAL;
     if (!c->has_demag) return fail(c, MM_ESTATE, "mm_demag_init has not been called");
+    if (c->dist) return fail(c, MM_EUNSUPPORTED, "a slab context holds only its own K-hat columns");
     const size_t nC = (size_t)c->g.Cx * c->g.Cy * c->g.Cz;
     if (n < nC) return fail(c, MM_EINVAL, "host_out too small");
     const Geom& g = c->g;
@@ -1354,3 +1386,5 @@ void mm_destroy(mm_ctx* c)
 }
 
 }  // extern "C"
+
+#include "mm_dist.cuh"

@@ -66,6 +66,11 @@ struct EpiParams {
     float e[MM_MAXK];
     const float* ke[MM_MAXK];
     unsigned int* maxbits;   // atomicMax target (bit pattern of a non-negative float)
+    // slab decomposition (mm_dist_*): planes z = -1 and z = Nz of m_in held by the neighbouring ranks, [3][Ny][Nx]
+    // each; NULL: the slab ends at an open boundary of the global grid (or the grid is not split)
+    const float* zlo;
+    const float* zhi;
+    unsigned long long cell0;   // global index of the slab's first cell (thermal counter, reading A6)
     const float* dt_scale;   // device scalar dt gamma0 Ms multiplying a_self, a[], e_self, e[] (NULL: already folded in)
 };
 

@@ -55,6 +55,12 @@ class Material(C.Structure):
         return m
 
 
+class Slab(C.Structure):
+    """mm_slab of include/mm.h."""
+    _fields_ = [("rank", C.c_int), ("nranks", C.c_int), ("z0", C.c_int), ("z1", C.c_int), ("kx0", C.c_int),
+                ("kx1", C.c_int)]
+
+
 _lib = None
 
 
@@ -93,6 +99,15 @@ def lib():
         L.mm_launch_count.restype = C.c_uint64
         L.mm_set_fast_path.argtypes = [vp, C.c_int]
         L.mm_copy_bandwidth.argtypes = [vp, vp, vp, C.c_size_t, C.c_int, d3]
+        sz = C.POINTER(C.c_size_t)
+        L.mm_slab_partition.argtypes = [i3, i3, C.c_int, C.c_int, C.POINTER(Slab)]
+        L.mm_create_dist.argtypes = [C.POINTER(vp), i3, d3, i3, vp, C.c_int, C.c_int]
+        L.mm_dist_buffers.argtypes = [vp, C.POINTER(vp), sz, C.POINTER(vp), sz]
+        L.mm_dist_segment.argtypes = [vp, C.c_int, C.c_int, sz, sz, sz, sz]
+        L.mm_slab_segment.argtypes = [i3, i3, C.c_int, C.c_int, C.c_int, C.c_int, sz, sz, sz, sz]
+        L.mm_dist_forward.argtypes = [vp, vp]
+        L.mm_dist_mid.argtypes = [vp]
+        L.mm_dist_backward.argtypes = [vp, vp, vp, vp, vp, C.c_int, C.c_uint64, C.c_double]
         L.mm_last_error.argtypes = [vp]
         L.mm_last_error.restype = C.c_char_p
         L.mm_destroy.argtypes = [vp]
@@ -118,6 +133,24 @@ def demag_tensor_host(cell, grid, pbc, offsets) -> np.ndarray:
     if st != MM_OK:
         raise MMError(st, "mm_demag_tensor_host")
     return out
+
+
+def slab_partition(grid, pbc, nranks, rank) -> Slab:
+    """mm_slab_partition: planes and spectrum columns of one rank (host only)."""
+    out = Slab()
+    st = lib().mm_slab_partition(_i3(grid), _i3(pbc), int(nranks), int(rank), C.byref(out))
+    if st != MM_OK:
+        raise MMError(st, "mm_slab_partition")
+    return out
+
+
+def slab_segment(grid, pbc, nranks, rank, peer, comp):
+    """mm_slab_segment: (slab_off, slab_count, pencil_off, pencil_count) in complex elements (host only)."""
+    v = [C.c_size_t() for _ in range(4)]
+    st = lib().mm_slab_segment(_i3(grid), _i3(pbc), int(nranks), int(rank), int(peer), int(comp), *[C.byref(x) for x in v])
+    if st != MM_OK:
+        raise MMError(st, "mm_slab_segment")
+    return tuple(int(x.value) for x in v)
 
 
 def demag_khat_host(cell, grid, pbc) -> np.ndarray:
