@@ -297,6 +297,44 @@ def run_sweep(args):
                       "data": "synthetic", "higher_is_better": False, "n_gpus": 1, "sweep": rows}))
 
 
+def run_batch(args):
+    """SURVEY 8(f) row f-3 (a sweep of 200 small simulations): 200 films of 64 x 16 x 1 cells advanced
+    together in one batch context (one launch per pass for all films) against the same 200 films advanced one
+    context at a time (each launch-bound).  RK4, fixed step.  One JSON line."""
+    import numpy as np
+    import torch
+    import paper_1102_3069_b200 as mm
+    from paper_1102_3069_b200 import workloads as wlm
+    torch.cuda.set_device(0)
+    B, grid, nstep = 200, (64, 16, 1), 50
+    wl = wlm.scaled(wlm.config(1), grid)
+    m1 = wlm.initial_m(wl)
+    mb = torch.from_numpy(np.ascontiguousarray(np.repeat(m1, B, axis=1))).cuda()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    simb = mm.Sim(wl.grid, wl.cell, wl.pbc, wl.mat, nfilms=B)
+    simb.steps_fixed(mb, "rk4", 1e-13, nstep)
+    torch.cuda.synchronize(); e0.record()
+    simb.steps_fixed(mb, "rk4", 1e-13, nstep)
+    e1.record(); torch.cuda.synchronize()
+    t_batch = e0.elapsed_time(e1) * 1e-3
+    simb.close()
+    sim1 = mm.Sim(wl.grid, wl.cell, wl.pbc, wl.mat)
+    md = torch.from_numpy(m1).cuda()
+    sim1.steps_fixed(md, "rk4", 1e-13, nstep)
+    nsingle = 20                                   # films advanced one after the other, scaled to B
+    torch.cuda.synchronize(); e0.record()
+    for _ in range(nsingle):
+        sim1.steps_fixed(md, "rk4", 1e-13, nstep)
+    e1.record(); torch.cuda.synchronize()
+    t_single = e0.elapsed_time(e1) * 1e-3 * B / nsingle
+    sim1.close()
+    print(json.dumps({"metric": "RK4 steps of a 64x16x1 film per second, 200 films", "unit": "film-steps/s",
+                      "batch_context": B * nstep / t_batch, "one_context_at_a_time": B * nstep / t_single,
+                      "speedup": t_single / t_batch, "us_per_film_step_batch": t_batch / (B * nstep) * 1e6,
+                      "us_per_film_step_single": t_single / (B * nstep) * 1e6, "dtype": "f32", "data": "synthetic",
+                      "n_gpus": 1, "higher_is_better": True}))
+
+
 def run_cufft_compare(args):
     """the same magnetostatic convolution through the FFT LIBRARY (torch.fft = cuFFT): pad, 3D
     R2C, multiply by the full half-spectrum kernel, C2R, crop.  A bench-only comparison (north_star: cuFFT never
@@ -367,17 +405,20 @@ def main():
     ap.add_argument("--cufft", action="store_true", help="bench-only comparison with the FFT library (torch.fft)")
     ap.add_argument("--sweep", action="store_true", help="Euler-step time on N^2 / N^3 grids (Table 1 shape)")
     ap.add_argument("--opt", action="append", default=[], help="mm_set_option KEY=VALUE (may repeat)")
+    ap.add_argument("--batch", action="store_true", help="200 films of 64x16x1 in one batch context (row f-3)")
     ap.add_argument("--dry", action="store_true", help="multi-process plumbing only, no GPU (CPU test hook)")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
-    if args.gpus > 1 and "WORLD_SIZE" not in os.environ and not (args.sweep or args.cufft):
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ and not (args.sweep or args.cufft or args.batch):
         # run as the driver runs it for N > 1: one rank per GPU under torch.distributed.run
         sys.exit(respawn_under_torchrun(args.gpus, sys.argv[1:]))
     if args.dry:
         return run_dry(args)
     if args.sweep:
         return run_sweep(args)
+    if args.batch:
+        return run_batch(args)
     if args.cufft:
         return run_cufft_compare(args)
 

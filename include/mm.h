@@ -230,6 +230,22 @@ mm_status mm_padded_size(const mm_ctx* ctx, int P_out[3], int C_out[3]);
  * without a context; HOST only, needs no device.  MM_EUNSUPPORTED if a padded size is not 2^a 3^b 5^c 7^d. */
 mm_status mm_padded_size_of(const int grid[3], const int pbc[3], int P_out[3], int C_out[3]);
 
+/* mm_create_batch -- nfilms INDEPENDENT films of the same grid (Nz = 1), cell size, boundary conditions and
+ * material in one context (many small simulations, the shape of the paper's 200-run sweep,
+ * PAPER.md:181, where one small grid is launch-bound).  Every field is float32 [3][nfilms][Ny][Nx]: film b is plane
+ * b.  Each pass is ONE launch over all films (they share K-hat; nothing couples two planes), and every entry point
+ * of a plain context works unchanged: the steppers advance all films with the same dt, the max-norm (error
+ * estimate, step control) is taken over the whole batch, the thermal draw differs from film to film.
+ * Needs padded x and y lengths 32 ... 1024 with a size-specialised kernel and Nx % 4 == 0 (MM_EUNSUPPORTED at
+ * mm_demag_init otherwise). */
+mm_status mm_create_batch(mm_ctx** out, const int grid[3], const double cellsize[3], const int pbc[3],
+                          void* cuda_stream, int nfilms);
+
+/* mm_batch_set_field -- one applied field per film (a hysteresis sweep in one context): B_host[nfilms][3] in
+ * tesla replaces mm_material.Bext; NULL returns to the material's uniform field.  Needs mm_set_material and
+ * mm_demag_init first.  Blocking. */
+mm_status mm_batch_set_field(mm_ctx* ctx, const double* B_host);
+
 /* mm_set_option -- per-context tuning switches (integers; defaults are the measured best on B200):
  *   "graph"          1 (default): mm_steps_fixed replays a captured CUDA graph of one step; 0: plain launches
  *   "x_pipe"         bit 0: forward x pass in its cp.async-pipelined form (default 1); bit 1: inverse x pass too

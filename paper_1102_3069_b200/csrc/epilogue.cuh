@@ -106,6 +106,15 @@ __device__ __forceinline__ float epilogue_finish_v(const EpiParams& p, size_t id
 #pragma unroll
         for (int c = 0; c < 3; ++c) h[c][u] += s * p.u[c] + p.hext[c];
     }
+    if (p.hext_b) {      // one applied field per film of a batch (the V cells lie in one row, hence in one plane)
+        const float* __restrict__ hb = p.hext_b + 3 * (idx / p.plane_cells);
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            const float d = __ldg(hb + c) - p.hext[c];
+#pragma unroll
+            for (int u = 0; u < V; ++u) h[c][u] += d;
+        }
+    }
     // ---- cubic anisotropy (Eq. (5), reading A14): h -= sum_i (dE/da_i) c_i ----
     if (p.cubic) {
 #pragma unroll

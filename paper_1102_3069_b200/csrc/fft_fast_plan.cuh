@@ -30,6 +30,7 @@ namespace ff {
 inline bool split(int L, int* T, int* E)
 {
     switch (L) {
+    case 32: *T = 4; *E = 8; return true;
     case 64: *T = 8; *E = 8; return true;
     case 192: *T = 8; *E = 24; return true;
     case 384: *T = 8; *E = 48; return true;
@@ -57,8 +58,9 @@ k_mul2d(Geom g, float2* __restrict__ spec, const float* __restrict__ khat)
     const float kxx = __ldg(khat + ko), kyy_ = __ldg(khat + ko + nC), kzz = __ldg(khat + ko + 2 * nC);
     const float kxy = sy * __ldg(khat + ko + 3 * nC), kxz = __ldg(khat + ko + 4 * nC);
     const float kyz = sy * __ldg(khat + ko + 5 * nC);
-    const size_t cs = (size_t)g.Py * g.CxS;
-    float2* p = spec + (size_t)ky * g.CxS + kx;
+    // blockIdx.z = plane: a batch of B independent films is B planes of one array (mm_create_batch); Nz = 1 else
+    const size_t cs = (size_t)g.Nz * g.Py * g.CxS;
+    float2* p = spec + ((size_t)blockIdx.z * g.Py + ky) * g.CxS + kx;
     const float2 mx = p[0], my = p[cs], mz = p[2 * cs];
     p[0] = make_float2(kxx * mx.x + kxy * my.x + kxz * mz.x, kxx * mx.y + kxy * my.y + kxz * mz.y);
     p[cs] = make_float2(kxy * mx.x + kyy_ * my.x + kyz * mz.x, kxy * mx.y + kyy_ * my.y + kyz * mz.y);
@@ -237,6 +239,7 @@ bool launch_mid3(const FastPlan& fp, const Geom& g, cudaStream_t st, const ColTi
 
 #define MM_FF_SIZES(L, CALL)                 \
     switch (L) {                              \
+    case 32: { CALL(4, 8); } break;           \
     case 64: { CALL(8, 8); } break;           \
     case 192: { CALL(8, 24); } break;         \
     case 384: { CALL(8, 48); } break;         \
@@ -383,7 +386,7 @@ inline bool fast_yzy_chunked(FastPlan& fp, const Geom& g, cudaStream_t st, float
 inline bool fast_mul2(const FastPlan& fp, const Geom& g, cudaStream_t st, float2* specB, const float* khat)
 {
     if (!fp.ok_mul2) return false;
-    dim3 grid((g.Cx + 255) / 256, g.Py);
+    dim3 grid((g.Cx + 255) / 256, g.Py, g.Nz);
     ff::k_mul2d<<<grid, 256, 0, st>>>(g, specB, khat);
     return true;
 }
@@ -395,7 +398,7 @@ inline bool fast_plan_init(FastPlan& fp, const Geom& g, std::string* err)
     fp.ok_xr = !fp.ok_x && (g.Px == 1536 || g.Px == 2048) && g.Nx % 2 == 0;
     fp.twx = nullptr;
     fp.ok_y = g.Py > 1 && ff::split(g.Py, &T, &E);
-    fp.ok_mid3 = g.Pz > 1 && g.Py > 1 && ff::split(g.Pz, &T, &E) && E <= 16;
+    fp.ok_mid3 = g.Pz >= 64 && g.Py > 1 && ff::split(g.Pz, &T, &E) && E <= 16;
     fp.ok_mul2 = g.Pz == 1 && fp.ok_y;
     // fp.x_pipe, fp.mid_pipe, fp.chunk_w, fp.nstream come from the context (mm_set_option; defaults set by
     // mm_create).  L2-resident chunks (chunk_w = columns per chunk, multiple of 16) are off by default:

@@ -154,6 +154,9 @@ struct mm_ctx {
     bool k0_valid;
     int k0_method;
     FastPlan fp;
+    // batch of independent films (mm_create_batch): g.Nz = number of films, Pz = 1, no coupling along z
+    int batch;
+    float* hext_b;    // per-film applied field [batch][3], reduced units (mm_batch_set_field), or NULL
     // slab decomposition (mm_dist.cuh): g holds the LOCAL planes, gmid the geometry of the z pass on the pencil
     bool dist;
     mm_slab slab;
@@ -215,7 +218,8 @@ void fill_material(const mm_ctx* c, EpiParams& p, uint64_t step, double dt_therm
     const Geom& g = c->g;
     const double Ms = M.Ms;
     const double g0 = M.gamma0 > 0 ? M.gamma0 : GAMMA0_DEFAULT;
-    const int ext[3] = { g.Nx, g.Ny, c->dist ? c->gNz : g.Nz };     // a slab has z neighbours even with one local plane
+    // a slab has z neighbours even with one local plane; the films of a batch are not coupled
+    const int ext[3] = { g.Nx, g.Ny, c->dist ? c->gNz : (c->batch ? 1 : g.Nz) };
     p.demag = M.demag ? 1 : 0;
     const bool ex_in_k = M.exchange_in_kernel && M.demag;      // then the convolution carries the exchange field
     for (int a = 0; a < 3; ++a)
@@ -227,6 +231,8 @@ void fill_material(const mm_ctx* c, EpiParams& p, uint64_t step, double dt_therm
         p.u[a] = un > 0 ? (float)(u[a] / un) : 0.f;
         p.hext[a] = (float)(M.Bext[a] / (MU0 * Ms));
     }
+    p.hext_b = c->batch ? c->hext_b : nullptr;
+    p.plane_cells = (unsigned)(g.Nx * g.Ny);
     p.geometry = M.geometry ? 1 : 0;
     p.cubic = (M.K1 != 0.0 || M.K2 != 0.0) ? 1 : 0;
     if (p.cubic) {
@@ -650,6 +656,7 @@ mm_status mm_create(mm_ctx** out, const int grid[3], const double cellsize[3], c
     c->gstream = nullptr;
     c->gev[0] = c->gev[1] = nullptr;
     c->use_graph = 1;
+    c->batch = 0; c->hext_b = nullptr;
     c->dist = false; c->gNz = grid[2]; c->slab_buf = c->pencil_buf = nullptr; c->slab_elems = c->pencil_elems = 0;
     c->gexec = nullptr; c->g_method = -1; c->g_dt = 0.0; c->g_m = nullptr; c->g_epoch = 0; c->g_per = 0;
     c->epoch = 1;
@@ -705,6 +712,7 @@ static void free_workspaces(mm_ctx* c)
     for (int a = 0; a < 3; ++a) fr(c->tw[a]);
     for (int i = 0; i < 7; ++i) fr(c->kb[i]);
     fr(c->ms[0]); fr(c->ms[1]); fr(c->mtmp); fr(c->mhost); fr(c->hfield);
+    fr(c->hext_b);
     fr(c->maxbits); fr(c->ctl); fr(c->ctl_scratch); fr(c->step_dev); fr(c->slab_buf); fr(c->pencil_buf);
     fast_plan_destroy(c->fp);
 }
@@ -730,7 +738,8 @@ mm_status mm_demag_init(mm_ctx* c)
 static mm_status demag_init_impl(mm_ctx* c)
 {
     const Geom& g = c->g;
-    const int grid[3] = { g.Nx, g.Ny, c->dist ? c->gNz : g.Nz };     // the kernel is that of the whole grid
+    // the kernel is that of the whole grid (slab ranks) / of one film (batch)
+    const int grid[3] = { g.Nx, g.Ny, c->dist ? c->gNz : (c->batch ? 1 : g.Nz) };
     const size_t nC = (size_t)g.Cx * g.Cy * g.Cz;
     std::vector<float> kh;
     try {
@@ -800,6 +809,8 @@ static mm_status demag_init_impl(mm_ctx* c)
     if ((s = set_smem(c, k_gen_inv_x)) != MM_OK) return s;
     std::string ferr;
     if (!fast_plan_init(c->fp, g, &ferr)) return fail(c, MM_ECUDA, ferr);
+    if (c->batch && !((c->fp.ok_x || c->fp.ok_xr) && c->fp.ok_mul2 && g.Nx % 4 == 0))
+        return fail(c, MM_EUNSUPPORTED, "mm_create_batch needs padded x and y lengths with size-specialised kernels (32 ... 1024) and Nx % 4 == 0");
     if (c->dist) {
         if (!(c->fp.ok_x && c->fp.ok_y && c->fp.ok_mid3))
             return fail(c, MM_EUNSUPPORTED, "mm_create_dist needs size-specialised kernels for all three padded lengths");
@@ -1303,6 +1314,40 @@ mm_status mm_padded_size(const mm_ctx* c, int P_out[3], int C_out[3])
     return MM_OK;
 }
 
+mm_status mm_create_batch(mm_ctx** out, const int grid[3], const double cellsize[3], const int pbc[3],
+                          void* cuda_stream, int nfilms)
+{
+    if (!out) return MM_EINVAL;
+    *out = nullptr;
+    if (!grid || nfilms < 1) return fail(nullptr, MM_EINVAL, "mm_create_batch: nfilms must be >= 1");
+    if (grid[2] != 1) return fail(nullptr, MM_EUNSUPPORTED, "mm_create_batch: the members are films (Nz = 1)");
+    mm_ctx* c = nullptr;
+    const mm_status s = mm_create(&c, grid, cellsize, pbc, cuda_stream);
+    if (s != MM_OK) return s;
+    c->batch = nfilms;
+    c->g.Nz = nfilms;            // planes of every field and spectrum; Pz = Cz = 1: no transform along z
+    *out = c;
+    return MM_OK;
+}
+
+mm_status mm_batch_set_field(mm_ctx* c, const double* B_host)
+{
+    if (!c || !c->batch) return MM_EINVAL;
+    mm_status s = check_ready(c);
+    if (s != MM_OK) return s;
+    c->epoch++;
+    if (!B_host) {               // back to the material's uniform field
+        if (c->hext_b) { cudaFree(c->hext_b); c->hext_b = nullptr; }
+        return MM_OK;
+    }
+    std::vector<float> h((size_t)3 * c->batch);
+    for (size_t i = 0; i < h.size(); ++i) h[i] = (float)(B_host[i] / (MU0 * c->mat.Ms));
+    if (!c->hext_b) CUDA_TRY(c, cudaMalloc(&c->hext_b, h.size() * sizeof(float)));
+    CUDA_TRY(c, cudaMemcpyAsync(c->hext_b, h.data(), h.size() * sizeof(float), cudaMemcpyHostToDevice, c->stream));
+    CUDA_TRY(c, cudaStreamSynchronize(c->stream));       // `h` is a local
+    return MM_OK;
+}
+
 mm_status mm_padded_size_of(const int grid[3], const int pbc[3], int P_out[3], int C_out[3])
 {
     if (!grid || !pbc) return MM_EINVAL;
@@ -1340,6 +1385,8 @@ uint64_t mm_launch_count(const mm_ctx* c) { return c ? c->kt.launches : 0; }
 mm_status mm_set_fast_path(mm_ctx* c, int enable)
 {
     if (!c) return MM_EINVAL;
+    if ((c->batch || c->dist) && enable >= 0 && (enable & FAST_ALL) != FAST_ALL)
+        return fail(c, MM_EUNSUPPORTED, "batch and slab contexts run the size-specialised kernels only");
     c->fast = enable < 0 ? FAST_ALL : (enable & FAST_ALL);
     c->epoch++;
     return MM_OK;

@@ -38,6 +38,8 @@ struct EpiParams {
     float wex[3];        // 2A/(mu0 Ms^2 d_a^2); 0 for a one-cell axis           Eq. (3)
     float kan, u[3];     // 2Ku/(mu0 Ms^2), axis                                  Eq. (4)
     float hext[3];       // B/(mu0 Ms)
+    const float* hext_b; // batch of films (mm_create_batch): per-plane applied field [Nz][3], overrides hext; or NULL
+    unsigned plane_cells; // Ny * Nx (plane index of a cell = idx / plane_cells), used with hext_b
     int geometry;        // cells with m = 0 are empty (reading A15)
     int cubic;           // Eq. (5)
     float k1c, k2c;      // 2 K1/(mu0 Ms^2), 2 K2/(mu0 Ms^2)

@@ -100,6 +100,8 @@ def lib():
         L.mm_set_fast_path.argtypes = [vp, C.c_int]
         L.mm_copy_bandwidth.argtypes = [vp, vp, vp, C.c_size_t, C.c_int, d3]
         sz = C.POINTER(C.c_size_t)
+        L.mm_create_batch.argtypes = [C.POINTER(vp), i3, d3, i3, vp, C.c_int]
+        L.mm_batch_set_field.argtypes = [vp, vp]
         L.mm_slab_partition.argtypes = [i3, i3, C.c_int, C.c_int, C.POINTER(Slab)]
         L.mm_create_dist.argtypes = [C.POINTER(vp), i3, d3, i3, vp, C.c_int, C.c_int]
         L.mm_dist_buffers.argtypes = [vp, C.POINTER(vp), sz, C.POINTER(vp), sz]
@@ -170,12 +172,12 @@ class Sim:
     """One mm_ctx.  Fields are torch CUDA float32 tensors of shape (3, Nz, Ny, Nx)."""
 
     def __init__(self, grid, cell, pbc=(0, 0, 0), mat=None, demag=True, stream=None, demag_init=True,
-                 options=None):
+                 options=None, nfilms=0):
         import torch
         self.torch = torch
         self.L = lib()
         self.grid = tuple(int(v) for v in grid)
-        self.shape = (3, self.grid[2], self.grid[1], self.grid[0])
+        self.shape = (3, int(nfilms) if nfilms else self.grid[2], self.grid[1], self.grid[0])
         self.ctx = C.c_void_p()
         if torch.cuda.is_available():
             torch.cuda.init()
@@ -183,7 +185,10 @@ class Sim:
             sp = C.c_void_p(s.cuda_stream)
         else:
             sp = C.c_void_p(0)
-        st = self.L.mm_create(C.byref(self.ctx), _i3(grid), _d3(cell), _i3(pbc), sp)
+        if nfilms:                # mm_create_batch: nfilms independent films, fields (3, nfilms, Ny, Nx)
+            st = self.L.mm_create_batch(C.byref(self.ctx), _i3(grid), _d3(cell), _i3(pbc), sp, int(nfilms))
+        else:
+            st = self.L.mm_create(C.byref(self.ctx), _i3(grid), _d3(cell), _i3(pbc), sp)
         if st != MM_OK:
             raise MMError(st, self.L.mm_last_error(None).decode())
         for k, v in (options or {}).items():
@@ -207,6 +212,14 @@ class Sim:
 
     def set_option(self, key, value):
         self._chk(self.L.mm_set_option(self.ctx, key.encode(), int(value)))
+
+    def batch_set_field(self, B):
+        """One applied field (tesla) per film, array (nfilms, 3); None: the material's uniform field again."""
+        if B is None:
+            self._chk(self.L.mm_batch_set_field(self.ctx, C.c_void_p(0)))
+            return
+        b = np.ascontiguousarray(np.asarray(B, dtype=np.float64).reshape(self.shape[1], 3))
+        self._chk(self.L.mm_batch_set_field(self.ctx, b.ctypes.data_as(C.c_void_p)))
 
     def demag_init(self):
         self._chk(self.L.mm_demag_init(self.ctx))

@@ -263,6 +263,8 @@ FAST_GRIDS = [
     ((1024, 16, 2), (3e-9, 3e-9, 3e-9), (0, 0, 0)),     # x = 2048, same
     ((1536, 8, 1), (3e-9, 3e-9, 3e-9), (1, 0, 0)),      # x = 1536 periodic (no padding)
     ((32, 40, 128), (3e-9, 3e-9, 3e-9), (0, 0, 1)),     # periodic z of length 128 (no padding), ragged kx tile
+    ((16, 16, 8), (3e-9, 3e-9, 3e-9), (0, 0, 0)),       # 32 x 32 x 16: the shortest size-specialised lines (x, y)
+    ((64, 16, 1), (4e-9, 4e-9, 3e-9), (0, 0, 0)),       # film 128 x 32 (the batch-of-films shape)
 ]
 
 
