@@ -80,8 +80,8 @@ def algorithmic_bytes(wl, method="rk4"):
 
 def measured_traffic(config, pass_name):
     """DRAM bytes per launch of the pass's kernel(s) from the committed ncu --set full capture
-    (profiles/r1_fast_path_traffic.txt: dram__bytes_read.sum + dram__bytes_write.sum), or None."""
-    p = os.path.join(ROOT, "profiles", "r1_fast_path_traffic.txt")
+    (profiles/r2_fast_path_traffic.txt: dram__bytes_read.sum + dram__bytes_write.sum), or None."""
+    p = os.path.join(ROOT, "profiles", "r2_fast_path_traffic.txt")
     try:
         d = json.load(open(p))
         return d.get(config, {}).get(pass_name)
