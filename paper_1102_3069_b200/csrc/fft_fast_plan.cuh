@@ -11,6 +11,8 @@ struct FastPlan {
     bool ok_xr;                          // x passes through the half-length complex transform (Px = 1536, 2048)
     float2* twx;                         // ok_xr: exp(-i pi k / Lc), k < Lc = Px / 2
     float2* tw[3];                       // per axis: tw[k2 * T + t] = exp(-2 pi i t k2 / L)
+    int y_split;                         // y lines of 2048 / 4096: 2 / 4 interleaved transforms of 1024 (else 0)
+    float2* twl;                         // y_split: exp(-2 pi i j / Py), j < Py
     int nsm;                             // SM count (persistent grids)
     int x_pipe;                          // x passes, cp.async-pipelined forms: bit 0 forward (default), bit 1 inverse (option "x_pipe")
     int mid_pipe;                        // last-axis pass: persistent pipelined kernel (option "mid_pipe")
@@ -309,11 +311,85 @@ inline bool fast_inv_x_h(const FastPlan& fp, const Geom& g, cudaStream_t st, con
     return r;
 }
 
+// ---------------------------------------------------------------------------------------------
+// Long y lines (Py = R * 1024, R = 2 or 4; the paper's Table 1 goes to 1024^2 and 2048^2 cells):
+// one decimation-in-time level outside the size-specialised kernel.  Rows n = R r + q form R interleaved
+// sequences; each is transformed by the 1024-point kernel with a row stride of R (the ColTile strides carry it,
+// the kernel is unchanged: a zero-padded line of Py has zero-padded sub-sequences of 1024), sub-spectrum S_q
+// landing in rows q * 1024 + k of the spectrum.  k_y_combine then forms, in place and per (plane, k, column),
+//   forward:  X[k + 1024 m] = sum_q w_R^(q m) (w_Py^(q k) S_q[k])
+//   inverse:  Y_q[k] = w_Py^(-q k) sum_m w_R^(-q m) X[k + 1024 m]      (before the R inverse transforms)
+// ---------------------------------------------------------------------------------------------
+namespace ff {
+template <int R, int SGN>
+__global__ void __launch_bounds__(128)
+k_y_combine(ColTile ct, int nplane, int Ls, float2* __restrict__ b, const float2* __restrict__ twl)
+{
+    const int col = blockIdx.x * blockDim.x + threadIdx.x;
+    const int k = blockIdx.y, cz = blockIdx.z;
+    if (col >= ct.ncol || cz >= nplane) return;
+    float2* p = b + (size_t)cz * ct.b_plane + (size_t)k * ct.b_row + col;
+    const size_t rs = (size_t)Ls * ct.b_row;
+    float2 v[R];
+#pragma unroll
+    for (int q = 0; q < R; ++q) v[q] = p[q * rs];
+    auto tw = [&](int q) {                       // w_Py^(q k), conjugated for the inverse
+        float2 w = __ldg(twl + q * k);
+        if (SGN > 0) w.y = -w.y;
+        return w;
+    };
+    if (SGN < 0) {
+#pragma unroll
+        for (int q = 1; q < R; ++q) v[q] = cmul(v[q], tw(q));
+    }
+    if constexpr (R == 2) {
+        const float2 a0 = cadd(v[0], v[1]), a1 = csub(v[0], v[1]);
+        v[0] = a0; v[1] = a1;
+    } else {
+        const float2 s02 = cadd(v[0], v[2]), d02 = csub(v[0], v[2]);
+        const float2 s13 = cadd(v[1], v[3]), d13 = cmuli<SGN>(csub(v[1], v[3]));
+        v[0] = cadd(s02, s13); v[2] = csub(s02, s13);
+        v[1] = cadd(d02, d13); v[3] = csub(d02, d13);
+    }
+    if (SGN > 0) {
+#pragma unroll
+        for (int q = 1; q < R; ++q) v[q] = cmul(v[q], tw(q));
+    }
+#pragma unroll
+    for (int q = 0; q < R; ++q) p[q * rs] = v[q];
+}
+}  // namespace ff
+
+template <int R>
+inline bool fast_y_long(const FastPlan& fp, const Geom& g, cudaStream_t st, int sgn, const ff::ColTile& ct, float2* a,
+                        float2* b)
+{
+    constexpr int Ls = 1024;
+    const int nplane = 3 * g.Nz;
+    dim3 cg((ct.ncol + 127) / 128, Ls, nplane);
+    if (sgn > 0) ff::k_y_combine<R, 1><<<cg, 128, 0, st>>>(ct, nplane, Ls, b, fp.twl);
+    for (int q = 0; q < R; ++q) {
+        ff::ColTile cq = ct;
+        cq.a_row = ct.a_row * R;
+        float2* aq = a + (size_t)q * ct.a_row;
+        float2* bq = b + (size_t)q * Ls * ct.b_row;
+        const bool ok = sgn < 0 ? (g.pery ? ff::launch_y<32, 32, -1, true>(fp, g, st, cq, aq, bq)
+                                          : ff::launch_y<32, 32, -1, false>(fp, g, st, cq, aq, bq))
+                                : (g.pery ? ff::launch_y<32, 32, 1, true>(fp, g, st, cq, aq, bq)
+                                          : ff::launch_y<32, 32, 1, false>(fp, g, st, cq, aq, bq));
+        if (!ok) return false;
+    }
+    if (sgn < 0) ff::k_y_combine<R, -1><<<cg, 128, 0, st>>>(ct, nplane, Ls, b, fp.twl);
+    return true;
+}
+
 // sgn < 0: specA rows y < Ny -> specB rows ky < Py; sgn > 0: back.  a, b point at column ct.kx0.
 inline bool fast_y(const FastPlan& fp, const Geom& g, cudaStream_t st, int sgn, const ff::ColTile& ct, float2* a,
                    float2* b)
 {
     if (!fp.ok_y) return false;
+    if (fp.y_split == 2) return fast_y_long<2>(fp, g, st, sgn, ct, a, b);
+    if (fp.y_split == 4) return fast_y_long<4>(fp, g, st, sgn, ct, a, b);
     bool r = false;
 #define CALL(T, E)                                                                         \
     r = sgn < 0 ? (g.pery ? ff::launch_y<T, E, -1, true>(fp, g, st, ct, a, b)              \
@@ -397,7 +473,9 @@ inline bool fast_plan_init(FastPlan& fp, const Geom& g, std::string* err)
     fp.ok_x = ff::split(g.Px, &T, &E);
     fp.ok_xr = !fp.ok_x && (g.Px == 1536 || g.Px == 2048) && g.Nx % 2 == 0;
     fp.twx = nullptr;
-    fp.ok_y = g.Py > 1 && ff::split(g.Py, &T, &E);
+    fp.y_split = (g.Py == 2048 || g.Py == 4096) ? g.Py / 1024 : 0;
+    fp.twl = nullptr;
+    fp.ok_y = g.Py > 1 && (ff::split(g.Py, &T, &E) || fp.y_split);
     fp.ok_mid3 = g.Pz >= 64 && g.Py > 1 && ff::split(g.Pz, &T, &E) && E <= 16;
     fp.ok_mul2 = g.Pz == 1 && fp.ok_y;
     // fp.x_pipe, fp.mid_pipe, fp.chunk_w, fp.nstream come from the context (mm_set_option; defaults set by
@@ -428,7 +506,19 @@ inline bool fast_plan_init(FastPlan& fp, const Geom& g, std::string* err)
         if (err) *err = "fast plan: cannot read the SM count of the current device";
         return false;
     }
-    const int P[3] = { fp.ok_xr ? g.Px / 2 : g.Px, g.Py, g.Pz };
+    const int P[3] = { fp.ok_xr ? g.Px / 2 : g.Px, fp.y_split ? 1024 : g.Py, g.Pz };
+    if (fp.y_split) {
+        std::vector<float2> tl((size_t)g.Py);
+        for (int j = 0; j < g.Py; ++j) {
+            const long double ang = -2.0L * 3.14159265358979323846264338327950288L * j / g.Py;
+            tl[j] = make_float2((float)cosl(ang), (float)sinl(ang));
+        }
+        if (cudaMalloc(&fp.twl, tl.size() * sizeof(float2)) != cudaSuccess ||
+            cudaMemcpy(fp.twl, tl.data(), tl.size() * sizeof(float2), cudaMemcpyHostToDevice) != cudaSuccess) {
+            if (err) *err = "fast plan: twiddle table allocation failed";
+            return false;
+        }
+    }
     if (fp.ok_xr) {
         const int Lc = g.Px / 2;
         std::vector<float2> tx((size_t)Lc);
@@ -545,6 +635,8 @@ inline void fast_plan_destroy(FastPlan& fp)
     for (int a = 0; a < 3; ++a) { cudaFree(fp.tw[a]); fp.tw[a] = nullptr; }
     cudaFree(fp.twx);
     fp.twx = nullptr;
+    cudaFree(fp.twl);
+    fp.twl = nullptr;
     for (int s = 0; s < 4; ++s) {
         if (fp.stream[s]) cudaStreamDestroy(fp.stream[s]);
         if (fp.ev_join[s]) cudaEventDestroy(fp.ev_join[s]);

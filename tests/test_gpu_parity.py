@@ -265,6 +265,10 @@ FAST_GRIDS = [
     ((32, 40, 128), (3e-9, 3e-9, 3e-9), (0, 0, 1)),     # periodic z of length 128 (no padding), ragged kx tile
     ((16, 16, 8), (3e-9, 3e-9, 3e-9), (0, 0, 0)),       # 32 x 32 x 16: the shortest size-specialised lines (x, y)
     ((64, 16, 1), (4e-9, 4e-9, 3e-9), (0, 0, 0)),       # film 128 x 32 (the batch-of-films shape)
+    ((16, 1024, 1), (3e-9, 3e-9, 3e-9), (0, 0, 0)),     # y = 2048: two interleaved 1024-point transforms + combine
+    ((8, 2048, 1), (3e-9, 3e-9, 3e-9), (0, 0, 0)),      # y = 4096: four
+    ((16, 2048, 1), (3e-9, 3e-9, 3e-9), (0, 1, 0)),     # y = 2048 periodic (no padding)
+    ((32, 1024, 2), (3e-9, 3e-9, 3e-9), (0, 0, 0)),     # y = 2048 in a 3D grid (z generic), ragged kx tile
 ]
 
 
