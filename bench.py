@@ -266,8 +266,7 @@ def run_sweep(args):
     import paper_1102_3069_b200 as mm
     from paper_1102_3069_b200 import workloads as wlm
     torch.cuda.set_device(0)
-    # 2048^2 of the paper's table is left out: its padded x length 4096 exceeds the longest line of the kernels
-    grids = [(n, n, 1) for n in (32, 64, 128, 256, 512, 1024)] + [(n, n, n) for n in (8, 16, 32, 64, 128, 256)]
+    grids = [(n, n, 1) for n in (32, 64, 128, 256, 512, 1024, 2048)] + [(n, n, n) for n in (8, 16, 32, 64, 128, 256)]
     # PAPER.md:225 (Fig. 6): "non-smooth" sizes are slower than the power of two above them (992^2 was 5x slower
     # than 1024^2 on the paper's GPU).  992 = 2^5 * 31 is refused here (only 2^a 3^b 5^c 7^d sizes are accepted,
     # PAPER.md:171); its smooth neighbours 960 = 2^6*3*5, 1000 = 2^3*5^3 and 1008 = 2^4*3^2*7 run on the generic

@@ -11,6 +11,10 @@ struct FastPlan {
     bool ok_xr;                          // x passes through the half-length complex transform (Px = 1536, 2048)
     float2* twx;                         // ok_xr: exp(-i pi k / Lc), k < Lc = Px / 2
     float2* tw[3];                       // per axis: tw[k2 * T + t] = exp(-2 pi i t k2 / L)
+    bool x_split;                        // Px = 4096: even / odd samples through the 2048-point real transform + combine
+    float* xs_real;                      // x_split: de-interleaved rows [2 nrow][Nx / 2]
+    float2* xs_spec;                     // x_split: their half spectra [2 nrow][XS_STRIDE]
+    float2* twx4;                        // x_split: exp(-2 pi i j / 4096), j <= 1024
     int y_split;                         // y lines of 2048 / 4096: 2 / 4 interleaved transforms of 1024 (else 0)
     float2* twl;                         // y_split: exp(-2 pi i j / Py), j < Py
     int nsm;                             // SM count (persistent grids)
@@ -255,8 +259,74 @@ bool launch_mid3(const FastPlan& fp, const Geom& g, cudaStream_t st, const ColTi
 
 }  // namespace ff
 
+// ---------------------------------------------------------------------------------------------
+// x lines of 4096 (2048 cells, open; 4096 cells, periodic -- PAPER.md:245, the largest 2D grid of Table 1): one
+// decimation-in-time level outside the kernels.  The even and the odd samples of a row are two real sequences of
+// half the length; each goes through the 2048-point real transform (k_fwd_x_r / k_inv_x_h_r, unchanged), and
+//   forward:  X[j] = E[j] + w^j O[j],  X[2048 - j] = conj(E[j] - w^j O[j]),  j <= 1024,  w = exp(-2 pi i / 4096)
+//   inverse:  E'[j] = X[j] + conj X[2048 - j],  O'[j] = conj(w^j) (X[j] - conj X[2048 - j])
+// ---------------------------------------------------------------------------------------------
+#define MM_XS_STRIDE 1032
+namespace ff {
+__global__ void k_x_deinterleave(const float2* __restrict__ m, float* __restrict__ tmp, size_t nrow, int half)
+{
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < nrow * half; i += (size_t)gridDim.x * blockDim.x) {
+        const size_t row = i / half, n = i - row * half;
+        const float2 v = m[i];
+        tmp[(2 * row) * half + n] = v.x;
+        tmp[(2 * row + 1) * half + n] = v.y;
+    }
+}
+__global__ void k_x_interleave(const float* __restrict__ tmp, float2* __restrict__ out, size_t nrow, int half)
+{
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < nrow * half; i += (size_t)gridDim.x * blockDim.x) {
+        const size_t row = i / half, n = i - row * half;
+        out[i] = make_float2(tmp[(2 * row) * half + n], tmp[(2 * row + 1) * half + n]);
+    }
+}
+template <int SGN>
+__global__ void k_x_combine(float2* __restrict__ ts, float2* __restrict__ specA, size_t nrow, int CxS,
+                            const float2* __restrict__ tw4)
+{
+    const int j = blockIdx.x * blockDim.x + threadIdx.x;
+    const size_t row = blockIdx.y;
+    if (j > 1024 || row >= nrow) return;
+    float2* e = ts + (2 * row) * MM_XS_STRIDE + j;
+    float2* o = ts + (2 * row + 1) * MM_XS_STRIDE + j;
+    float2* x = specA + row * CxS;
+    const float2 w = __ldg(tw4 + j);
+    if (SGN < 0) {
+        const float2 E = *e, wO = cmul(w, *o);
+        x[j] = cadd(E, wO);
+        if (j != 1024) x[2048 - j] = cconj(csub(E, wO));
+    } else {
+        const float2 A = x[j], B = cconj(x[2048 - j]);
+        *e = cadd(A, B);
+        *o = cmul(cconj(w), csub(A, B));
+    }
+}
+}  // namespace ff
+
+inline Geom x_split_geom(const Geom& g)
+{
+    Geom h = g;
+    h.Nx = g.Nx / 2; h.Ny = 2 * g.Ny; h.Px = g.Px / 2; h.Cx = h.Px / 2 + 1; h.CxS = MM_XS_STRIDE;
+    return h;
+}
+
 inline bool fast_fwd_x(const FastPlan& fp, const Geom& g, cudaStream_t st, const float* m, float2* specA)
 {
+    if (fp.x_split) {
+        const size_t nrow = (size_t)3 * g.Nz * g.Ny;
+        const Geom h = x_split_geom(g);
+        ff::k_x_deinterleave<<<fp.nsm * 8, 256, 0, st>>>(reinterpret_cast<const float2*>(m), fp.xs_real, nrow, g.Nx / 2);
+        if (!(g.perx ? ff::launch_fwd_x_r<32, 32, true>(fp, h, st, fp.xs_real, fp.xs_spec)
+                     : ff::launch_fwd_x_r<32, 32, false>(fp, h, st, fp.xs_real, fp.xs_spec)))
+            return false;
+        dim3 cg((1025 + 127) / 128, (unsigned)nrow);
+        ff::k_x_combine<-1><<<cg, 128, 0, st>>>(fp.xs_spec, specA, nrow, g.CxS, fp.twx4);
+        return true;
+    }
     if (fp.ok_xr) {
         if (g.Px == 1536) return g.perx ? ff::launch_fwd_x_r<16, 48, true>(fp, g, st, m, specA)
                                         : ff::launch_fwd_x_r<16, 48, false>(fp, g, st, m, specA);
@@ -295,6 +365,17 @@ inline bool fast_inv_x(const FastPlan& fp, const Geom& g, cudaStream_t st, const
 inline bool fast_inv_x_h(const FastPlan& fp, const Geom& g, cudaStream_t st, const float2* specA, float* out,
                          float scale)
 {
+    if (fp.x_split) {
+        const size_t nrow = (size_t)3 * g.Nz * g.Ny;
+        const Geom h = x_split_geom(g);
+        dim3 cg((1025 + 127) / 128, (unsigned)nrow);
+        ff::k_x_combine<1><<<cg, 128, 0, st>>>(fp.xs_spec, const_cast<float2*>(specA), nrow, g.CxS, fp.twx4);
+        if (!(g.perx ? ff::launch_inv_x_h_r<32, 32, true>(fp, h, st, fp.xs_spec, fp.xs_real, scale)
+                     : ff::launch_inv_x_h_r<32, 32, false>(fp, h, st, fp.xs_spec, fp.xs_real, scale)))
+            return false;
+        ff::k_x_interleave<<<fp.nsm * 8, 256, 0, st>>>(fp.xs_real, reinterpret_cast<float2*>(out), nrow, g.Nx / 2);
+        return true;
+    }
     if (fp.ok_xr) {
         if (g.Px == 1536) return g.perx ? ff::launch_inv_x_h_r<16, 48, true>(fp, g, st, specA, out, scale)
                                         : ff::launch_inv_x_h_r<16, 48, false>(fp, g, st, specA, out, scale);
@@ -472,6 +553,8 @@ inline bool fast_plan_init(FastPlan& fp, const Geom& g, std::string* err)
     int T, E, dev = 0;
     fp.ok_x = ff::split(g.Px, &T, &E);
     fp.ok_xr = !fp.ok_x && (g.Px == 1536 || g.Px == 2048) && g.Nx % 2 == 0;
+    fp.x_split = g.Px == 4096 && g.Nx % 4 == 0 && (size_t)3 * g.Nz * g.Ny <= 65535;      // (rows: grid.y of the combine)
+    fp.xs_real = nullptr; fp.xs_spec = nullptr; fp.twx4 = nullptr;
     fp.twx = nullptr;
     fp.y_split = (g.Py == 2048 || g.Py == 4096) ? g.Py / 1024 : 0;
     fp.twl = nullptr;
@@ -506,7 +589,23 @@ inline bool fast_plan_init(FastPlan& fp, const Geom& g, std::string* err)
         if (err) *err = "fast plan: cannot read the SM count of the current device";
         return false;
     }
-    const int P[3] = { fp.ok_xr ? g.Px / 2 : g.Px, fp.y_split ? 1024 : g.Py, g.Pz };
+    const int P[3] = { fp.x_split ? 1024 : (fp.ok_xr ? g.Px / 2 : g.Px), fp.y_split ? 1024 : g.Py, g.Pz };
+    if (fp.x_split) {
+        const size_t nrow = (size_t)3 * g.Nz * g.Ny;
+        std::vector<float2> t4(1025);
+        for (int j = 0; j <= 1024; ++j) {
+            const long double ang = -2.0L * 3.14159265358979323846264338327950288L * j / 4096.0L;
+            t4[j] = make_float2((float)cosl(ang), (float)sinl(ang));
+        }
+        if (cudaMalloc(&fp.xs_real, nrow * g.Nx * sizeof(float)) != cudaSuccess ||
+            cudaMalloc(&fp.xs_spec, 2 * nrow * MM_XS_STRIDE * sizeof(float2)) != cudaSuccess ||
+            cudaMemset(fp.xs_spec, 0, 2 * nrow * MM_XS_STRIDE * sizeof(float2)) != cudaSuccess ||
+            cudaMalloc(&fp.twx4, t4.size() * sizeof(float2)) != cudaSuccess ||
+            cudaMemcpy(fp.twx4, t4.data(), t4.size() * sizeof(float2), cudaMemcpyHostToDevice) != cudaSuccess) {
+            if (err) *err = "fast plan: x-split workspace allocation failed";
+            return false;
+        }
+    }
     if (fp.y_split) {
         std::vector<float2> tl((size_t)g.Py);
         for (int j = 0; j < g.Py; ++j) {
@@ -519,8 +618,8 @@ inline bool fast_plan_init(FastPlan& fp, const Geom& g, std::string* err)
             return false;
         }
     }
-    if (fp.ok_xr) {
-        const int Lc = g.Px / 2;
+    if (fp.ok_xr || fp.x_split) {
+        const int Lc = fp.x_split ? 1024 : g.Px / 2;
         std::vector<float2> tx((size_t)Lc);
         for (int k = 0; k < Lc; ++k) {
             const long double ang = -3.14159265358979323846264338327950288L * k / Lc;
@@ -637,6 +736,8 @@ inline void fast_plan_destroy(FastPlan& fp)
     fp.twx = nullptr;
     cudaFree(fp.twl);
     fp.twl = nullptr;
+    cudaFree(fp.xs_real); cudaFree(fp.xs_spec); cudaFree(fp.twx4);
+    fp.xs_real = nullptr; fp.xs_spec = nullptr; fp.twx4 = nullptr;
     for (int s = 0; s < 4; ++s) {
         if (fp.stream[s]) cudaStreamDestroy(fp.stream[s]);
         if (fp.ev_join[s]) cudaEventDestroy(fp.ev_join[s]);
