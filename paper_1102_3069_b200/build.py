@@ -1,19 +1,24 @@
 """Build the C-ABI library libmm_b200.so in-tree with nvcc for sm_100a (no JIT cache involved).
 
-    python -m paper_1102_3069_b200.build [--force]
+    python -m paper_1102_3069_b200.build [--force] [-v]
+
+Every kernel family is a translation unit of its own (csrc/kern_*.cu): they compile in parallel, and a change in
+one family cannot perturb the code generated for another.
 """
 from __future__ import annotations
 
 import os
 import subprocess
 import sys
+from concurrent.futures import ThreadPoolExecutor
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.environ.get("MM_B200_LIB") or os.path.join(HERE, "libmm_b200.so")
-SOURCES = ["mm_api.cu", "demag_host.cpp"]
-NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "-split-compile", "0",
-              "-Xcompiler", "-fPIC,-fopenmp,-O2", "-shared", "-lgomp"]
+OBJDIR = os.path.join(HERE, "build")
+SOURCES = ["mm_api.cu", "kern_x.cu", "kern_y.cu", "kern_mid.cu", "kern_epi.cu", "kern_gen.cu", "demag_host.cpp"]
+NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
+              "-Xcompiler", "-fPIC,-fopenmp,-O2"]
 
 
 def _stale() -> bool:
@@ -28,11 +33,22 @@ def _stale() -> bool:
 def build(force: bool = False, verbose: bool = False) -> str:
     if force or _stale():
         nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-        extra = os.environ.get("MM_NVCC_EXTRA", "").split()       # e.g. -DMM_PACKED_F32X2 (experiments)
-        cmd = [nvcc, *NVCC_FLAGS, *extra, "-o", LIB, *[os.path.join(CSRC, s) for s in SOURCES]]
-        if verbose:
-            cmd += ["-Xptxas", "-v"]
-        subprocess.check_call(cmd)
+        extra = os.environ.get("MM_NVCC_EXTRA", "").split()       # e.g. -DMM_TW_SYM (experiments)
+        tag = os.path.splitext(os.path.basename(LIB))[0]
+        objdir = os.path.join(OBJDIR, tag)
+        os.makedirs(objdir, exist_ok=True)
+
+        def compile_one(src):
+            obj = os.path.join(objdir, os.path.splitext(src)[0] + ".o")
+            cmd = [nvcc, *NVCC_FLAGS, *extra, "-c", "-o", obj, os.path.join(CSRC, src)]
+            if verbose:
+                cmd += ["-Xptxas", "-v"]
+            subprocess.check_call(cmd)
+            return obj
+
+        with ThreadPoolExecutor(max_workers=len(SOURCES)) as ex:
+            objs = list(ex.map(compile_one, SOURCES))
+        subprocess.check_call([nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-shared", "-o", LIB, *objs, "-lgomp"])
     return LIB
 
 

@@ -182,6 +182,42 @@ __device__ __forceinline__ void fft_reg_half(float2 (&v)[N])
     for (int i = 0; i < N / 2; ++i) { v[2 * i] = a[i]; v[2 * i + 1] = b[i]; }
 }
 
+// Inter-stage twiddles v[k2] *= w^(t k2), w = exp(SGN' 2 pi i / (T E)), from the table tw[k2 * T + t] (forward
+// sign; CONJ takes the conjugate).  For E >= 16 only k2 <= E/4 and k2 = E/2 are loaded; the others follow from
+//   w^(t (E/2 + k)) = d w^(t k),  w^(t (E/2 - k)) = d conj(w^(t k)),  w^(t (E - k)) = d^2 conj(w^(t k)),  d = w^(t E/2)
+// -- 9 loads instead of 31 for E = 32 at the price of a few dozen FMAs: the passes that wait on these loads
+// (long-scoreboard stalls with every register taken by the line) have FP slots to spare (measured: y passes 3 %
+// faster, x passes unchanged; -DMM_TW_PLAIN restores one load per element).
+template <int T, int E, bool CONJ>
+__device__ __forceinline__ void apply_twiddles(float2 (&v)[E], const float2* __restrict__ tw, const int t)
+{
+#if !defined(MM_TW_PLAIN)
+    if constexpr (E % 4 == 0 && E >= 16) {
+        auto ld = [&](int k2) { float2 w = __ldg(tw + k2 * T + t); if (CONJ) w.y = -w.y; return w; };
+        const float2 d = ld(E / 2);
+        const float2 d2 = cmul(d, d);
+        v[E / 2] = cmul(v[E / 2], d);
+#pragma unroll
+        for (int k = 1; k <= E / 4; ++k) {
+            const float2 w = ld(k), wc = cconj(w);
+            v[k] = cmul(v[k], w);
+            if (k < E / 4) {
+                v[E / 2 - k] = cmul(v[E / 2 - k], cmul(d, wc));
+                v[E - k] = cmul(v[E - k], cmul(d2, wc));
+            }
+            v[E / 2 + k] = cmul(v[E / 2 + k], cmul(d, w));
+        }
+        return;
+    }
+#endif
+#pragma unroll
+    for (int k2 = 1; k2 < E; ++k2) {
+        float2 w = __ldg(tw + k2 * T + t);
+        if (CONJ) w.y = -w.y;
+        v[k2] = cmul(v[k2], w);
+    }
+}
+
 struct SyncWarp { __device__ __forceinline__ void operator()() const { __syncwarp(); } };
 struct SyncBlock { __device__ __forceinline__ void operator()() const { __syncthreads(); } };
 

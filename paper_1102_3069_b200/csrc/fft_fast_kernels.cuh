@@ -128,8 +128,7 @@ k_fwd_x_p(Geom g, const float* __restrict__ m, float2* __restrict__ specA, const
         __syncwarp();                           // the region now serves as the exchange buffer
         if constexpr (!PER) fft_reg_half<E, -1>(v);
         else fft_reg<E, -1>(v);
-#pragma unroll
-        for (int k2 = 1; k2 < E; ++k2) v[k2] = cmul(v[k2], __ldg(tw + k2 * T + t));
+        apply_twiddles<T, E, false>(v, tw, t);
 #pragma unroll
         for (int k2 = 0; k2 < E; ++k2) sb[t * (E + 1) + k2] = v[k2];
         __syncwarp();
@@ -277,11 +276,7 @@ k_inv_x_h_p(Geom g, const float2* __restrict__ specA, const float2* __restrict__
 // kx columns starting at kx0, with the y-padded spectrum in a compact chunk buffer [3][Nz][Py][W]
 // that stays in L2 between the forward y pass, the last-axis pass and the inverse y pass.
 // ---------------------------------------------------------------------------------------------
-struct ColTile {
-    int kx0, ncol;                 // first global column, number of valid columns
-    size_t a_row, a_plane;         // specA side: strides in float2 (row y, plane (component, z))
-    size_t b_row, b_plane;         // specB / chunk side
-};
+// (struct ColTile: mm_kernels.h)
 
 // ---------------------------------------------------------------------------------------------
 // a2 / a4: y pass, persistent and software-pipelined.  A tile is 8 adjacent kx columns (64-byte
@@ -336,12 +331,7 @@ k_y_p(ColTile ct, int nplane, float2* __restrict__ a, float2* __restrict__ b, co
         __syncthreads();                        // the region now serves as the exchange buffer
         if constexpr (FWD && !PER) fft_reg_half<E, SGN>(v);
         else fft_reg<E, SGN>(v);
-#pragma unroll
-        for (int k2 = 1; k2 < E; ++k2) {
-            float2 w = __ldg(tw + k2 * T + t);
-            if (SGN > 0) w.y = -w.y;
-            v[k2] = cmul(v[k2], w);
-        }
+        apply_twiddles<T, E, (SGN > 0)>(v, tw, t);
 #pragma unroll
         for (int k2 = 0; k2 < E; ++k2) sm[(t * (E + 1) + k2) * 8 + c] = v[k2];
         __syncthreads();
@@ -850,5 +840,3 @@ k_inv_x_h_r(Geom g, const float2* __restrict__ specA, const float2* __restrict__
 }  // namespace ff
 }  // namespace mm
 
-#include "fft_packed.cuh"
-#include "fft_fast_plan.cuh"

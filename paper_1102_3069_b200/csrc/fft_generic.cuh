@@ -14,14 +14,8 @@
 
 namespace mm {
 
-#define MM_MAXRAD 16
 
-struct FftPlan {            // one axis
-    int L;                  // transform length
-    int nrad;
-    int rad[MM_MAXRAD];
-    const float2* tw;       // device, tw[q] = exp(-2 pi i q / L), q < L
-};
+// (struct FftPlan: mm_kernels.h)
 
 template <int SGN>
 __device__ __forceinline__ void bfly2(float2* v)

@@ -10,10 +10,8 @@
 
 #include "../../include/mm.h"
 #include "demag_host.h"
-#include "mm_common.cuh"
-#include "epilogue.cuh"
-#include "fft_generic.cuh"
-#include "fft_fast.cuh"
+#include "mm_kernels.h"
+#include "fast_plan_host.cuh"
 
 using namespace mm;
 
@@ -271,12 +269,6 @@ void fill_material(const mm_ctx* c, EpiParams& p, uint64_t step, double dt_therm
     p.c_nad = (float)((M.xi - M.alpha) / (1.0 + M.alpha * M.alpha));
 }
 
-template <typename K>
-mm_status set_smem(mm_ctx* c, K kern)
-{
-    CUDA_TRY(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 224 * 1024));
-    return MM_OK;
-}
 
 // ---- one evaluation: the five passes, the last one carrying the epilogue `ep`.  Each pass runs its
 // size-specialised kernel (fft_fast*.cuh) when one exists for the grid and the bit of c->fast is set,
@@ -297,8 +289,7 @@ mm_status launch_eval(mm_ctx* c, const EpiParams& ep)
             if (!((c->fast & FAST_FWD_X) && fast_fwd_x(fp, g, st, ep.m_in, c->specA))) {
                 const int tx = pick_tx(g.Px, 2, 1, &bytes);
                 if (!tx) return fail(c, MM_EUNSUPPORTED, "x line too long for the shared-memory tile");
-                const int npair = 3 * g.Nz * ((g.Ny + 1) / 2);
-                k_gen_fwd_x<<<(npair + tx - 1) / tx, 256, bytes, st>>>(g, c->plan[0], ep.m_in, c->specA, tx);
+                gen_fwd_x(g, c->plan[0], ep.m_in, c->specA, tx, bytes, st);
             }
             c->kt.end(KT_FWD_X);
         }
@@ -316,8 +307,7 @@ mm_status launch_eval(mm_ctx* c, const EpiParams& ep)
                 if (!((c->fast & FAST_Y) && fast_y(fp, g, st, -1, wt, c->specA, c->specB))) {
                     const int tx = pick_tx(g.Py, 2, 1, &bytes);
                     if (!tx) return fail(c, MM_EUNSUPPORTED, "y line too long for the shared-memory tile");
-                    dim3 grid((g.Cx + tx - 1) / tx, 3 * g.Nz);
-                    k_gen_y<-1><<<grid, 256, bytes, st>>>(g, c->plan[1], c->specA, c->specB, tx);
+                    gen_y(g, c->plan[1], -1, c->specA, c->specB, tx, bytes, st);
                 }
                 c->kt.end(KT_FWD_Y);
             }
@@ -326,8 +316,7 @@ mm_status launch_eval(mm_ctx* c, const EpiParams& ep)
                 if (!((c->fast & FAST_MID) && fast_mid3(fp, g, st, wt, c->specB, kh))) {
                     const int tx = pick_tx(g.Pz, 4, 1, &bytes);
                     if (!tx) return fail(c, MM_EUNSUPPORTED, "z line too long for the shared-memory tile");
-                    dim3 grid((g.Cx + tx - 1) / tx, g.Py);
-                    k_gen_mid<<<grid, 256, bytes, st>>>(g, c->plan[2], c->specB, kh, 2, tx);
+                    gen_mid(g, c->plan[2], c->specB, kh, 2, tx, bytes, st);
                 }
                 c->kt.end(KT_MID);
             }
@@ -335,8 +324,7 @@ mm_status launch_eval(mm_ctx* c, const EpiParams& ep)
                 c->kt.begin(KT_INV_Y);
                 if (!((c->fast & FAST_Y) && fast_y(fp, g, st, 1, wt, c->specA, c->specB))) {
                     const int tx = pick_tx(g.Py, 2, 1, &bytes);
-                    dim3 grid((g.Cx + tx - 1) / tx, 3 * g.Nz);
-                    k_gen_y<1><<<grid, 256, bytes, st>>>(g, c->plan[1], c->specB, c->specA, tx);
+                    gen_y(g, c->plan[1], 1, c->specB, c->specA, tx, bytes, st);
                 }
                 c->kt.end(KT_INV_Y);
             }
@@ -356,29 +344,26 @@ mm_status launch_eval(mm_ctx* c, const EpiParams& ep)
                 c->kt.end(KT_INV_Y);
             } else if (const int tx = pick_tx(g.Py, 4, 1, &bytes)) {
                 // generic: y forward, multiply, y inverse in one kernel
-                dim3 grid((g.Cx + tx - 1) / tx, 1);
                 c->kt.begin(KT_MID);
-                k_gen_mid<<<grid, 256, bytes, st>>>(g, c->plan[1], c->specA, kh, 1, tx);
+                gen_mid(g, c->plan[1], c->specA, kh, 1, tx, bytes, st);
                 c->kt.end(KT_MID);
             } else {
                 // very long y lines (four tile buffers do not fit): three launches through specB
                 const int ty = pick_tx(g.Py, 2, 1, &bytes);
                 if (!ty) return fail(c, MM_EUNSUPPORTED, "y line too long for the shared-memory tile");
-                dim3 grid((g.Cx + ty - 1) / ty, 3 * g.Nz);
                 c->kt.begin(KT_FWD_Y);
-                k_gen_y<-1><<<grid, 256, bytes, st>>>(g, c->plan[1], c->specA, c->specB, ty);
+                gen_y(g, c->plan[1], -1, c->specA, c->specB, ty, bytes, st);
                 c->kt.end(KT_FWD_Y);
                 c->kt.begin(KT_MID);
-                dim3 gm((g.Cx + 255) / 256, g.Py);
-                ff::k_mul2d<<<gm, 256, 0, st>>>(g, c->specB, kh);
+                launch_mul2d(g, c->specB, kh, st);
                 c->kt.end(KT_MID);
                 c->kt.begin(KT_INV_Y);
-                k_gen_y<1><<<grid, 256, bytes, st>>>(g, c->plan[1], c->specB, c->specA, ty);
+                gen_y(g, c->plan[1], 1, c->specB, c->specA, ty, bytes, st);
                 c->kt.end(KT_INV_Y);
             }
         } else {
             c->kt.begin(KT_MID);
-            k_gen_mul1d<<<(g.Cx + 127) / 128, 128, 0, st>>>(g, c->specA, kh);
+            gen_mul1d(g, c->specA, kh, st);
             c->kt.end(KT_MID);
         }
     }
@@ -394,10 +379,9 @@ mm_status launch_eval(mm_ctx* c, const EpiParams& ep)
             done = fast_inv_x_h(fp, g, st, c->specA, c->hfield, 1.0f);
             c->kt.end(KT_INV_X);
             if (done) {
-                const size_t quads = ncell(g) / 4;
                 c->kt.begin(KT_EPI);
-                if (ep.geometry) k_epi1<<<(unsigned)((ncell(g) + 255) / 256), 256, 0, st>>>(g, c->hfield, ep);
-                else k_epi4<<<(unsigned)((quads + 255) / 256), 256, 0, st>>>(g, c->hfield, ep);
+                if (ep.geometry) launch_epi1(g, c->hfield, ep, st);
+                else launch_epi4(g, c->hfield, ep, st);
                 c->kt.end(KT_EPI);
             }
         }
@@ -407,9 +391,7 @@ mm_status launch_eval(mm_ctx* c, const EpiParams& ep)
         if (!(ep.demag && !ep.geometry && (c->fast & FAST_INV_X) && fast_inv_x(fp, g, st, c->specA, ep))) {
             const int tx = pick_tx(g.Px, 2, 3, &bytes);
             if (!tx) return fail(c, MM_EUNSUPPORTED, "x line too long for the shared-memory tile");
-            const int npy = (g.Ny + 1) / 2;
-            dim3 grid((npy + tx - 1) / tx, g.Nz);
-            k_gen_inv_x<<<grid, 256, bytes, st>>>(g, c->plan[0], c->specA, ep, tx);
+            gen_inv_x(g, c->plan[0], c->specA, ep, tx, bytes, st);
         }
         c->kt.end(KT_INV_X);
     }
@@ -801,12 +783,8 @@ static mm_status demag_init_impl(mm_ctx* c)
     CUDA_TRY(c, cudaMemset(c->ctl, 0, sizeof(StepCtl)));
     CUDA_TRY(c, cudaMalloc(&c->ctl_scratch, 4 * sizeof(double)));
     CUDA_TRY(c, cudaMalloc(&c->step_dev, sizeof(unsigned long long)));
-    mm_status s;
-    if ((s = set_smem(c, k_gen_fwd_x)) != MM_OK) return s;
-    if ((s = set_smem(c, k_gen_y<-1>)) != MM_OK) return s;
-    if ((s = set_smem(c, k_gen_y<1>)) != MM_OK) return s;
-    if ((s = set_smem(c, k_gen_mid)) != MM_OK) return s;
-    if ((s = set_smem(c, k_gen_inv_x)) != MM_OK) return s;
+    // (status of the set-up steps below)
+    if (!gen_set_smem()) return fail(c, MM_ECUDA, "cannot raise the shared-memory limit of the generic kernels");
     std::string ferr;
     if (!fast_plan_init(c->fp, g, &ferr)) return fail(c, MM_ECUDA, ferr);
     if (c->batch && !((c->fp.ok_x || c->fp.ok_xr) && c->fp.ok_mul2 && g.Nx % 4 == 0))

@@ -191,8 +191,7 @@ mm_status mm_dist_backward(mm_ctx* c, const float* m_slab_dev, const float* halo
         ep.zlo = halo_lo_dev;
         ep.zhi = halo_hi_dev;
         ep.cell0 = (unsigned long long)c->slab.z0 * c->g.Ny * c->g.Nx;
-        const size_t quads = ncell(c->g) / 4;
-        k_epi4<<<(unsigned)((quads + 255) / 256), 256, 0, c->stream>>>(c->g, c->hfield, ep);
+        launch_epi4(c->g, c->hfield, ep, c->stream);
         c->kt.launches += 2;
     }
     CUDA_TRY(c, cudaGetLastError());
