@@ -94,7 +94,11 @@ __device__ __forceinline__ void stv(float* __restrict__ p, const float (&v)[V])
 // Adds anisotropy, Zeeman and thermal fields, forms the torque, does the Runge-Kutta stage combine.
 // All loads come before all stores.  Returns the value to be max-reduced (error norm or
 // |dm/dtau|), 0 when no reduction is asked for.
-template <int V>
+// LEAN: no cubic anisotropy, thermal field, current or per-film field (the caller has checked): those branches and
+// the gradient array D drop out at compile time, which is worth a dozen registers in the streaming kernel.
+// NA >= 0: the number of earlier stage derivatives in the combine is known at compile time (their loads unroll and
+// can be issued early); -1: taken from p.na.
+template <int V, bool LEAN = false, int NA = -1>
 __device__ __forceinline__ float epilogue_finish_v(const EpiParams& p, size_t idx, size_t n, const float (&m)[3][V],
                                                    float (&h)[3][V], const float (&D)[3][V])
 {
@@ -106,7 +110,7 @@ __device__ __forceinline__ float epilogue_finish_v(const EpiParams& p, size_t id
 #pragma unroll
         for (int c = 0; c < 3; ++c) h[c][u] += s * p.u[c] + p.hext[c];
     }
-    if (p.hext_b) {      // one applied field per film of a batch (the V cells lie in one row, hence in one plane)
+    if (!LEAN && p.hext_b) {      // one applied field per film of a batch (the V cells lie in one row, hence in one plane)
         const float* __restrict__ hb = p.hext_b + 3 * (idx / p.plane_cells);
 #pragma unroll
         for (int c = 0; c < 3; ++c) {
@@ -116,7 +120,7 @@ __device__ __forceinline__ float epilogue_finish_v(const EpiParams& p, size_t id
         }
     }
     // ---- cubic anisotropy (Eq. (5), reading A14): h -= sum_i (dE/da_i) c_i ----
-    if (p.cubic) {
+    if (!LEAN && p.cubic) {
 #pragma unroll
         for (int u = 0; u < V; ++u) {
             const float a1 = m[0][u] * p.c1[0] + m[1][u] * p.c1[1] + m[2][u] * p.c1[2];
@@ -131,7 +135,7 @@ __device__ __forceinline__ float epilogue_finish_v(const EpiParams& p, size_t id
         }
     }
     // ---- thermal field (Eq. (6), reading A6) ----
-    if (p.thermal) {
+    if (!LEAN && p.thermal) {
 #pragma unroll
         for (int u = 0; u < V; ++u) {
             float eta[3];
@@ -161,7 +165,7 @@ __device__ __forceinline__ float epilogue_finish_v(const EpiParams& p, size_t id
         cross3(mm_, mxh, mxmxh);
 #pragma unroll
         for (int c = 0; c < 3; ++c) k[c][u] = -p.inv1pa2 * (mxh[c] + p.alpha * mxmxh[c]);
-        if (p.stt) {   // Eq. (7): - c_ad m x (m x D) - c_nad m x D
+        if (!LEAN && p.stt) {   // Eq. (7): - c_ad m x (m x D) - c_nad m x D
             const float DD[3] = { D[0][u], D[1][u], D[2][u] };
             float mxD[3], mxmxD[3];
             cross3(mm_, DD, mxD);
@@ -189,7 +193,8 @@ __device__ __forceinline__ float epilogue_finish_v(const EpiParams& p, size_t id
         for (int c = 0; c < 3; ++c)
 #pragma unroll
             for (int u = 0; u < V; ++u) acc[c][u] = ds * p.a_self * k[c][u];
-        for (int j = 0; j < p.na; ++j) {
+#pragma unroll
+        for (int j = 0; j < (NA >= 0 ? NA : p.na); ++j) {
             const float* __restrict__ kj = p.ka[j];
             const float aj = ds * p.a[j];
 #pragma unroll

@@ -192,7 +192,11 @@ template <int T, int E, bool CONJ>
 __device__ __forceinline__ void apply_twiddles(float2 (&v)[E], const float2* __restrict__ tw, const int t)
 {
 #if !defined(MM_TW_PLAIN)
-    if constexpr (E % 4 == 0 && E >= 16) {
+    constexpr bool SYM = E % 4 == 0 && E >= 16;
+#else
+    constexpr bool SYM = false;
+#endif
+    if constexpr (SYM) {
         auto ld = [&](int k2) { float2 w = __ldg(tw + k2 * T + t); if (CONJ) w.y = -w.y; return w; };
         const float2 d = ld(E / 2);
         const float2 d2 = cmul(d, d);
@@ -207,14 +211,13 @@ __device__ __forceinline__ void apply_twiddles(float2 (&v)[E], const float2* __r
             }
             v[E / 2 + k] = cmul(v[E / 2 + k], cmul(d, w));
         }
-        return;
-    }
-#endif
+    } else {
 #pragma unroll
-    for (int k2 = 1; k2 < E; ++k2) {
-        float2 w = __ldg(tw + k2 * T + t);
-        if (CONJ) w.y = -w.y;
-        v[k2] = cmul(v[k2], w);
+        for (int k2 = 1; k2 < E; ++k2) {
+            float2 w = __ldg(tw + k2 * T + t);
+            if (CONJ) w.y = -w.y;
+            v[k2] = cmul(v[k2], w);
+        }
     }
 }
 

@@ -28,7 +28,11 @@ k_epi1(Geom g, const float* __restrict__ hms, EpiParams ep)
 // cells along x (float4 traffic), takes its x neighbours from the adjacent lanes and the y / z
 // neighbours from the rows above and below.  Needs Nx % 4 == 0.  One quad per thread.
 // ---------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(256, 3)
+#ifndef MM_EPI4_MINB
+#define MM_EPI4_MINB 3
+#endif
+template <bool LEAN, int NA>
+__global__ void __launch_bounds__(256, MM_EPI4_MINB)
 k_epi4(Geom g, const float* __restrict__ hms, EpiParams ep)
 {
     const int nx4 = g.Nx >> 2;
@@ -71,9 +75,9 @@ k_epi4(Geom g, const float* __restrict__ hms, EpiParams ep)
         for (int c = 0; c < 3; ++c) {
             ldv<4>(hms + idx + c * n, h[c]);
 #pragma unroll
-            for (int u = 0; u < 4; ++u) D[c][u] = 0.f;
+            for (int u = 0; u < 4; ++u) if (!LEAN) D[c][u] = 0.f;
         }
-        red = __float_as_uint(epilogue_finish_v<4>(ep, idx, n, m, h, D)) & 0x7fffffffu;
+        red = __float_as_uint(epilogue_finish_v<4, LEAN, NA>(ep, idx, n, m, h, D)) & 0x7fffffffu;
     } else if (active) {
         const int ym = y > 0 ? y - 1 : (g.pery ? g.Ny - 1 : y);
         const int yp = y + 1 < g.Ny ? y + 1 : (g.pery ? 0 : y);
@@ -102,10 +106,10 @@ k_epi4(Geom g, const float* __restrict__ hms, EpiParams ep)
                 h[c][u] += ep.wex[0] * ((xp - mc) + (xm - mc));
                 h[c][u] += ep.wex[1] * ((b[u] - mc) + (a[u] - mc));
                 h[c][u] += ep.wex[2] * ((e[u] - mc) + (d[u] - mc));
-                D[c][u] = ep.cj[0] * (xp - xm) + ep.cj[1] * (b[u] - a[u]) + ep.cj[2] * (e[u] - d[u]);
+                if (!LEAN) D[c][u] = ep.cj[0] * (xp - xm) + ep.cj[1] * (b[u] - a[u]) + ep.cj[2] * (e[u] - d[u]);
             }
         }
-        red = __float_as_uint(epilogue_finish_v<4>(ep, idx, n, m, h, D)) & 0x7fffffffu;
+        red = __float_as_uint(epilogue_finish_v<4, LEAN, NA>(ep, idx, n, m, h, D)) & 0x7fffffffu;
     }
     if (ep.do_err) block_max_atomic(red, ep.maxbits);
 }
@@ -114,7 +118,15 @@ k_epi4(Geom g, const float* __restrict__ hms, EpiParams ep)
 void launch_epi4(const Geom& g, const float* hms, const EpiParams& ep, cudaStream_t st)
 {
     const size_t quads = (size_t)g.Nx * g.Ny * g.Nz / 4;
-    k_epi4<<<(unsigned)((quads + 255) / 256), 256, 0, st>>>(g, hms, ep);
+    // the common case (no cubic anisotropy, thermal field, current, per-film field) has leaner instantiations, with
+    // the number of earlier stage derivatives of the usual stage shapes (0: inner stages, 3: last RK4 stage) fixed
+    const unsigned nb = (unsigned)((quads + 255) / 256);
+    const bool lean = !ep.cubic && !ep.thermal && !ep.stt && !ep.hext_b;
+    const int na = (ep.mode == EPI_STAGE && ep.m_out) ? ep.na : 0;
+    if (lean && na == 0) k_epi4<true, 0><<<nb, 256, 0, st>>>(g, hms, ep);
+    else if (lean && na == 3) k_epi4<true, 3><<<nb, 256, 0, st>>>(g, hms, ep);
+    else if (lean) k_epi4<true, -1><<<nb, 256, 0, st>>>(g, hms, ep);
+    else k_epi4<false, -1><<<nb, 256, 0, st>>>(g, hms, ep);
 }
 
 void launch_epi1(const Geom& g, const float* hms, const EpiParams& ep, cudaStream_t st)
