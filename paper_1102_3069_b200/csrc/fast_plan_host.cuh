@@ -52,6 +52,8 @@ inline bool fast_plan_init(FastPlan& fp, const Geom& g, std::string* err)
     fp.ok_y = g.Py > 1 && (ff::split(g.Py, &T, &E) || fp.y_split);
     fp.ok_mid3 = g.Pz >= 64 && g.Py > 1 && ff::split(g.Pz, &T, &E) && E <= 16;
     fp.ok_mul2 = g.Pz == 1 && fp.ok_y;
+    fp.z_long = g.Pz >= 64 && g.Py > 1 && ff::split(g.Pz, &T, &E) && E > 16 && g.Pz <= 65535;
+    fp.zbuf = nullptr;
     // fp.x_pipe, fp.mid_pipe, fp.chunk_w, fp.nstream come from the context (mm_set_option; defaults set by
     // mm_create).  L2-resident chunks (chunk_w = columns per chunk, multiple of 16) are off by default:
     // measured on B200 at 512x512x64 they give bit-identical results and cut DRAM traffic, but no time,
@@ -81,6 +83,13 @@ inline bool fast_plan_init(FastPlan& fp, const Geom& g, std::string* err)
         return false;
     }
     const int P[3] = { fp.x_split ? 1024 : (fp.ok_xr ? g.Px / 2 : g.Px), fp.y_split ? 1024 : g.Py, g.Pz };
+    if (fp.z_long) {
+        const size_t nz = (size_t)3 * g.Pz * g.Py * g.CxS;
+        if (cudaMalloc(&fp.zbuf, nz * sizeof(float2)) != cudaSuccess || cudaMemset(fp.zbuf, 0, nz * sizeof(float2)) != cudaSuccess) {
+            if (err) *err = "fast plan: z-padded spectrum allocation failed";
+            return false;
+        }
+    }
     if (fp.x_split) {
         const size_t nrow = (size_t)3 * g.Nz * g.Ny;
         std::vector<float2> t4(1025);
@@ -227,6 +236,8 @@ inline void fast_plan_destroy(FastPlan& fp)
     fp.twx = nullptr;
     cudaFree(fp.twl);
     fp.twl = nullptr;
+    cudaFree(fp.zbuf);
+    fp.zbuf = nullptr;
     cudaFree(fp.xs_real); cudaFree(fp.xs_spec); cudaFree(fp.twx4);
     fp.xs_real = nullptr; fp.xs_spec = nullptr; fp.twx4 = nullptr;
     for (int s = 0; s < 4; ++s) {

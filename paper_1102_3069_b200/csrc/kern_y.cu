@@ -7,20 +7,28 @@
 
 namespace mm {
 namespace ff {
+// lines along any strided axis: nplane planes, strides in the ColTile, twiddle table tw of the line length
 template <int T, int E, int SGN, bool PER>
-bool launch_y(const FastPlan& fp, const Geom& g, cudaStream_t st, const ColTile& ct, float2* a, float2* b)
+bool launch_lines(const FastPlan& fp, cudaStream_t st, const ColTile& ct, int nplane, float2* a, float2* b,
+                  const float2* tw)
 {
     const size_t bytes = (size_t)T * (E + 1) * 8 * sizeof(float2);
     static bool oncep[MM_MAX_DEV] = {};
     if (!ensure_smem_dev(k_y_p<T, E, SGN, PER>, bytes, oncep)) return false;
-    const int ntile = ((ct.ncol + 7) / 8) * 3 * g.Nz;
+    const int ntile = ((ct.ncol + 7) / 8) * nplane;
     int per_sm = (int)((227 * 1024) / (bytes + 1024));
     const int cap = 2048 / (8 * T) < ((T == 32) ? 2 : 8) ? 2048 / (8 * T) : ((T == 32) ? 2 : 8);
     if (per_sm > cap) per_sm = cap;
     if (per_sm < 1) per_sm = 1;
     const int grid = ntile < fp.nsm * per_sm ? ntile : fp.nsm * per_sm;
-    k_y_p<T, E, SGN, PER><<<grid, 8 * T, bytes, st>>>(ct, 3 * g.Nz, a, b, fp.tw[1]);
+    k_y_p<T, E, SGN, PER><<<grid, 8 * T, bytes, st>>>(ct, nplane, a, b, tw);
     return true;
+}
+
+template <int T, int E, int SGN, bool PER>
+bool launch_y(const FastPlan& fp, const Geom& g, cudaStream_t st, const ColTile& ct, float2* a, float2* b)
+{
+    return launch_lines<T, E, SGN, PER>(fp, st, ct, 3 * g.Nz, a, b, fp.tw[1]);
 }
 
 #define MM_FF_SIZES(L, CALL)                 \
@@ -128,5 +136,68 @@ bool fast_y(const FastPlan& fp, const Geom& g, cudaStream_t st, int sgn, const f
     return r;
 }
 
+
+
+// ---------------------------------------------------------------------------------------------
+// a3 for z lines that do not fit the fused last-axis kernels (padded z length 384, 512, 768, 1024: a thread cannot hold
+// the line of all three components): the z pass unfused -- forward z transform of each component into a z-padded
+// buffer [3][Pz][Py][CxS] by the y-pass kernel (a line is a line: the strides sit in the ColTile), the K-hat product
+// as an elementwise kernel with the octant's mirror and sign rules, inverse z transform back into the Nz planes.
+// More bytes than the fused kernels (the padded spectrum is materialised), but every pass at streaming speed.
+// ---------------------------------------------------------------------------------------------
+namespace ff {
+__global__ void __launch_bounds__(128)
+k_mul3d(Geom g, float2* __restrict__ spec, const float* __restrict__ khat)
+{
+    const int kx = blockIdx.x * blockDim.x + threadIdx.x;
+    if (kx >= g.Cx) return;
+    const int ky = blockIdx.y, kz = blockIdx.z;
+    int qy = ky, qz = kz;
+    float sy = 1.f, sz = 1.f;
+    if (2 * qy > g.Py) { qy = g.Py - qy; sy = -1.f; }
+    if (2 * qz > g.Pz) { qz = g.Pz - qz; sz = -1.f; }
+    const size_t nC = (size_t)g.CxK * g.Cy * g.Cz;
+    const size_t ko = ((size_t)qz * g.Cy + qy) * g.CxK + kx;
+    const float kxx = __ldg(khat + ko), kyy = __ldg(khat + ko + nC), kzz = __ldg(khat + ko + 2 * nC);
+    const float kxy = sy * __ldg(khat + ko + 3 * nC), kxz = sz * __ldg(khat + ko + 4 * nC);
+    const float kyz = sy * sz * __ldg(khat + ko + 5 * nC);
+    const size_t cs = (size_t)g.Pz * g.Py * g.CxS;
+    float2* p = spec + ((size_t)kz * g.Py + ky) * g.CxS + kx;
+    const float2 mx = p[0], my = p[cs], mz = p[2 * cs];
+    p[0] = make_float2(kxx * mx.x + kxy * my.x + kxz * mz.x, kxx * mx.y + kxy * my.y + kxz * mz.y);
+    p[cs] = make_float2(kxy * mx.x + kyy * my.x + kyz * mz.x, kxy * mx.y + kyy * my.y + kyz * mz.y);
+    p[2 * cs] = make_float2(kxz * mx.x + kyz * my.x + kzz * mz.x, kxz * mx.y + kyz * my.y + kzz * mz.y);
+}
+}  // namespace ff
+
+bool fast_z_long(const FastPlan& fp, const Geom& g, cudaStream_t st, float2* specB, const float* khat)
+{
+    if (!fp.z_long || !fp.zbuf) return false;
+    ff::ColTile ct;
+    ct.kx0 = 0; ct.ncol = g.Cx;
+    ct.a_row = (size_t)g.Py * g.CxS; ct.a_plane = g.CxS;        // a "row" is a z plane, a "plane" a ky row
+    ct.b_row = (size_t)g.Py * g.CxS; ct.b_plane = g.CxS;
+    const size_t ca = (size_t)g.Nz * g.Py * g.CxS, cb = (size_t)g.Pz * g.Py * g.CxS;
+    for (int sgn = -1; sgn <= 1; sgn += 2) {
+        for (int comp = 0; comp < 3; ++comp) {
+            float2* a = specB + comp * ca;
+            float2* b = fp.zbuf + comp * cb;
+            bool r = false;
+#define CALL(T, E)                                                                                           \
+    r = sgn < 0 ? (g.perz ? ff::launch_lines<T, E, -1, true>(fp, st, ct, g.Py, a, b, fp.tw[2])               \
+                          : ff::launch_lines<T, E, -1, false>(fp, st, ct, g.Py, a, b, fp.tw[2]))             \
+                : (g.perz ? ff::launch_lines<T, E, 1, true>(fp, st, ct, g.Py, a, b, fp.tw[2])                \
+                          : ff::launch_lines<T, E, 1, false>(fp, st, ct, g.Py, a, b, fp.tw[2]))
+            MM_FF_SIZES(g.Pz, CALL)
+#undef CALL
+            if (!r) return false;
+        }
+        if (sgn < 0) {
+            dim3 grid((g.Cx + 127) / 128, g.Py, g.Pz);
+            ff::k_mul3d<<<grid, 128, 0, st>>>(g, fp.zbuf, khat);
+        }
+    }
+    return true;
+}
 
 }  // namespace mm

@@ -313,7 +313,7 @@ mm_status launch_eval(mm_ctx* c, const EpiParams& ep)
             }
             {   // a3
                 c->kt.begin(KT_MID);
-                if (!((c->fast & FAST_MID) && fast_mid3(fp, g, st, wt, c->specB, kh))) {
+                if (!((c->fast & FAST_MID) && (fast_mid3(fp, g, st, wt, c->specB, kh) || fast_z_long(fp, g, st, c->specB, kh)))) {
                     const int tx = pick_tx(g.Pz, 4, 1, &bytes);
                     if (!tx) return fail(c, MM_EUNSUPPORTED, "z line too long for the shared-memory tile");
                     gen_mid(g, c->plan[2], c->specB, kh, 2, tx, bytes, st);

@@ -42,6 +42,8 @@ struct FastPlan {
     float* xs_real;                      // x_split: de-interleaved rows [2 nrow][Nx / 2]
     float2* xs_spec;                     // x_split: their half spectra [2 nrow][XS_STRIDE]
     float2* twx4;                        // x_split: exp(-2 pi i j / 4096), j <= 1024
+    bool z_long;                         // z lines too long for the fused last-axis kernels: unfused z pass through zbuf
+    float2* zbuf;                        // z_long: z-padded spectrum [3][Pz][Py][CxS]
     int y_split;                         // y lines of 2048 / 4096: 2 / 4 interleaved transforms of 1024 (else 0)
     float2* twl;                         // y_split: exp(-2 pi i j / Py), j < Py
     int nsm;                             // SM count (persistent grids)
@@ -123,6 +125,7 @@ bool fast_inv_x_h(const FastPlan& fp, const Geom& g, cudaStream_t st, const floa
 bool fast_y(const FastPlan& fp, const Geom& g, cudaStream_t st, int sgn, const ff::ColTile& ct, float2* a, float2* b);
 bool fast_mid3(const FastPlan& fp, const Geom& g, cudaStream_t st, const ff::ColTile& ct, float2* specB,
                const float* khat);
+bool fast_z_long(const FastPlan& fp, const Geom& g, cudaStream_t st, float2* specB, const float* khat);
 bool fast_mul2(const FastPlan& fp, const Geom& g, cudaStream_t st, float2* specB, const float* khat);
 void launch_mul2d(const Geom& g, float2* spec, const float* khat, cudaStream_t st);      // any size
 // ---- per-cell tail of the split last pass ----

@@ -272,6 +272,9 @@ FAST_GRIDS = [
     ((2048, 8, 1), (3e-9, 3e-9, 3e-9), (0, 0, 0)),      # x = 4096: even / odd samples through the 2048-point real transform
     ((4096, 4, 1), (3e-9, 3e-9, 3e-9), (1, 0, 0)),      # x = 4096 periodic (no padding)
     ((2048, 6, 2), (3e-9, 3e-9, 3e-9), (0, 0, 0)),      # x = 4096 in a 3D grid
+    ((32, 16, 256), (3e-9, 3e-9, 3e-9), (0, 0, 0)),     # z = 512: unfused z pass through the z-padded buffer
+    ((16, 20, 192), (3e-9, 3e-9, 3e-9), (0, 0, 0)),     # z = 384 (one factor 3), y generic (40)
+    ((32, 16, 512), (3e-9, 3e-9, 3e-9), (0, 0, 1)),     # z = 512 periodic (no padding)
 ]
 
 
