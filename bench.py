@@ -271,7 +271,7 @@ def run_sweep(args):
     # than 1024^2 on the paper's GPU).  992 = 2^5 * 31 is refused here (only 2^a 3^b 5^c 7^d sizes are accepted,
     # PAPER.md:171); its smooth neighbours 960 = 2^6*3*5, 1000 = 2^3*5^3 and 1008 = 2^4*3^2*7 run on the generic
     # radix-2/3/5/7 kernels and show the same shape next to 1024^2.
-    grids += [(n, n, 1) for n in (960, 1000, 1008)]
+    grids += [(n, n, 1) for n in (896, 960, 1152, 1000, 1008)]
     rows = []
     for g in grids:
         wl = wlm.scaled(wlm.config(5), g)

@@ -39,20 +39,65 @@ inline bool fast_yzy_chunked(FastPlan& fp, const Geom& g, cudaStream_t st, float
 }
 
 
+// P = R * Ls with Ls a length the line kernels take and the smallest R of {2, 3, 4, 5, 7, 9} (largest Ls)
+inline bool choose_split(int P, int* R, int* Ls, bool real_x = false)
+{
+    int T, E;
+    for (int r : { 2, 3, 4, 5, 7, 9 }) {
+        if (P % r != 0) continue;
+        const int ls = P / r;
+        if (ff::split(ls, &T, &E) || (real_x && (ls == 1536 || ls == 2048))) { *R = r; *Ls = ls; return true; }
+    }
+    return false;
+}
+
+inline bool upload(float2** dst, const std::vector<float2>& v)
+{
+    return cudaMalloc(dst, v.size() * sizeof(float2)) == cudaSuccess &&
+           cudaMemcpy(*dst, v.data(), v.size() * sizeof(float2), cudaMemcpyHostToDevice) == cudaSuccess;
+}
+
+inline std::vector<float2> roots_of_unity(int P)          // exp(-2 pi i j / P), j < P
+{
+    std::vector<float2> t((size_t)P);
+    for (int j = 0; j < P; ++j) {
+        const long double ang = -2.0L * 3.14159265358979323846264338327950288L * j / P;
+        t[j] = make_float2((float)cosl(ang), (float)sinl(ang));
+    }
+    return t;
+}
+
 inline bool fast_plan_init(FastPlan& fp, const Geom& g, std::string* err)
 {
     int T, E, dev = 0;
+    // x: a kernel for Px itself (pair-packed rows, or the half-length form for 1536 / 2048), else R interleaved
+    // real transforms of Ls = Px / R (cells per sub-row: Nx / R must be a whole number, even for the half-length form)
     fp.ok_x = ff::split(g.Px, &T, &E);
     fp.ok_xr = !fp.ok_x && (g.Px == 1536 || g.Px == 2048) && g.Nx % 2 == 0;
-    fp.x_split = g.Px == 4096 && g.Nx % 4 == 0 && (size_t)3 * g.Nz * g.Ny <= 65535;      // (rows: grid.y of the combine)
-    fp.xs_real = nullptr; fp.xs_spec = nullptr; fp.twx4 = nullptr;
+    fp.x_R = 1; fp.x_Ls = g.Px; fp.xs_stride = 0;
+    fp.xs_real = nullptr; fp.xs_spec = nullptr; fp.twxl = nullptr;
     fp.twx = nullptr;
-    fp.y_split = (g.Py == 2048 || g.Py == 4096) ? g.Py / 1024 : 0;
-    fp.twl = nullptr;
-    fp.ok_y = g.Py > 1 && (ff::split(g.Py, &T, &E) || fp.y_split);
+    if (!fp.ok_x && !fp.ok_xr) {
+        int R, Ls;
+        if (choose_split(g.Px, &R, &Ls, true) && g.Nx % R == 0 && (g.Nx / R) % 4 == 0 && g.Nx % 4 == 0) {
+            fp.x_R = R; fp.x_Ls = Ls; fp.xs_stride = (Ls / 2 + 1 + 7) & ~7;
+        }
+    }
+    // y and z lines
+    for (int a = 1; a < 3; ++a) {
+        const int P = a == 1 ? g.Py : g.Pz;
+        fp.ax[a].R = 1; fp.ax[a].Ls = P; fp.ax[a].tw = nullptr; fp.ax[a].twl = nullptr;
+        if (P > 1 && !ff::split(P, &T, &E)) {
+            int R, Ls;
+            if (choose_split(P, &R, &Ls)) { fp.ax[a].R = R; fp.ax[a].Ls = Ls; }
+            else fp.ax[a].R = 0;                 // no size-specialised path along this axis
+        }
+    }
+    fp.ax[0] = fp.ax[1];
+    fp.ok_y = g.Py > 1 && fp.ax[1].R >= 1;
     fp.ok_mid3 = g.Pz >= 64 && g.Py > 1 && ff::split(g.Pz, &T, &E) && E <= 16;
     fp.ok_mul2 = g.Pz == 1 && fp.ok_y;
-    fp.z_long = g.Pz >= 64 && g.Py > 1 && ff::split(g.Pz, &T, &E) && E > 16 && g.Pz <= 65535;
+    fp.z_long = !fp.ok_mid3 && g.Pz >= 32 && g.Py > 1 && fp.ax[2].R >= 1 && g.Pz <= 65535 && g.Py <= 65535;
     fp.zbuf = nullptr;
     // fp.x_pipe, fp.mid_pipe, fp.chunk_w, fp.nstream come from the context (mm_set_option; defaults set by
     // mm_create).  L2-resident chunks (chunk_w = columns per chunk, multiple of 16) are off by default:
@@ -82,7 +127,6 @@ inline bool fast_plan_init(FastPlan& fp, const Geom& g, std::string* err)
         if (err) *err = "fast plan: cannot read the SM count of the current device";
         return false;
     }
-    const int P[3] = { fp.x_split ? 1024 : (fp.ok_xr ? g.Px / 2 : g.Px), fp.y_split ? 1024 : g.Py, g.Pz };
     if (fp.z_long) {
         const size_t nz = (size_t)3 * g.Pz * g.Py * g.CxS;
         if (cudaMalloc(&fp.zbuf, nz * sizeof(float2)) != cudaSuccess || cudaMemset(fp.zbuf, 0, nz * sizeof(float2)) != cudaSuccess) {
@@ -90,61 +134,50 @@ inline bool fast_plan_init(FastPlan& fp, const Geom& g, std::string* err)
             return false;
         }
     }
-    if (fp.x_split) {
-        const size_t nrow = (size_t)3 * g.Nz * g.Ny;
-        std::vector<float2> t4(1025);
-        for (int j = 0; j <= 1024; ++j) {
-            const long double ang = -2.0L * 3.14159265358979323846264338327950288L * j / 4096.0L;
-            t4[j] = make_float2((float)cosl(ang), (float)sinl(ang));
-        }
+    if (fp.x_R > 1) {
+        const size_t nrow = (size_t)3 * g.Nz * g.Ny, ns = nrow * fp.x_R * fp.xs_stride;
         if (cudaMalloc(&fp.xs_real, nrow * g.Nx * sizeof(float)) != cudaSuccess ||
-            cudaMalloc(&fp.xs_spec, 2 * nrow * MM_XS_STRIDE * sizeof(float2)) != cudaSuccess ||
-            cudaMemset(fp.xs_spec, 0, 2 * nrow * MM_XS_STRIDE * sizeof(float2)) != cudaSuccess ||
-            cudaMalloc(&fp.twx4, t4.size() * sizeof(float2)) != cudaSuccess ||
-            cudaMemcpy(fp.twx4, t4.data(), t4.size() * sizeof(float2), cudaMemcpyHostToDevice) != cudaSuccess) {
+            cudaMalloc(&fp.xs_spec, ns * sizeof(float2)) != cudaSuccess ||
+            cudaMemset(fp.xs_spec, 0, ns * sizeof(float2)) != cudaSuccess || !upload(&fp.twxl, roots_of_unity(g.Px))) {
             if (err) *err = "fast plan: x-split workspace allocation failed";
             return false;
         }
     }
-    if (fp.y_split) {
-        std::vector<float2> tl((size_t)g.Py);
-        for (int j = 0; j < g.Py; ++j) {
-            const long double ang = -2.0L * 3.14159265358979323846264338327950288L * j / g.Py;
-            tl[j] = make_float2((float)cosl(ang), (float)sinl(ang));
-        }
-        if (cudaMalloc(&fp.twl, tl.size() * sizeof(float2)) != cudaSuccess ||
-            cudaMemcpy(fp.twl, tl.data(), tl.size() * sizeof(float2), cudaMemcpyHostToDevice) != cudaSuccess) {
+    for (int a = 1; a < 3; ++a)
+        if (fp.ax[a].R > 1 && !upload(&fp.ax[a].twl, roots_of_unity(a == 1 ? g.Py : g.Pz))) {
             if (err) *err = "fast plan: twiddle table allocation failed";
             return false;
         }
-    }
-    if (fp.ok_xr || fp.x_split) {
-        const int Lc = fp.x_split ? 1024 : g.Px / 2;
+    // the kernels' own tables are those of the length they transform: the sub-length where a line is split
+    const int xin = fp.x_R > 1 ? fp.x_Ls : g.Px;                       // length of the real transform the x kernels run
+    const bool x_half = !ff::split(xin, &T, &E) && (xin == 1536 || xin == 2048);
+    const int P[3] = { x_half ? xin / 2 : xin, fp.ax[1].R >= 1 ? fp.ax[1].Ls : 0, fp.ax[2].R >= 1 ? fp.ax[2].Ls : 0 };
+    if (x_half) {
+        const int Lc = xin / 2;
         std::vector<float2> tx((size_t)Lc);
         for (int k = 0; k < Lc; ++k) {
             const long double ang = -3.14159265358979323846264338327950288L * k / Lc;
             tx[k] = make_float2((float)cosl(ang), (float)sinl(ang));
         }
-        if (cudaMalloc(&fp.twx, tx.size() * sizeof(float2)) != cudaSuccess ||
-            cudaMemcpy(fp.twx, tx.data(), tx.size() * sizeof(float2), cudaMemcpyHostToDevice) != cudaSuccess) {
+        if (!upload(&fp.twx, tx)) {
             if (err) *err = "fast plan: twiddle table allocation failed";
             return false;
         }
     }
     for (int a = 0; a < 3; ++a) {
         fp.tw[a] = nullptr;
-        if (!ff::split(P[a], &T, &E)) continue;
+        if (P[a] < 2 || !ff::split(P[a], &T, &E)) continue;
         std::vector<float2> tw((size_t)P[a]);
         for (int k2 = 0; k2 < E; ++k2)
             for (int t = 0; t < T; ++t) {
                 const long double ang = -2.0L * 3.14159265358979323846264338327950288L * ((long long)t * k2 % P[a]) / P[a];
                 tw[(size_t)k2 * T + t] = make_float2((float)cosl(ang), (float)sinl(ang));
             }
-        if (cudaMalloc(&fp.tw[a], tw.size() * sizeof(float2)) != cudaSuccess ||
-            cudaMemcpy(fp.tw[a], tw.data(), tw.size() * sizeof(float2), cudaMemcpyHostToDevice) != cudaSuccess) {
+        if (!upload(&fp.tw[a], tw)) {
             if (err) *err = "fast plan: twiddle table allocation failed";
             return false;
         }
+        if (a > 0) fp.ax[a].tw = fp.tw[a];
     }
     return true;
 }
@@ -234,12 +267,11 @@ inline void fast_plan_destroy(FastPlan& fp)
     for (int a = 0; a < 3; ++a) { cudaFree(fp.tw[a]); fp.tw[a] = nullptr; }
     cudaFree(fp.twx);
     fp.twx = nullptr;
-    cudaFree(fp.twl);
-    fp.twl = nullptr;
+    for (int a = 1; a < 3; ++a) { cudaFree(fp.ax[a].twl); fp.ax[a].twl = nullptr; fp.ax[a].tw = nullptr; }
     cudaFree(fp.zbuf);
     fp.zbuf = nullptr;
-    cudaFree(fp.xs_real); cudaFree(fp.xs_spec); cudaFree(fp.twx4);
-    fp.xs_real = nullptr; fp.xs_spec = nullptr; fp.twx4 = nullptr;
+    cudaFree(fp.xs_real); cudaFree(fp.xs_spec); cudaFree(fp.twxl);
+    fp.xs_real = nullptr; fp.xs_spec = nullptr; fp.twxl = nullptr;
     for (int s = 0; s < 4; ++s) {
         if (fp.stream[s]) cudaStreamDestroy(fp.stream[s]);
         if (fp.ev_join[s]) cudaEventDestroy(fp.ev_join[s]);

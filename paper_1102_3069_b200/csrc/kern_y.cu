@@ -25,12 +25,6 @@ bool launch_lines(const FastPlan& fp, cudaStream_t st, const ColTile& ct, int np
     return true;
 }
 
-template <int T, int E, int SGN, bool PER>
-bool launch_y(const FastPlan& fp, const Geom& g, cudaStream_t st, const ColTile& ct, float2* a, float2* b)
-{
-    return launch_lines<T, E, SGN, PER>(fp, st, ct, 3 * g.Nz, a, b, fp.tw[1]);
-}
-
 #define MM_FF_SIZES(L, CALL)                 \
     switch (L) {                              \
     case 32: { CALL(4, 8); } break;           \
@@ -47,96 +41,122 @@ bool launch_y(const FastPlan& fp, const Geom& g, cudaStream_t st, const ColTile&
 }  // namespace ff
 
 // ---------------------------------------------------------------------------------------------
-// Long y lines (Py = R * 1024, R = 2 or 4; the paper's Table 1 goes to 1024^2 and 2048^2 cells):
-// one decimation-in-time level outside the size-specialised kernel.  Rows n = R r + q form R interleaved
-// sequences; each is transformed by the 1024-point kernel with a row stride of R (the ColTile strides carry it,
-// the kernel is unchanged: a zero-padded line of Py has zero-padded sub-sequences of 1024), sub-spectrum S_q
-// landing in rows q * 1024 + k of the spectrum.  k_y_combine then forms, in place and per (plane, k, column),
-//   forward:  X[k + 1024 m] = sum_q w_R^(q m) (w_Py^(q k) S_q[k])
-//   inverse:  Y_q[k] = w_Py^(-q k) sum_m w_R^(-q m) X[k + 1024 m]      (before the R inverse transforms)
+// Lines whose length P has no kernel of its own but factors as P = R * Ls with Ls a size-specialised length and
+// R in {2, 3, 4, 5, 7, 9} -- long lines (2048, 4096; the paper's Table 1 goes to 2048^2 cells) and
+// the lengths 2^n * {5, 7, 9} of PAPER.md:171: one decimation-in-time level outside the kernel.  Rows n = R r + q form
+// R interleaved sequences; each is transformed by the Ls-point kernel with a row stride of R (the ColTile strides
+// carry it, the kernel is unchanged: a zero-padded line has zero-padded sub-sequences), sub-spectrum S_q landing in
+// rows q * Ls + k.  k_lines_combine then forms, in place and per (plane, k, column), with w = exp(-2 pi i / P):
+//   forward:  X[k + Ls m] = sum_q w^(q (k + Ls m)) S_q[k]
+//   inverse:  Y_q[k] = sum_m conj(w^(q (k + Ls m))) X[k + Ls m]      (before the R inverse transforms)
 // ---------------------------------------------------------------------------------------------
 namespace ff {
 template <int R, int SGN>
 __global__ void __launch_bounds__(128)
-k_y_combine(ColTile ct, int nplane, int Ls, float2* __restrict__ b, const float2* __restrict__ twl)
+k_lines_combine(ColTile ct, int nplane, int Ls, int P, float2* __restrict__ b, const float2* __restrict__ twl)
 {
-    const int col = blockIdx.x * blockDim.x + threadIdx.x;
+    __shared__ float2 W[R * R];                  // W[q * R + m] = w^(q (k + Ls m)), conjugated for the inverse
     const int k = blockIdx.y, cz = blockIdx.z;
+    if ((int)threadIdx.x < R * R) {
+        const int q = threadIdx.x / R, m = threadIdx.x - q * R;
+        float2 w = __ldg(twl + (int)(((long long)q * (k + (long long)m * Ls)) % P));
+        if (SGN > 0) w.y = -w.y;
+        W[threadIdx.x] = w;
+    }
+    __syncthreads();
+    const int col = blockIdx.x * blockDim.x + threadIdx.x;
     if (col >= ct.ncol || cz >= nplane) return;
     float2* p = b + (size_t)cz * ct.b_plane + (size_t)k * ct.b_row + col;
     const size_t rs = (size_t)Ls * ct.b_row;
-    float2 v[R];
+    float2 v[R], o[R];
 #pragma unroll
     for (int q = 0; q < R; ++q) v[q] = p[q * rs];
-    auto tw = [&](int q) {                       // w_Py^(q k), conjugated for the inverse
-        float2 w = __ldg(twl + q * k);
-        if (SGN > 0) w.y = -w.y;
-        return w;
-    };
-    if (SGN < 0) {
+    if constexpr (R == 2 || R == 4) {
+        // w^(q (k + Ls m)) = w^(q k) w_R^(q m): twiddle by w^(q k) = W[q * R] (m = 0), then a radix-R butterfly
+        if (SGN < 0) {
 #pragma unroll
-        for (int q = 1; q < R; ++q) v[q] = cmul(v[q], tw(q));
-    }
-    if constexpr (R == 2) {
-        const float2 a0 = cadd(v[0], v[1]), a1 = csub(v[0], v[1]);
-        v[0] = a0; v[1] = a1;
+            for (int q = 1; q < R; ++q) v[q] = cmul(v[q], W[q * R]);
+        }
+        if constexpr (R == 2) {
+            o[0] = cadd(v[0], v[1]); o[1] = csub(v[0], v[1]);
+        } else {
+            const float2 s02 = cadd(v[0], v[2]), d02 = csub(v[0], v[2]);
+            const float2 s13 = cadd(v[1], v[3]), d13 = cmuli<SGN>(csub(v[1], v[3]));
+            o[0] = cadd(s02, s13); o[2] = csub(s02, s13);
+            o[1] = cadd(d02, d13); o[3] = csub(d02, d13);
+        }
+        if (SGN > 0) {
+#pragma unroll
+            for (int q = 1; q < R; ++q) o[q] = cmul(o[q], W[q * R]);
+        }
     } else {
-        const float2 s02 = cadd(v[0], v[2]), d02 = csub(v[0], v[2]);
-        const float2 s13 = cadd(v[1], v[3]), d13 = cmuli<SGN>(csub(v[1], v[3]));
-        v[0] = cadd(s02, s13); v[2] = csub(s02, s13);
-        v[1] = cadd(d02, d13); v[3] = csub(d02, d13);
-    }
-    if (SGN > 0) {
 #pragma unroll
-        for (int q = 1; q < R; ++q) v[q] = cmul(v[q], tw(q));
+        for (int u = 0; u < R; ++u) {
+            float2 acc = make_float2(0.f, 0.f);
+#pragma unroll
+            for (int q = 0; q < R; ++q) {
+                // forward: output m = u sums over q; inverse: output q = u sums over m
+                const float2 w = SGN < 0 ? W[q * R + u] : W[u * R + q];
+                acc.x = fmaf(w.x, v[q].x, fmaf(-w.y, v[q].y, acc.x));
+                acc.y = fmaf(w.x, v[q].y, fmaf(w.y, v[q].x, acc.y));
+            }
+            o[u] = acc;
+        }
     }
 #pragma unroll
-    for (int q = 0; q < R; ++q) p[q * rs] = v[q];
+    for (int q = 0; q < R; ++q) p[q * rs] = o[q];
+}
+
+template <int SGN>
+inline void launch_lines_combine(cudaStream_t st, dim3 cg, const ColTile& ct, int nplane, int R, int Ls, int P, float2* b,
+                                 const float2* twl)
+{
+    switch (R) {
+    case 2: k_lines_combine<2, SGN><<<cg, 128, 0, st>>>(ct, nplane, Ls, P, b, twl); break;
+    case 3: k_lines_combine<3, SGN><<<cg, 128, 0, st>>>(ct, nplane, Ls, P, b, twl); break;
+    case 4: k_lines_combine<4, SGN><<<cg, 128, 0, st>>>(ct, nplane, Ls, P, b, twl); break;
+    case 5: k_lines_combine<5, SGN><<<cg, 128, 0, st>>>(ct, nplane, Ls, P, b, twl); break;
+    case 7: k_lines_combine<7, SGN><<<cg, 128, 0, st>>>(ct, nplane, Ls, P, b, twl); break;
+    case 9: k_lines_combine<9, SGN><<<cg, 128, 0, st>>>(ct, nplane, Ls, P, b, twl); break;
+    default: break;
+    }
 }
 }  // namespace ff
 
-template <int R>
-bool fast_y_long(const FastPlan& fp, const Geom& g, cudaStream_t st, int sgn, const ff::ColTile& ct, float2* a,
-                        float2* b)
+// lines of length P along a strided axis: directly, or as R interleaved transforms of Ls = P / R plus the combine
+bool fast_lines(const FastPlan& fp, cudaStream_t st, int sgn, bool per, const ff::ColTile& ct, int nplane, float2* a,
+                float2* b, int P, const AxisPlan& ap)
 {
-    constexpr int Ls = 1024;
-    const int nplane = 3 * g.Nz;
+    auto sub = [&](int L, const ff::ColTile& c2, float2* a2, float2* b2) {
+        bool r = false;
+#define CALL(T, E)                                                                                   \
+    r = sgn < 0 ? (per ? ff::launch_lines<T, E, -1, true>(fp, st, c2, nplane, a2, b2, ap.tw)          \
+                       : ff::launch_lines<T, E, -1, false>(fp, st, c2, nplane, a2, b2, ap.tw))        \
+                : (per ? ff::launch_lines<T, E, 1, true>(fp, st, c2, nplane, a2, b2, ap.tw)           \
+                       : ff::launch_lines<T, E, 1, false>(fp, st, c2, nplane, a2, b2, ap.tw))
+        MM_FF_SIZES(L, CALL)
+#undef CALL
+        return r;
+    };
+    if (ap.R <= 1) return sub(P, ct, a, b);
+    const int R = ap.R, Ls = ap.Ls;
     dim3 cg((ct.ncol + 127) / 128, Ls, nplane);
-    if (sgn > 0) ff::k_y_combine<R, 1><<<cg, 128, 0, st>>>(ct, nplane, Ls, b, fp.twl);
+    if (sgn > 0) ff::launch_lines_combine<1>(st, cg, ct, nplane, R, Ls, P, b, ap.twl);
     for (int q = 0; q < R; ++q) {
         ff::ColTile cq = ct;
         cq.a_row = ct.a_row * R;
-        float2* aq = a + (size_t)q * ct.a_row;
-        float2* bq = b + (size_t)q * Ls * ct.b_row;
-        const bool ok = sgn < 0 ? (g.pery ? ff::launch_y<32, 32, -1, true>(fp, g, st, cq, aq, bq)
-                                          : ff::launch_y<32, 32, -1, false>(fp, g, st, cq, aq, bq))
-                                : (g.pery ? ff::launch_y<32, 32, 1, true>(fp, g, st, cq, aq, bq)
-                                          : ff::launch_y<32, 32, 1, false>(fp, g, st, cq, aq, bq));
-        if (!ok) return false;
+        if (!sub(Ls, cq, a + (size_t)q * ct.a_row, b + (size_t)q * Ls * ct.b_row)) return false;
     }
-    if (sgn < 0) ff::k_y_combine<R, -1><<<cg, 128, 0, st>>>(ct, nplane, Ls, b, fp.twl);
+    if (sgn < 0) ff::launch_lines_combine<-1>(st, cg, ct, nplane, R, Ls, P, b, ap.twl);
     return true;
 }
 
 // sgn < 0: specA rows y < Ny -> specB rows ky < Py; sgn > 0: back.  a, b point at column ct.kx0.
-bool fast_y(const FastPlan& fp, const Geom& g, cudaStream_t st, int sgn, const ff::ColTile& ct, float2* a,
-                   float2* b)
+bool fast_y(const FastPlan& fp, const Geom& g, cudaStream_t st, int sgn, const ff::ColTile& ct, float2* a, float2* b)
 {
     if (!fp.ok_y) return false;
-    if (fp.y_split == 2) return fast_y_long<2>(fp, g, st, sgn, ct, a, b);
-    if (fp.y_split == 4) return fast_y_long<4>(fp, g, st, sgn, ct, a, b);
-    bool r = false;
-#define CALL(T, E)                                                                         \
-    r = sgn < 0 ? (g.pery ? ff::launch_y<T, E, -1, true>(fp, g, st, ct, a, b)              \
-                          : ff::launch_y<T, E, -1, false>(fp, g, st, ct, a, b))            \
-                : (g.pery ? ff::launch_y<T, E, 1, true>(fp, g, st, ct, a, b)               \
-                          : ff::launch_y<T, E, 1, false>(fp, g, st, ct, a, b))
-    MM_FF_SIZES(g.Py, CALL)
-#undef CALL
-    return r;
+    return fast_lines(fp, st, sgn, g.pery != 0, ct, 3 * g.Nz, a, b, g.Py, fp.ax[1]);
 }
-
-
 
 // ---------------------------------------------------------------------------------------------
 // a3 for z lines that do not fit the fused last-axis kernels (padded z length 384, 512, 768, 1024: a thread cannot hold
@@ -179,19 +199,9 @@ bool fast_z_long(const FastPlan& fp, const Geom& g, cudaStream_t st, float2* spe
     ct.b_row = (size_t)g.Py * g.CxS; ct.b_plane = g.CxS;
     const size_t ca = (size_t)g.Nz * g.Py * g.CxS, cb = (size_t)g.Pz * g.Py * g.CxS;
     for (int sgn = -1; sgn <= 1; sgn += 2) {
-        for (int comp = 0; comp < 3; ++comp) {
-            float2* a = specB + comp * ca;
-            float2* b = fp.zbuf + comp * cb;
-            bool r = false;
-#define CALL(T, E)                                                                                           \
-    r = sgn < 0 ? (g.perz ? ff::launch_lines<T, E, -1, true>(fp, st, ct, g.Py, a, b, fp.tw[2])               \
-                          : ff::launch_lines<T, E, -1, false>(fp, st, ct, g.Py, a, b, fp.tw[2]))             \
-                : (g.perz ? ff::launch_lines<T, E, 1, true>(fp, st, ct, g.Py, a, b, fp.tw[2])                \
-                          : ff::launch_lines<T, E, 1, false>(fp, st, ct, g.Py, a, b, fp.tw[2]))
-            MM_FF_SIZES(g.Pz, CALL)
-#undef CALL
-            if (!r) return false;
-        }
+        for (int comp = 0; comp < 3; ++comp)
+            if (!fast_lines(fp, st, sgn, g.perz != 0, ct, g.Py, specB + comp * ca, fp.zbuf + comp * cb, g.Pz, fp.ax[2]))
+                return false;
         if (sgn < 0) {
             dim3 grid((g.Cx + 127) / 128, g.Py, g.Pz);
             ff::k_mul3d<<<grid, 128, 0, st>>>(g, fp.zbuf, khat);

@@ -369,7 +369,7 @@ mm_status launch_eval(mm_ctx* c, const EpiParams& ep)
     }
     // a5-a10
     bool done = false;
-    if (ep.demag && (c->fast & FAST_SPLIT) && (fp.ok_x || fp.ok_xr || fp.x_split) && (g.Nx % 4 == 0 || ep.geometry)) {
+    if (ep.demag && (c->fast & FAST_SPLIT) && (fp.ok_x || fp.ok_xr || fp.x_R > 1) && (g.Nx % 4 == 0 || ep.geometry)) {
         // split variant: inverse x pass -> H_ms field, then the streaming per-cell tail
         c->kt.begin(KT_INV_X);
         if (ep.mode == EPI_HMS) {

@@ -33,19 +33,25 @@ struct ColTile {
 
 enum FastBits { FAST_FWD_X = 1, FAST_Y = 2, FAST_MID = 4, FAST_INV_X = 8, FAST_SPLIT = 16, FAST_CHUNK = 32, FAST_ALL = 63 };
 
+// a line length P handled directly (R = 1, Ls = P) or as R interleaved transforms of Ls = P / R plus a combine
+struct AxisPlan {
+    int R, Ls;
+    const float2* tw;                    // twiddles of the Ls-point kernel, tw[k2 * T + t]
+    float2* twl;                         // R > 1: exp(-2 pi i j / P), j < P
+};
+
 struct FastPlan {
     bool ok_x, ok_y, ok_mid3, ok_mul2;   // which passes have a size-specialised kernel for this grid
     bool ok_xr;                          // x passes through the half-length complex transform (Px = 1536, 2048)
     float2* twx;                         // ok_xr: exp(-i pi k / Lc), k < Lc = Px / 2
     float2* tw[3];                       // per axis: tw[k2 * T + t] = exp(-2 pi i t k2 / L)
-    bool x_split;                        // Px = 4096: even / odd samples through the 2048-point real transform + combine
-    float* xs_real;                      // x_split: de-interleaved rows [2 nrow][Nx / 2]
-    float2* xs_spec;                     // x_split: their half spectra [2 nrow][XS_STRIDE]
-    float2* twx4;                        // x_split: exp(-2 pi i j / 4096), j <= 1024
+    int x_R, x_Ls, xs_stride;            // x lines as x_R interleaved real transforms of x_Ls = Px / x_R (x_R <= 1: direct)
+    float* xs_real;                      // x_R > 1: de-interleaved rows [x_R nrow][Nx / x_R]
+    float2* xs_spec;                     // x_R > 1: their half spectra [x_R nrow][xs_stride]
+    float2* twxl;                        // x_R > 1: exp(-2 pi i j / Px), j < Px
     bool z_long;                         // z lines too long for the fused last-axis kernels: unfused z pass through zbuf
     float2* zbuf;                        // z_long: z-padded spectrum [3][Pz][Py][CxS]
-    int y_split;                         // y lines of 2048 / 4096: 2 / 4 interleaved transforms of 1024 (else 0)
-    float2* twl;                         // y_split: exp(-2 pi i j / Py), j < Py
+    AxisPlan ax[3];                      // lines along y ([1]) and z ([2]): direct or R interleaved sub-transforms
     int nsm;                             // SM count (persistent grids)
     int x_pipe;                          // x passes, cp.async-pipelined forms: bit 0 forward (default), bit 1 inverse (option "x_pipe")
     int mid_pipe;                        // last-axis pass: persistent pipelined kernel (option "mid_pipe")
@@ -99,14 +105,6 @@ inline bool ensure_smem_dev(K kern, size_t bytes, bool (&done)[MM_MAX_DEV])
 }
 }  // namespace ff
 
-#define MM_XS_STRIDE 1032
-inline Geom x_split_geom(const Geom& g)
-{
-    Geom h = g;
-    h.Nx = g.Nx / 2; h.Ny = 2 * g.Ny; h.Px = g.Px / 2; h.Cx = h.Px / 2 + 1; h.CxS = MM_XS_STRIDE;
-    return h;
-}
-
 // the whole-array tile: every column, strides of mm_common.cuh
 inline ff::ColTile whole_tile(const Geom& g)
 {
@@ -122,6 +120,8 @@ inline ff::ColTile whole_tile(const Geom& g)
 bool fast_fwd_x(const FastPlan& fp, const Geom& g, cudaStream_t st, const float* m, float2* specA);
 bool fast_inv_x(const FastPlan& fp, const Geom& g, cudaStream_t st, const float2* specA, const EpiParams& ep);
 bool fast_inv_x_h(const FastPlan& fp, const Geom& g, cudaStream_t st, const float2* specA, float* out, float scale);
+bool fast_lines(const FastPlan& fp, cudaStream_t st, int sgn, bool per, const ff::ColTile& ct, int nplane, float2* a,
+                float2* b, int P, const AxisPlan& ap);
 bool fast_y(const FastPlan& fp, const Geom& g, cudaStream_t st, int sgn, const ff::ColTile& ct, float2* a, float2* b);
 bool fast_mid3(const FastPlan& fp, const Geom& g, cudaStream_t st, const ff::ColTile& ct, float2* specB,
                const float* khat);

@@ -275,6 +275,16 @@ FAST_GRIDS = [
     ((32, 16, 256), (3e-9, 3e-9, 3e-9), (0, 0, 0)),     # z = 512: unfused z pass through the z-padded buffer
     ((16, 20, 192), (3e-9, 3e-9, 3e-9), (0, 0, 0)),     # z = 384 (one factor 3), y generic (40)
     ((32, 16, 512), (3e-9, 3e-9, 3e-9), (0, 0, 1)),     # z = 512 periodic (no padding)
+    # lengths 2^n * {5, 7, 9} and 3 * 2^n beyond the kernels' own: R interleaved transforms + combine
+    ((16, 960, 1), (3e-9, 3e-9, 3e-9), (0, 0, 0)),      # y = 1920 = 5 * 384
+    ((16, 448, 1), (3e-9, 3e-9, 3e-9), (0, 0, 0)),      # y = 896 = 7 * 128
+    ((16, 576, 2), (3e-9, 3e-9, 3e-9), (0, 0, 0)),      # y = 1152 = 9 * 128, 3D
+    ((960, 16, 1), (3e-9, 3e-9, 3e-9), (0, 0, 0)),      # x = 1920 = 5 * 384 (pair-packed sub-rows)
+    ((448, 8, 1), (3e-9, 3e-9, 3e-9), (0, 0, 0)),       # x = 896 = 7 * 128
+    ((640, 8, 1), (3e-9, 3e-9, 3e-9), (1, 0, 0)),       # x = 640 = 5 * 128 periodic
+    ((1536, 8, 1), (3e-9, 3e-9, 3e-9), (0, 0, 0)),      # x = 3072 = 2 * 1536 (half-length sub-transform)
+    ((16, 16, 80), (3e-9, 3e-9, 3e-9), (0, 0, 0)),      # z = 160 = 5 * 32, unfused z pass
+    ((320, 160, 1), (3e-9, 3e-9, 3e-9), (0, 0, 0)),     # 640 x 320 = 5 * 128, 5 * 64: both axes split
 ]
 
 
