@@ -119,12 +119,15 @@ void launch_epi4(const Geom& g, const float* hms, const EpiParams& ep, cudaStrea
 {
     const size_t quads = (size_t)g.Nx * g.Ny * g.Nz / 4;
     // the common case (no cubic anisotropy, thermal field, current, per-film field) has leaner instantiations, with
-    // the number of earlier stage derivatives of the usual stage shapes (0: inner stages, 3: last RK4 stage) fixed
+    // the number of earlier stage derivatives fixed for the usual stage shapes (RK4: 0, 0, 0, 3; Dormand-Prince: 0 ... 4)
     const unsigned nb = (unsigned)((quads + 255) / 256);
     const bool lean = !ep.cubic && !ep.thermal && !ep.stt && !ep.hext_b;
     const int na = (ep.mode == EPI_STAGE && ep.m_out) ? ep.na : 0;
     if (lean && na == 0) k_epi4<true, 0><<<nb, 256, 0, st>>>(g, hms, ep);
+    else if (lean && na == 1) k_epi4<true, 1><<<nb, 256, 0, st>>>(g, hms, ep);
+    else if (lean && na == 2) k_epi4<true, 2><<<nb, 256, 0, st>>>(g, hms, ep);
     else if (lean && na == 3) k_epi4<true, 3><<<nb, 256, 0, st>>>(g, hms, ep);
+    else if (lean && na == 4) k_epi4<true, 4><<<nb, 256, 0, st>>>(g, hms, ep);
     else if (lean) k_epi4<true, -1><<<nb, 256, 0, st>>>(g, hms, ep);
     else k_epi4<false, -1><<<nb, 256, 0, st>>>(g, hms, ep);
 }
