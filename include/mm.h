@@ -342,6 +342,20 @@ mm_status mm_dist_backward(mm_ctx* ctx, const float* m_slab_dev, const float* ha
                            const float* halo_hi_dev, float* out_slab_dev, int what, uint64_t step,
                            double dt_for_thermal);
 
+/* Time stepping on slabs: stage `stage` (0-based) of a fixed-step method (MM_RK1, MM_RK2, MM_RK3, MM_RK4) runs like an
+ * evaluation -- mm_dist_forward on the stage's input state, the two all-to-alls around mm_dist_mid, the halo exchange of
+ * that same state -- and ends with mm_dist_backward_stage instead of mm_dist_backward: a4, a5 and the per-cell tail with
+ * the Runge-Kutta stage combine (a9), which writes the next stage's input into a buffer of the context, or, at the last
+ * stage, the new normalised state into m_slab_dev.
+ *   mm_dist_stage_input   *in_dev_out = the device field stage `stage` acts on (m_slab_dev for stage 0): the caller
+ *                         passes it to mm_dist_forward and takes the halo planes from it.
+ * The thermal draw is per global cell and step (reading A6).  Step control (embedded methods) is not offered on
+ * slabs: its max-norm would need a reduction over the ranks.  Errors: MM_EINVAL for any other method. */
+mm_status mm_dist_stage_input(mm_ctx* ctx, mm_method method, int stage, const float* m_slab_dev,
+                              const float** in_dev_out);
+mm_status mm_dist_backward_stage(mm_ctx* ctx, float* m_slab_dev, mm_method method, int stage, double dt,
+                                 uint64_t step, const float* halo_lo_dev, const float* halo_hi_dev);
+
 /* mm_last_error -- message for the last non-OK status of this context ("" if none); for a NULL ctx
  * the message of the last failed mm_create on this thread. */
 const char* mm_last_error(const mm_ctx* ctx);

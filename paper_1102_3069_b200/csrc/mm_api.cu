@@ -490,8 +490,8 @@ __global__ void k_copy4(const float4* __restrict__ src, float4* __restrict__ dst
 }
 
 // One stage of `tab` (0-based s).  Enqueues only.
-mm_status run_stage(mm_ctx* c, float* m_dev, const Tableau& tab, int s, double dt, uint64_t step,
-                    bool adaptive_target, bool dev_dt = false)
+EpiParams stage_params(mm_ctx* c, float* m_dev, const Tableau& tab, int s, double dt, uint64_t step,
+                       bool adaptive_target, bool dev_dt)
 {
     const int S = tab.S;
     // dev_dt: the step length lives on the device (StepCtl::dtr); the tableau goes in unscaled
@@ -546,7 +546,13 @@ mm_status run_stage(mm_ctx* c, float* m_dev, const Tableau& tab, int s, double d
             ep.e_self = (float)dtr;   // max |dm| of the last stage: NaN sentinel and diagnostics
         }
     }
-    return launch_eval(c, ep);
+    return ep;
+}
+
+mm_status run_stage(mm_ctx* c, float* m_dev, const Tableau& tab, int s, double dt, uint64_t step,
+                    bool adaptive_target, bool dev_dt = false)
+{
+    return launch_eval(c, stage_params(c, m_dev, tab, s, dt, step, adaptive_target, dev_dt));
 }
 
 // One trial step; enqueues everything, no synchronisation.  After it, maxbits holds the error

@@ -198,4 +198,56 @@ mm_status mm_dist_backward(mm_ctx* c, const float* m_slab_dev, const float* halo
     return MM_OK;
 }
 
+
+// ---- time stepping on slabs: stage `stage` of a fixed-step method, phase by phase like an evaluation ----
+static mm_status dist_tableau(mm_ctx* c, mm_method method, int stage, Tableau* tab)
+{
+    *tab = make_tableau(method);
+    if (tab->S == 0 || tab->embedded || tab->fsal || stage < 0 || stage >= tab->S)
+        return fail(c, MM_EINVAL, "slab stepping takes a stage of a fixed-step method (rk1, rk2, rk3, rk4)");
+    return MM_OK;
+}
+
+mm_status mm_dist_stage_input(mm_ctx* c, mm_method method, int stage, const float* m_slab_dev, const float** in_dev_out)
+{
+    mm_status s = dist_ready(c);
+    if (s != MM_OK) return s;
+    Tableau tab;
+    if ((s = dist_tableau(c, method, stage, &tab)) != MM_OK) return s;
+    if (!m_slab_dev || !in_dev_out) return fail(c, MM_EINVAL, "NULL pointer");
+    *in_dev_out = stage == 0 ? m_slab_dev : c->ms[(stage - 1) & 1];
+    return MM_OK;
+}
+
+mm_status mm_dist_backward_stage(mm_ctx* c, float* m_slab_dev, mm_method method, int stage, double dt, uint64_t step,
+                                 const float* halo_lo_dev, const float* halo_hi_dev)
+{
+    mm_status s = dist_ready(c);
+    if (s != MM_OK) return s;
+    Tableau tab;
+    if ((s = dist_tableau(c, method, stage, &tab)) != MM_OK) return s;
+    if (!m_slab_dev || !(dt > 0)) return fail(c, MM_EINVAL, "bad m_slab_dev / dt");
+    if (stage == 0) CUDA_TRY(c, cudaMemsetAsync(c->maxbits, 0, sizeof(unsigned int), c->stream));
+    for (int p = 0; p < c->slab.nranks; ++p) {
+        size_t off = 0;
+        mm_dist_segment(c, p, 0, &off, nullptr, nullptr, nullptr);
+        const ff::ColTile ct = peer_tile(c, p);
+        if (!fast_y(c->fp, c->g, c->stream, 1, ct, c->specA + ct.kx0, c->slab_buf + off))
+            return fail(c, MM_ECUDA, "inverse y pass failed");
+        c->kt.launches++;
+    }
+    if (!fast_inv_x_h(c->fp, c->g, c->stream, c->specA, c->hfield, 1.0f)) return fail(c, MM_ECUDA, "inverse x pass failed");
+    EpiParams ep = stage_params(c, m_slab_dev, tab, stage, dt, step, false, false);
+    ep.zlo = halo_lo_dev;
+    ep.zhi = halo_hi_dev;
+    ep.cell0 = (unsigned long long)c->slab.z0 * c->g.Ny * c->g.Nx;
+    launch_epi4(c->g, c->hfield, ep, c->stream);
+    c->kt.launches += 2;
+    if (stage == tab.S - 1 && ep.m_out != m_slab_dev)         // a one-stage method leaves the new state in a scratch field
+        CUDA_TRY(c, cudaMemcpyAsync(m_slab_dev, ep.m_out, 3 * ncell(c->g) * sizeof(float), cudaMemcpyDeviceToDevice,
+                                    c->stream));
+    CUDA_TRY(c, cudaGetLastError());
+    return MM_OK;
+}
+
 }  // extern "C"

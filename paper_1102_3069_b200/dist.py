@@ -81,6 +81,22 @@ class SlabRank:
         self._chk(self.L.mm_dist_backward(self.ctx, self._dev(m) if m is not None else C.c_void_p(0), p(halo_lo),
                                           p(halo_hi), self._dev(out), int(what), int(step), float(dt_thermal)))
 
+    def stage_input(self, m, method, stage):
+        """The field stage `stage` acts on, as a torch view (m itself for stage 0, else a buffer of the context)."""
+        out = C.c_void_p()
+        self._chk(self.L.mm_dist_stage_input(self.ctx, _mm.METHODS[method], int(stage), self._dev(m), C.byref(out)))
+        if out.value == m.data_ptr():
+            return m
+        n = 1
+        for v in self.shape:
+            n *= v
+        return self._view(out.value, n // 2).view(self.shape)
+
+    def backward_stage(self, m, method, stage, dt, step, halo_lo, halo_hi):
+        p = lambda t: C.c_void_p(t.data_ptr()) if t is not None else C.c_void_p(0)
+        self._chk(self.L.mm_dist_backward_stage(self.ctx, self._dev(m), _mm.METHODS[method], int(stage), float(dt),
+                                                int(step), p(halo_lo), p(halo_hi)))
+
     def halo_neighbours(self):
         """(rank below, rank above) whose boundary planes this rank needs, None at an open end of the grid."""
         lo = self.rank - 1 if self.rank > 0 else (self.nranks - 1 if self.pbc[2] > 0 else None)
@@ -202,3 +218,37 @@ def evaluate_nccl(rank_ctx, m, what="heff", step=0, dt_thermal=0.0, group=None):
     o = rank_ctx.torch.empty_like(m)
     rank_ctx.backward(m, lo, hi, o, WHAT[what], step, dt_thermal)
     return o
+
+
+NSTAGES = {"rk1": 1, "rk2": 2, "rk3": 3, "rk4": 4}
+
+
+def steps_fixed_local(ranks, ms, method, dt, n, step0=0):
+    """n fixed steps of rk1 / rk2 / rk3 / rk4 on `ranks` (all in this process); ms[r] is updated in place."""
+    tr = LocalTransport(ranks)
+    for i in range(n):
+        for s in range(NSTAGES[method]):
+            ins = [r.stage_input(m, method, s) for r, m in zip(ranks, ms)]
+            for r, x in zip(ranks, ins):
+                r.forward(x)
+            tr.all_to_all(True)
+            for r in ranks:
+                r.mid()
+            tr.all_to_all(False)
+            hal = tr.halos(ins)
+            for r, m, (lo, hi) in zip(ranks, ms, hal):
+                r.backward_stage(m, method, s, dt, step0 + i, lo, hi)
+
+
+def steps_fixed_nccl(rank_ctx, m, method, dt, n, step0=0, group=None):
+    """The same for this process's slab with the exchanges over NCCL."""
+    tr = NcclTransport(rank_ctx, group)
+    for i in range(n):
+        for s in range(NSTAGES[method]):
+            x = rank_ctx.stage_input(m, method, s)
+            rank_ctx.forward(x)
+            tr.all_to_all(True)
+            rank_ctx.mid()
+            tr.all_to_all(False)
+            lo, hi = tr.halos(x)
+            rank_ctx.backward_stage(m, method, s, dt, step0 + i, lo, hi)

@@ -110,6 +110,8 @@ def lib():
         L.mm_dist_forward.argtypes = [vp, vp]
         L.mm_dist_mid.argtypes = [vp]
         L.mm_dist_backward.argtypes = [vp, vp, vp, vp, vp, C.c_int, C.c_uint64, C.c_double]
+        L.mm_dist_stage_input.argtypes = [vp, C.c_int, C.c_int, vp, C.POINTER(vp)]
+        L.mm_dist_backward_stage.argtypes = [vp, vp, C.c_int, C.c_int, C.c_double, C.c_uint64, vp, vp]
         L.mm_last_error.argtypes = [vp]
         L.mm_last_error.restype = C.c_char_p
         L.mm_destroy.argtypes = [vp]

@@ -55,6 +55,52 @@ def test_slab_decomposition_matches_the_single_context_result(pbc, R):
     assert np.abs(got_t - ref_t).max() <= 2e-6 * np.abs(ref_t).max()
 
 
+@pytest.mark.parametrize("method,R,T", [("rk4", 2, 0.0), ("rk4", 3, 300.0), ("rk2", 2, 0.0), ("rk1", 2, 300.0),
+                                        ("rk3", 4, 0.0)])
+def test_slab_time_stepping_follows_the_oracle_and_the_single_context(method, R, T):
+    """Ten fixed steps on R slabs (stage by stage: forward, all-to-all, mid, all-to-all, halo planes of the STAGE
+    state, backward with the a9 combine): the gathered state against the oracle's textbook stepper (north_star
+    tolerance in m) and against mm_steps_fixed of one ordinary context (fp32 rounding of the z pass variant)."""
+    import torch
+    from oracle import mm_oracle as orc
+    from paper_1102_3069_b200 import dist as mmd
+    wl = util.small((64, 32, 64), (3e-9, 4e-9, 2e-9), (0, 0, 0), T=T, seed=21, j=(1e12, -5e11, 2e11), P=0.5, xi=0.04)
+    m = wlm.initial_m(wl)
+    dt, n = 5e-14, 10
+    pb = util.oracle_problem(wl)
+    mo = m.astype(np.float64)
+    for s in range(n):
+        mo = orc.rk_step(lambda x: pb.torque(x, s, dt), mo, dt, method)[0]
+    sim = util.gpu_sim(wl)
+    md = util.to_dev(m)
+    sim.steps_fixed(md, method, dt, n)
+    one = md.double().cpu().numpy()
+    sim.close()
+    ranks = [mmd.SlabRank(wl.grid, wl.cell, wl.pbc, wl.mat, r, R) for r in range(R)]
+    ms = [util.to_dev(m[:, r.slab.z0:r.slab.z1]) for r in ranks]
+    mmd.steps_fixed_local(ranks, ms, method, dt, n)
+    got = torch.cat(ms, dim=1).double().cpu().numpy()
+    for r in ranks:
+        r.close()
+    assert np.abs(got - mo).max() <= 1e-4, np.abs(got - mo).max()
+    assert np.abs(got - one).max() <= 5e-6, np.abs(got - one).max()
+    assert np.abs(np.sqrt((got * got).sum(0)) - 1.0).max() <= 1e-6
+
+
+def test_slab_stepping_refuses_the_step_controlled_methods():
+    import paper_1102_3069_b200 as mm
+    from paper_1102_3069_b200 import dist as mmd
+    wl = util.small((64, 32, 64), (3e-9, 3e-9, 3e-9))
+    r = mmd.SlabRank(wl.grid, wl.cell, wl.pbc, wl.mat, 0, 2)
+    m = util.to_dev(wlm.initial_m(wl)[:, r.slab.z0:r.slab.z1])
+    for method, stage in (("rkdp", 0), ("rk23", 1), ("rk4", 4), ("rk2", -1)):
+        with pytest.raises(mm.mm.MMError):
+            r.stage_input(m, method, stage)
+        with pytest.raises(mm.mm.MMError):
+            r.backward_stage(m, method, stage, 1e-14, 0, None, None)
+    r.close()
+
+
 def test_slab_context_refuses_the_single_gpu_entry_points_and_bad_grids():
     import paper_1102_3069_b200 as mm
     from paper_1102_3069_b200 import dist as mmd
