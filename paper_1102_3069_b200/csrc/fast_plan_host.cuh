@@ -236,6 +236,7 @@ inline bool khat_map(CUtensorMap* m, const Geom& g, const float* khat, int cols)
 inline void fast_plan_maps(FastPlan& fp, const Geom& g, const float2* specB, const float* khat)
 {
     fp.ok_mid_t = false;
+    fp.ok_panel = false;
     fp.has_kex_map = false;
     fp.k_ptr = khat;
     if (!(fp.ok_mid3 && g.Pz == 128 && specB && khat)) return;
@@ -257,6 +258,19 @@ inline void fast_plan_maps(FastPlan& fp, const Geom& g, const float2* specB, con
         return;
     }
     fp.ok_mid_t = true;
+    // the same array seen in panels of 16 columns (panel_tile): 5D (32 floats, Py, Nz, 3, panel)
+    {
+        mm_encode_tiled_fn enc = tensor_map_encoder();
+        const cuuint64_t rowb = 128, d5[5] = { 32, (cuuint64_t)g.Py, (cuuint64_t)g.Nz, 3, (cuuint64_t)((g.Cx + 15) / 16) };
+        const cuuint64_t s5[4] = { rowb, rowb * g.Py, rowb * g.Py * g.Nz, rowb * g.Py * g.Nz * 3 };
+        const cuuint32_t b5[5] = { 32, 1, (cuuint32_t)g.Nz, 3, 1 }, es[5] = { 1, 1, 1, 1, 1 };
+        auto mk = [&](CUtensorMap* m, const cuuint32_t* bx) {
+            return enc(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 5, const_cast<float2*>(specB), d5, s5, bx, es,
+                       CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+                       CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+        };
+        fp.ok_panel = enc && fp.ok_y && fp.ax[1].R == 1 && mk(&fp.map_spec_p, b5);
+    }
 }
 
 inline void fast_plan_destroy(FastPlan& fp)

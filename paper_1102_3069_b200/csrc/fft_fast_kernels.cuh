@@ -306,9 +306,13 @@ k_y_p(ColTile ct, int nplane, float2* __restrict__ a, float2* __restrict__ b, co
     const float2* __restrict__ src = FWD ? a : b;
     float2* __restrict__ dst = FWD ? b : a;
 
+    // column offset of tile bx on the specB side (panels of 16 columns: two tiles per panel)
+    auto boff = [&](int bx) -> size_t {
+        return ct.b_panel ? (size_t)(bx >> 1) * ct.b_panel + (size_t)(bx & 1) * 8 : (size_t)bx * 8;
+    };
     auto issue = [&](int i) {
         const int bx = i % ntx, cz = i / ntx;
-        const float2* __restrict__ s0 = src + (size_t)cz * s_plane + bx * 8;
+        const float2* __restrict__ s0 = src + (size_t)cz * s_plane + (FWD ? (size_t)bx * 8 : boff(bx));
         for (int u = tid; u < ROWS * 4; u += NT) {
             const int cu = u & 3, r = u >> 2;
             const int left = ct.ncol - (bx * 8 + 2 * cu);
@@ -350,7 +354,7 @@ k_y_p(ColTile ct, int nplane, float2* __restrict__ a, float2* __restrict__ b, co
             for (int k1 = 0; k1 < T; ++k1) v[q + (E / T) * k1] = u[q][k1];
         }
         if (col < ct.ncol) {
-            float2* __restrict__ dp = dst + (size_t)cz * d_plane + col;
+            float2* __restrict__ dp = dst + (size_t)cz * d_plane + (FWD ? boff(bx) + c : (size_t)col);
 #pragma unroll
             for (int j = 0; j < NOUT; ++j) dp[(size_t)(t + T * j) * d_row] = v[j];
         }

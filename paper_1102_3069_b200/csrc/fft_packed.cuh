@@ -180,7 +180,7 @@ struct MidT {
     static constexpr unsigned SMEM_BYTES = XB_BYTES + IB_BYTES + KB_BYTES + 64;
 };
 
-template <bool PER, int C>
+template <bool PER, int C, bool PANEL>
 __global__ void __launch_bounds__(8 * C, (PER ? 2 : 3) * (16 / C))
 k_mid_t(const __grid_constant__ CUtensorMap map_s, const __grid_constant__ CUtensorMap map_k, Geom g,
         float2* __restrict__ spec, const float4* __restrict__ twp)
@@ -194,7 +194,10 @@ k_mid_t(const __grid_constant__ CUtensorMap map_s, const __grid_constant__ CUten
     const int tid = threadIdx.x, c = tid % C, t = tid / C;
     const int ntx = (g.Cx + C - 1) / C;
     const int nitem = ntx * (g.Py / 2 + 1);
-    const size_t rstride = (size_t)g.Py * g.CxS, cstride = (size_t)g.Nz * rstride, step8 = 8 * rstride;
+    // PANEL: specB is [panel][3][Nz][Py][16] (mm_kernels.h panel_tile) and consecutive items are consecutive ky
+    const int npair = g.Py / 2 + 1;
+    const size_t rstride = PANEL ? (size_t)g.Py * 16 : (size_t)g.Py * g.CxS;
+    const size_t cstride = (size_t)g.Nz * rstride, step8 = 8 * rstride;
 
     if (tid == 0) {
         tma_prefetch_desc(&map_s);
@@ -206,14 +209,17 @@ k_mid_t(const __grid_constant__ CUtensorMap map_s, const __grid_constant__ CUten
     __syncthreads();
     auto issue_in = [&](int bx, int other) {
         mbar_expect_tx(bar, M::IB_BYTES);
-        tma_load_4d(const_cast<float2*>(ib), &map_s, bar, 2 * C * bx, other, 0, 0);
+        if (PANEL) tma_load_5d(const_cast<float2*>(ib), &map_s, bar, 0, other, 0, 0, bx);
+        else tma_load_4d(const_cast<float2*>(ib), &map_s, bar, 2 * C * bx, other, 0, 0);
     };
     auto issue_k = [&](int bx, int p) {
         mbar_expect_tx(bar + 1, M::KB_BYTES);
         tma_load_5d(const_cast<float*>(kb), &map_k, bar + 1, C * bx, p, 0, 0, 0);
     };
+    auto item_bx = [&](int i) { return PANEL ? i / npair : i % ntx; };
+    auto item_p = [&](int i) { return PANEL ? i % npair : i / ntx; };
     int q = blockIdx.x;
-    if (tid == 0 && q < nitem) { issue_k(q % ntx, q / ntx); issue_in(q % ntx, q / ntx); }
+    if (tid == 0 && q < nitem) { issue_k(item_bx(q), item_p(q)); issue_in(item_bx(q), item_p(q)); }
     unsigned par_in = 0, par_k = 0;
     // per-thread bases of the exchange tile (writer row t / reader column t) and of the K^ tile
     constexpr int XP = M::XP, RS = M::RS;
@@ -227,7 +233,7 @@ k_mid_t(const __grid_constant__ CUtensorMap map_s, const __grid_constant__ CUten
     const float4* twi = twp + t;                 // inverse: column t (stride 8)
 
     for (; q < nitem; q += gridDim.x) {
-        const int bx = q % ntx, p = q / ntx;
+        const int bx = item_bx(q), p = item_p(q);
         const int mir = (g.Py - p) % g.Py;
         const int nh = mir == p ? 1 : 2;
         const int qn = q + gridDim.x;
@@ -247,7 +253,7 @@ k_mid_t(const __grid_constant__ CUtensorMap map_s, const __grid_constant__ CUten
             __syncthreads();                     // the spectrum tile is in registers: refill it
             if (tid == 0) {
                 if (h + 1 < nh) issue_in(bx, mir);
-                else if (qn < nitem) issue_in(qn % ntx, qn / ntx);
+                else if (qn < nitem) issue_in(item_bx(qn), item_p(qn));
             }
             // ---------------- forward ----------------
             // Software-pipelined over the components: the read-back of component c is issued, then the first
@@ -336,10 +342,11 @@ k_mid_t(const __grid_constant__ CUtensorMap map_s, const __grid_constant__ CUten
                 }
             }
             __syncthreads();                     // K^ tile and the forward exchange are free again
-            if (tid == 0 && h + 1 == nh && qn < nitem) issue_k(qn % ntx, qn / ntx);
+            if (tid == 0 && h + 1 == nh && qn < nitem) issue_k(item_bx(qn), item_p(qn));
             // ---------------- inverse ----------------
             // rows t, t + 8, ... of this column: pointer increments instead of 64-bit multiplies per store
-            float2* __restrict__ op = spec + (size_t)other * g.CxS + col + (size_t)t * rstride;
+            float2* op = PANEL ? spec + (size_t)bx * (3 * cstride) + (size_t)other * 16 + c + (size_t)t * rstride
+                                            : spec + (size_t)other * g.CxS + col + (size_t)t * rstride;
             auto inv_first = [&](int comp) {
                 fft8<1>(V[comp]);                // V[comp][n2] lanes: k2 = 2t, 2t + 1
 #pragma unroll

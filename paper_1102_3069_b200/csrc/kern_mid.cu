@@ -32,17 +32,18 @@ k_mul2d(Geom g, float2* __restrict__ spec, const float* __restrict__ khat)
     p[2 * cs] = make_float2(kxz * mx.x + kyz * my.x + kzz * mz.x, kxz * mx.y + kyz * my.y + kzz * mz.y);
 }
 
-template <bool PER, int C>
+template <bool PER, int C, bool PANEL>
 bool launch_mid_t(const FastPlan& fp, const Geom& g, cudaStream_t st, float2* specB, const float* khat)
 {
     using M = pk::MidT<PER, C>;
     static bool once[MM_MAX_DEV] = {};
-    if (!ensure_smem_dev(pk::k_mid_t<PER, C>, M::SMEM_BYTES, once)) return false;
+    if (!ensure_smem_dev(pk::k_mid_t<PER, C, PANEL>, M::SMEM_BYTES, once)) return false;
     const int nitem = ((g.Cx + C - 1) / C) * (g.Py / 2 + 1);
     const int per_sm = (PER ? 2 : 3) * (16 / C);
     const int grid = nitem < fp.nsm * per_sm ? nitem : fp.nsm * per_sm;
-    pk::k_mid_t<PER, C><<<grid, 8 * C, M::SMEM_BYTES, st>>>(fp.map_spec, khat == fp.k_ptr ? fp.map_k : fp.map_kex, g,
-                                                             specB, fp.twp);
+    pk::k_mid_t<PER, C, PANEL><<<grid, 8 * C, M::SMEM_BYTES, st>>>(PANEL ? fp.map_spec_p : fp.map_spec,
+                                                                    khat == fp.k_ptr ? fp.map_k : fp.map_kex, g, specB,
+                                                                    fp.twp);
     return true;
 }
 
@@ -52,10 +53,12 @@ bool launch_mid3(const FastPlan& fp, const Geom& g, cudaStream_t st, const ColTi
 {
     if constexpr (T * E == 128) {
         // whole-array tiles only: the tensor maps describe specB and K-hat as laid out in mm_common.cuh
-        if (fp.mid_pipe >= 2 && fp.ok_mid_t && ct.kx0 == 0 && ct.ncol == g.Cx && ct.b_row == (size_t)g.CxS &&
-            (khat == fp.k_ptr || fp.has_kex_map))
-            return launch_mid_t<PER, 16>(fp, g, st, specB, khat);
+        if (fp.mid_pipe >= 2 && fp.ok_mid_t && ct.kx0 == 0 && ct.ncol == g.Cx && (khat == fp.k_ptr || fp.has_kex_map)) {
+            if (ct.b_panel) return fp.ok_panel && launch_mid_t<PER, 16, true>(fp, g, st, specB, khat);
+            if (ct.b_row == (size_t)g.CxS) return launch_mid_t<PER, 16, false>(fp, g, st, specB, khat);
+        }
     }
+    if (ct.b_panel) return false;        // only pk::k_mid_t reads the panel layout
     if (fp.mid_pipe) {
         constexpr int L = T * E;
         constexpr int NZ = PER ? L : L / 2;

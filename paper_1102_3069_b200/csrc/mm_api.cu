@@ -301,7 +301,8 @@ mm_status launch_eval(mm_ctx* c, const EpiParams& ep)
             c->kt.end(KT_MID);
             c->kt.launches += 3 * ((g.Cx + fp.chunk_w - 1) / fp.chunk_w) - 1;
         } else if (g.Pz > 1) {
-            const ff::ColTile wt = whole_tile(g);
+            const bool panel = (c->fast & FAST_Y) && (c->fast & FAST_MID) && fast_panel_ok(fp, g, kh);
+            const ff::ColTile wt = panel ? panel_tile(g) : whole_tile(g);
             {   // a2
                 c->kt.begin(KT_FWD_Y);
                 if (!((c->fast & FAST_Y) && fast_y(fp, g, st, -1, wt, c->specA, c->specB))) {
@@ -667,7 +668,7 @@ mm_status mm_create(mm_ctx** out, const int grid[3], const double cellsize[3], c
         if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&c->fp.nsm, cudaDevAttrMultiProcessorCount, dev);
         if (c->fp.nsm < 1) c->fp.nsm = 1;
     }
-    c->fp.x_pipe = 1; c->fp.mid_pipe = 2; c->fp.mid_cols = 16; c->fp.chunk_w = 0; c->fp.nstream = 3;     // mm_set_option defaults
+    c->fp.x_pipe = 1; c->fp.spec_panel = 1; c->fp.mid_pipe = 2; c->fp.mid_cols = 16; c->fp.chunk_w = 0; c->fp.nstream = 3;     // mm_set_option defaults
     *out = c;
     return MM_OK;
 }
@@ -761,7 +762,7 @@ static mm_status demag_init_impl(mm_ctx* c)
     CUDA_TRY(c, cudaMalloc(&c->specA, nA * sizeof(float2)));
     CUDA_TRY(c, cudaMemset(c->specA, 0, nA * sizeof(float2)));
     if (g.Py > 1 && !c->dist) {      // (a slab rank's y passes write into / read from slab_buf)
-        const size_t nB = (size_t)3 * g.Nz * g.Py * g.CxS;
+        const size_t nB = (size_t)3 * g.Nz * g.Py * specb_cols(g);     // room for the 16-column panel form
         CUDA_TRY(c, cudaMalloc(&c->specB, nB * sizeof(float2)));
         CUDA_TRY(c, cudaMemset(c->specB, 0, nB * sizeof(float2)));
     }
@@ -1353,6 +1354,7 @@ mm_status mm_set_option(mm_ctx* c, const char* key, int value)
     if (k == "graph") { c->use_graph = value != 0; return MM_OK; }
     if (k == "x_pipe") { c->fp.x_pipe = value & 3; return MM_OK; }
     if (k == "mid_pipe") { c->fp.mid_pipe = value; return MM_OK; }
+    if (k == "spec_panel") { c->fp.spec_panel = value; return MM_OK; }
     if (k == "chunk_w" || k == "chunk_streams") {
         // the chunk streams and the slot layout are fixed when the workspaces are made
         if (c->has_demag) return fail(c, MM_ESTATE, "option " + k + " must be set before mm_demag_init");

@@ -25,9 +25,11 @@ namespace ff {
 // `ncol` kx columns starting at kx0, with the y-padded spectrum in a compact buffer [3][Nz][Py][W].
 // ---------------------------------------------------------------------------------------------
 struct ColTile {
+    ColTile() : kx0(0), ncol(0), a_row(0), a_plane(0), b_row(0), b_plane(0), b_panel(0) {}
     int kx0, ncol;                 // first global column, number of valid columns
     size_t a_row, a_plane;         // specA side: strides in float2 (row y, plane (component, z))
     size_t b_row, b_plane;         // specB / chunk side
+    size_t b_panel;                // specB in panels of 16 columns [panel][3 Nz][Py][16] (stride of a panel), 0: plain rows
 };
 }  // namespace ff
 
@@ -57,6 +59,9 @@ struct FastPlan {
     int mid_pipe;                        // last-axis pass: persistent pipelined kernel (option "mid_pipe")
     // last-axis pass through TMA tiles and sibling-packed codelets (pk::k_mid_t; mid_pipe >= 2, Pz = 128)
     bool ok_mid_t, has_kex_map;
+    bool ok_panel;                       // specB may be kept in 16-column panels between a2, a3 and a4 (option "spec_panel")
+    int spec_panel;
+    CUtensorMap map_spec_p;              // specB in panels: (32 floats, Py, Nz, 3, panel)
     int mid_cols;                        // kx columns per work item of pk::k_mid_t
     CUtensorMap map_spec, map_k, map_kex;  // specB [3][Nz][Py][2 CxS] floats; K-hat / K-hat + exchange [6][Cz][Cy][CxK]
     const float* k_ptr;                  // the K-hat array map_k describes (map_kex: any other)
@@ -112,8 +117,22 @@ inline ff::ColTile whole_tile(const Geom& g)
     ct.kx0 = 0; ct.ncol = g.Cx;
     ct.a_row = g.CxS; ct.a_plane = (size_t)g.Ny * g.CxS;
     ct.b_row = g.CxS; ct.b_plane = (size_t)g.Py * g.CxS;
+    ct.b_panel = 0;
     return ct;
 }
+
+// the whole array with specB in panels of 16 kx columns: [panel][3][Nz][Py][16].  A y-pass tile (8 columns, all ky of
+// one plane) and its neighbour then fill one contiguous 16 Py float2 block, and the rows of a last-axis work item
+// (16 columns, one ky) sit next to those of ky + 1 -- the DRAM-friendly form of the same traffic.
+inline ff::ColTile panel_tile(const Geom& g)
+{
+    ff::ColTile ct = whole_tile(g);
+    ct.b_row = 16; ct.b_plane = (size_t)g.Py * 16;
+    ct.b_panel = (size_t)3 * g.Nz * g.Py * 16;
+    return ct;
+}
+// columns specB must have room for (the last panel is padded)
+inline size_t specb_cols(const Geom& g) { const size_t cp = (size_t)((g.Cx + 15) / 16) * 16; return cp > (size_t)g.CxS ? cp : (size_t)g.CxS; }
 
 
 // ---- size-specialised passes (return false: no kernel for this size, the caller falls back) ----
@@ -125,6 +144,13 @@ bool fast_lines(const FastPlan& fp, cudaStream_t st, int sgn, bool per, const ff
 bool fast_y(const FastPlan& fp, const Geom& g, cudaStream_t st, int sgn, const ff::ColTile& ct, float2* a, float2* b);
 bool fast_mid3(const FastPlan& fp, const Geom& g, cudaStream_t st, const ff::ColTile& ct, float2* specB,
                const float* khat);
+// true: a2, a3, a4 of a whole-array evaluation may run with specB in panels (pk::k_mid_t is the z pass, the y passes
+// have a kernel for Py itself)
+inline bool fast_panel_ok(const FastPlan& fp, const Geom& g, const float* khat)
+{
+    return fp.spec_panel && fp.mid_pipe >= 2 && fp.ok_mid_t && fp.ok_panel && fp.ok_y && g.Pz == 128 &&
+           (khat == fp.k_ptr || fp.has_kex_map);
+}
 bool fast_z_long(const FastPlan& fp, const Geom& g, cudaStream_t st, float2* specB, const float* khat);
 bool fast_mul2(const FastPlan& fp, const Geom& g, cudaStream_t st, float2* specB, const float* khat);
 void launch_mul2d(const Geom& g, float2* spec, const float* khat, cudaStream_t st);      // any size

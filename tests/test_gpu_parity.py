@@ -364,6 +364,22 @@ def test_chunked_l2_resident_passes_match_whole_array_passes(grid, pbc):
     sim.close()
 
 
+@pytest.mark.parametrize("grid,pbc", [((64, 32, 64), (0, 0, 0)), ((200, 48, 64), (0, 0, 0)), ((64, 64, 128), (0, 1, 1))])
+def test_panel_layout_of_the_spectrum_changes_no_bit(grid, pbc):
+    """Option spec_panel: the y-transformed spectrum in 16-column panels (a2, a3, a4 with pk::k_mid_t as the z pass)
+    against plain rows -- same arithmetic, another address map: bit for bit, also with a ragged last panel."""
+    wl = util.small(grid, (3e-9, 4e-9, 2e-9), pbc, j=(1e12, -5e11, 2e11), P=0.5, xi=0.04)
+    md = util.to_dev(wlm.initial_m(wl))
+    out = {}
+    for flag in (1, 0):
+        sim = util.gpu_sim(wl, options={"spec_panel": flag})
+        out[flag] = (sim.demag_field(md).clone(), sim.torque(md).clone())
+        sim.close()
+    assert float((out[0][0] - out[1][0]).abs().max()) == 0.0
+    assert float((out[0][1] - out[1][1]).abs().max()) == 0.0
+    assert float(out[1][0].abs().max()) > 0.0
+
+
 def test_full_size_headline_grid_sampled_against_the_definition():
     """BASELINE.json's metric size (512x512x64, the launch configuration bench.py times).  The oracle
     cannot evaluate a dense state at this size in test time, so: (a) a sparse state of a few source
