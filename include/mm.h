@@ -184,6 +184,26 @@ mm_status mm_steps_maxdm(mm_ctx* ctx, float* m_dev, mm_method method, double max
  * Synchronises the stream. */
 mm_status mm_average(mm_ctx* ctx, const float* field_dev, double avg_host[3]);
 
+/* mm_average_static -- the same reduction (<f> over all cells of f [3][ncell]; fp64 accumulation) for
+ * callers that cannot allocate device memory (code under CUDA graph capture, tight serving loops): it needs no
+ * context and calls no cudaMalloc / cudaFree / allocating library routine.  Its scratch -- per-block partial sums
+ * and an arrival counter, 192 KB -- is a fixed file-scope device array that every GPU loading the library holds
+ * until the process exits.
+ *   field_dev   device, float [3][ncell], read only
+ *   ncell       cells per component, 1 .. MM_AVERAGE_STATIC_MAX_CELLS (larger: MM_EUNSUPPORTED, nothing launched)
+ *   avg_dev     DEVICE, double [3], written by the kernel (no host synchronisation; read it after the stream)
+ *   stream      cudaStream_t as void* (NULL: the default stream); runs on the device current at the call
+ *   err,err_len host, may be NULL / 0: receives a message for a non-OK status
+ * All calls share the one scratch array: calls that overlap on the GPU (different streams without an ordering
+ * between them, or two host threads) race on it -- order them.  The counter is cleared at the start of every call
+ * and every partial sum a call reads is written by that call, so nothing depends on an earlier call.  The first
+ * call on a device looks the array's address up (cudaGetSymbolAddress; make that call outside graph capture).
+ * The result is the sum in block order: reproducible bit for bit, and equal to mm_average's to fp64 rounding.
+ * Errors: MM_EINVAL (NULL pointer, ncell = 0), MM_EUNSUPPORTED (ncell beyond the maximum), MM_ECUDA. */
+#define MM_AVERAGE_STATIC_MAX_CELLS ((size_t)67108864)
+mm_status mm_average_static(const float* field_dev, size_t ncell, double* avg_dev, void* stream, char* err,
+                            size_t err_len);
+
 /* mm_steps_fixed_host -- the same as mm_steps_fixed for a state held in HOST memory (pinned memory
  * gives the full PCIe rate): m_host is copied to the device, advanced n steps and copied back, all on
  * the context's stream; returns after the copy back.  This is the end-to-end call bench.py times. */

@@ -84,6 +84,7 @@ def lib():
         L.mm_steps_adaptive.argtypes = [vp, vp, C.c_int, C.c_int, d3, C.c_double, d3, i3, d3]
         L.mm_steps_maxdm.argtypes = [vp, vp, C.c_int, C.c_double, C.c_int, d3, d3]
         L.mm_average.argtypes = [vp, vp, d3]
+        L.mm_average_static.argtypes = [vp, C.c_size_t, vp, vp, C.c_char_p, C.c_size_t]
         L.mm_kernel_timing.argtypes = [vp, C.c_int]
         L.mm_kernel_times.argtypes = [vp, d3, C.POINTER(C.c_uint64)]
         L.mm_fused_eval.argtypes = [vp, vp, C.c_int, C.c_int, C.c_double, C.c_uint64]
@@ -155,6 +156,22 @@ def slab_segment(grid, pbc, nranks, rank, peer, comp):
     if st != MM_OK:
         raise MMError(st, "mm_slab_segment")
     return tuple(int(x.value) for x in v)
+
+
+AVERAGE_STATIC_MAX_CELLS = 67108864          # MM_AVERAGE_STATIC_MAX_CELLS of include/mm.h
+
+
+def average_static(field, out, stream=None):
+    """mm_average_static: <f> of a CUDA float32 tensor [3, ...] into the CUDA float64 tensor out[3] (caller's memory),
+    through the library's fixed scratch array -- nothing is allocated on the way, no host synchronisation."""
+    assert field.is_cuda and field.is_contiguous() and field.shape[0] == 3 and str(field.dtype) == "torch.float32"
+    assert out.is_cuda and out.is_contiguous() and out.numel() == 3 and str(out.dtype) == "torch.float64"
+    err = C.create_string_buffer(512)
+    st = lib().mm_average_static(C.c_void_p(field.data_ptr()), field.numel() // 3, C.c_void_p(out.data_ptr()),
+                                 C.c_void_p(stream.cuda_stream if stream is not None else 0), err, len(err))
+    if st != MM_OK:
+        raise MMError(st, err.value.decode())
+    return out
 
 
 def demag_khat_host(cell, grid, pbc) -> np.ndarray:
