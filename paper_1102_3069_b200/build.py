@@ -16,7 +16,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.environ.get("MM_B200_LIB") or os.path.join(HERE, "libmm_b200.so")
 OBJDIR = os.path.join(HERE, "build")
-SOURCES = ["mm_api.cu", "kern_x.cu", "kern_y.cu", "kern_mid.cu", "kern_epi.cu", "kern_gen.cu", "kern_static.cu", "demag_host.cpp"]
+SOURCES = ["mm_api.cu", "kern_x.cu", "kern_xq.cu", "kern_y.cu", "kern_mid.cu", "kern_epi.cu", "kern_gen.cu", "kern_static.cu", "demag_host.cpp"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC,-fopenmp,-O2"]
 

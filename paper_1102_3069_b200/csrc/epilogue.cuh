@@ -410,6 +410,81 @@ __device__ __forceinline__ float pair_cell(const EpiParams& p, const PairGeom& q
 
 // Block-wide max of non-negative floats (NaN wins), one atomicMax per block (step a10).
 // Order-independent, hence bit-reproducible.
+// ---------------------------------------------------------------------------------------------
+// The per-cell tail of one quad (4 consecutive cells along x, first cell (4 x4, y, z)) with H_ms read through `hs`
+// (hs(c, v): the quad's four values of component c; shared memory in the fused last pass k_inv_x_q).  Same
+// arithmetic as k_epi4.  Must be called by all 32 lanes of a warp, whose quads are consecutive along x in one row
+// (the x neighbours of a quad's end cells come from the adjacent lanes).  Returns the value to be max-reduced.
+// ---------------------------------------------------------------------------------------------
+template <bool LEAN, int NA, typename HS>
+__device__ __forceinline__ unsigned int epilogue_quad(const Geom& g, const EpiParams& ep, int x4, int y, int z, HS hs)
+{
+    const int nx4 = g.Nx >> 2;
+    const int x = x4 << 2;
+    const size_t plane = (size_t)g.Ny * g.Nx;
+    const size_t n = plane * g.Nz;
+    const size_t rowc = (size_t)z * plane + (size_t)y * g.Nx;
+    const size_t idx = rowc + x;
+    const float* __restrict__ mi = ep.m_in;
+    const unsigned lane = threadIdx.x & 31;
+    float m[3][4], h[3][4], D[3][4];
+#pragma unroll
+    for (int c = 0; c < 3; ++c) ldv<4>(mi + idx + c * n, m[c]);
+    float xl[3], xr[3];
+    {
+        const bool lsh = lane > 0 && x4 > 0, rsh = lane < 31 && x4 + 1 < nx4;
+        const int xli = x > 0 ? x - 1 : (g.perx ? g.Nx - 1 : x);
+        const int xri = x + 4 < g.Nx ? x + 4 : (g.perx ? 0 : x + 3);
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            const float up = __shfl_up_sync(0xffffffffu, m[c][3], 1);
+            const float dn = __shfl_down_sync(0xffffffffu, m[c][0], 1);
+            xl[c] = lsh ? up : mi[rowc + xli + c * n];
+            xr[c] = rsh ? dn : mi[rowc + xri + c * n];
+        }
+    }
+    const bool need_nb = ep.wex[0] != 0.f || ep.wex[1] != 0.f || ep.wex[2] != 0.f || ep.stt;
+    if (!need_nb) {
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            hs(c, h[c]);
+#pragma unroll
+            for (int u = 0; u < 4; ++u) if (!LEAN) D[c][u] = 0.f;
+        }
+        return __float_as_uint(epilogue_finish_v<4, LEAN, NA>(ep, idx, n, m, h, D)) & 0x7fffffffu;
+    }
+    const int ym = y > 0 ? y - 1 : (g.pery ? g.Ny - 1 : y);
+    const int yp = y + 1 < g.Ny ? y + 1 : (g.pery ? 0 : y);
+    const int zm = z > 0 ? z - 1 : (g.perz ? g.Nz - 1 : z);
+    const int zp = z + 1 < g.Nz ? z + 1 : (g.perz ? 0 : z);
+    const size_t iym = (size_t)z * plane + (size_t)ym * g.Nx + x, iyp = (size_t)z * plane + (size_t)yp * g.Nx + x;
+    const size_t izm = (size_t)zm * plane + (size_t)y * g.Nx + x, izp = (size_t)zp * plane + (size_t)y * g.Nx + x;
+    const bool lo_h = ep.zlo != nullptr && z == 0, hi_h = ep.zhi != nullptr && z == g.Nz - 1;
+    const float* __restrict__ pzm = lo_h ? ep.zlo + (size_t)y * g.Nx + x : mi + izm;
+    const float* __restrict__ pzp = hi_h ? ep.zhi + (size_t)y * g.Nx + x : mi + izp;
+    const size_t szm = lo_h ? plane : n, szp = hi_h ? plane : n;
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        float a[4], b[4], d[4], e[4];
+        hs(c, h[c]);
+        ldv<4>(mi + iym + c * n, a);
+        ldv<4>(mi + iyp + c * n, b);
+        ldv<4>(pzm + c * szm, d);
+        ldv<4>(pzp + c * szp, e);
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            const float mc = m[c][u];
+            const float xm = u > 0 ? m[c][u > 0 ? u - 1 : 0] : xl[c];
+            const float xp = u < 3 ? m[c][u < 3 ? u + 1 : 3] : xr[c];
+            h[c][u] += ep.wex[0] * ((xp - mc) + (xm - mc));
+            h[c][u] += ep.wex[1] * ((b[u] - mc) + (a[u] - mc));
+            h[c][u] += ep.wex[2] * ((e[u] - mc) + (d[u] - mc));
+            if (!LEAN) D[c][u] = ep.cj[0] * (xp - xm) + ep.cj[1] * (b[u] - a[u]) + ep.cj[2] * (e[u] - d[u]);
+        }
+    }
+    return __float_as_uint(epilogue_finish_v<4, LEAN, NA>(ep, idx, n, m, h, D)) & 0x7fffffffu;
+}
+
 __device__ __forceinline__ void block_max_atomic(unsigned int b, unsigned int* target)
 {
 #pragma unroll

@@ -370,7 +370,12 @@ mm_status launch_eval(mm_ctx* c, const EpiParams& ep)
     }
     // a5-a10
     bool done = false;
-    if (ep.demag && (c->fast & FAST_SPLIT) && (fp.ok_x || fp.ok_xr || fp.x_R > 1) && (g.Nx % 4 == 0 || ep.geometry)) {
+    if (ep.demag && (c->fast & FAST_SPLIT) && fast_inv_x_q_ok(fp, g, ep)) {
+        c->kt.begin(KT_INV_X);
+        done = fast_inv_x_q(fp, g, st, c->specA, ep);
+        c->kt.end(KT_INV_X);
+    }
+    if (!done && ep.demag && (c->fast & FAST_SPLIT) && (fp.ok_x || fp.ok_xr || fp.x_R > 1) && (g.Nx % 4 == 0 || ep.geometry)) {
         // split variant: inverse x pass -> H_ms field, then the streaming per-cell tail
         c->kt.begin(KT_INV_X);
         if (ep.mode == EPI_HMS) {
@@ -668,7 +673,7 @@ mm_status mm_create(mm_ctx** out, const int grid[3], const double cellsize[3], c
         if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&c->fp.nsm, cudaDevAttrMultiProcessorCount, dev);
         if (c->fp.nsm < 1) c->fp.nsm = 1;
     }
-    c->fp.x_pipe = 1; c->fp.spec_panel = 1; c->fp.mid_pipe = 2; c->fp.mid_cols = 16; c->fp.chunk_w = 0; c->fp.nstream = 3;     // mm_set_option defaults
+    c->fp.x_pipe = 1; c->fp.spec_panel = 1; c->fp.last_fused = 1; c->fp.q_blocks = 4; c->fp.mid_pipe = 2; c->fp.mid_cols = 16; c->fp.chunk_w = 0; c->fp.nstream = 3;     // mm_set_option defaults
     *out = c;
     return MM_OK;
 }
@@ -1355,6 +1360,8 @@ mm_status mm_set_option(mm_ctx* c, const char* key, int value)
     if (k == "x_pipe") { c->fp.x_pipe = value & 3; return MM_OK; }
     if (k == "mid_pipe") { c->fp.mid_pipe = value; return MM_OK; }
     if (k == "spec_panel") { c->fp.spec_panel = value; return MM_OK; }
+    if (k == "last_fused") { c->fp.last_fused = value; return MM_OK; }
+    if (k == "q_blocks") { c->fp.q_blocks = value < 1 ? 1 : value; return MM_OK; }
     if (k == "chunk_w" || k == "chunk_streams") {
         // the chunk streams and the slot layout are fixed when the workspaces are made
         if (c->has_demag) return fail(c, MM_ESTATE, "option " + k + " must be set before mm_demag_init");

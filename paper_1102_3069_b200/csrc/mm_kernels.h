@@ -61,6 +61,8 @@ struct FastPlan {
     bool ok_mid_t, has_kex_map;
     bool ok_panel;                       // specB may be kept in 16-column panels between a2, a3 and a4 (option "spec_panel")
     int spec_panel;
+    int last_fused;                      // option "last_fused": a5-a10 in one kernel (k_inv_x_q) where it applies
+    int q_blocks;                        // option "q_blocks": resident blocks per SM of k_inv_x_q
     CUtensorMap map_spec_p;              // specB in panels: (32 floats, Py, Nz, 3, panel)
     int mid_cols;                        // kx columns per work item of pk::k_mid_t
     CUtensorMap map_spec, map_k, map_kex;  // specB [3][Nz][Py][2 CxS] floats; K-hat / K-hat + exchange [6][Cz][Cy][CxK]
@@ -139,6 +141,13 @@ inline size_t specb_cols(const Geom& g) { const size_t cp = (size_t)((g.Cx + 15)
 bool fast_fwd_x(const FastPlan& fp, const Geom& g, cudaStream_t st, const float* m, float2* specA);
 bool fast_inv_x(const FastPlan& fp, const Geom& g, cudaStream_t st, const float2* specA, const EpiParams& ep);
 bool fast_inv_x_h(const FastPlan& fp, const Geom& g, cudaStream_t st, const float2* specA, float* out, float scale);
+bool fast_inv_x_q(const FastPlan& fp, const Geom& g, cudaStream_t st, const float2* specA, const EpiParams& ep);
+// where the one-kernel last pass applies: x lines of 1024 with their own kernel, whole warps of quads per row, no
+// staircase geometry, an output that needs the per-cell tail
+inline bool fast_inv_x_q_ok(const FastPlan& fp, const Geom& g, const EpiParams& ep)
+{
+    return fp.last_fused && fp.ok_x && fp.x_R <= 1 && g.Px == 1024 && g.Nx % 128 == 0 && !ep.geometry && ep.mode != EPI_HMS;
+}
 bool fast_lines(const FastPlan& fp, cudaStream_t st, int sgn, bool per, const ff::ColTile& ct, int nplane, float2* a,
                 float2* b, int P, const AxisPlan& ap);
 bool fast_y(const FastPlan& fp, const Geom& g, cudaStream_t st, int sgn, const ff::ColTile& ct, float2* a, float2* b);

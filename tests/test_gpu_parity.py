@@ -380,6 +380,44 @@ def test_panel_layout_of_the_spectrum_changes_no_bit(grid, pbc):
     assert float(out[1][0].abs().max()) > 0.0
 
 
+@pytest.mark.parametrize("grid,pbc,kw", [
+    ((512, 16, 8), (0, 0, 0), {}),
+    ((512, 15, 4), (0, 0, 0), dict(T=300.0, j=(1e12, -5e11, 2e11), P=0.5, xi=0.04)),     # odd Ny: a last single row
+    ((1024, 8, 4), (1, 0, 0), dict(K1=4.8e4, K2=-1.0e4)),                                   # periodic x, cubic anisotropy
+    ((512, 32, 2), (0, 1, 1), dict(T=300.0))])
+def test_one_kernel_last_pass_gives_the_bits_of_the_split_one(grid, pbc, kw):
+    """Option last_fused: inverse x transform and per-cell tail of a row pair in one block (k_inv_x_q, H_ms through
+    shared memory) against k_inv_x_h + k_epi4 (H_ms through HBM): the same arithmetic on the same values, so H_eff,
+    torque, fixed steps and controlled steps agree bit for bit; and the field meets the oracle."""
+    wl = util.small(grid, (3e-9, 4e-9, 5e-9), pbc, seed=3, **kw)
+    m = wlm.initial_m(wl)
+    res = {}
+    for flag in (0, 1):
+        sim = util.gpu_sim(wl, options={"last_fused": flag})
+        md = util.to_dev(m)
+        H = sim.heff(md, step=2, dt_thermal=5e-14).clone()
+        Tq = sim.torque(md, step=2, dt_thermal=5e-14).clone()
+        l0 = sim.launch_count()
+        sim.torque(md)
+        nl = sim.launch_count() - l0
+        sim.steps_fixed(md, "rk4", 5e-14, 3)
+        out = [H, Tq, md.clone(), nl]
+        if not kw.get("T"):
+            md2 = util.to_dev(m)
+            _, err = sim.steps_fixed(md2, "rkdp", 5e-14, 2)
+            out += [md2.clone(), err]
+        res[flag] = out
+        sim.close()
+    assert res[1][3] == res[0][3] - 1                     # one launch fewer per evaluation
+    for a, b in zip(res[0][:3], res[1][:3]):
+        assert float((a - b).abs().max()) == 0.0
+    if not kw.get("T"):
+        assert float((res[0][4] - res[1][4]).abs().max()) == 0.0 and res[0][5] == res[1][5]
+    if not any(pbc):                                       # (periodic float128 image sums take too long here)
+        ref = util.oracle_problem(wl).heff(m.astype(np.float64), 2, 5e-14)
+        _cmp(res[1][0], ref, TOL_H)
+
+
 def test_full_size_headline_grid_sampled_against_the_definition():
     """BASELINE.json's metric size (512x512x64, the launch configuration bench.py times).  The oracle
     cannot evaluate a dense state at this size in test time, so: (a) a sparse state of a few source
