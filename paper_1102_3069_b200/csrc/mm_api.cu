@@ -637,7 +637,9 @@ mm_status mm_create(mm_ctx** out, const int grid[3], const double cellsize[3], c
     g.Px = P[0]; g.Py = P[1]; g.Pz = P[2];
     g.Cx = P[0] / 2 + 1; g.Cy = P[1] / 2 + 1; g.Cz = P[2] / 2 + 1;
     g.CxS = (g.Cx + 7) & ~7;     // rows start on 64-byte boundaries
-    g.CxK = (g.Cx + 3) & ~3;
+    // K-hat rows: 16-byte multiples; whole 128-byte lines where the TMA tiles of pk::k_mid_t read 64-byte pieces of them
+    // (a piece that straddles lines made the pass read 1.3 - 1.5 times its K-hat bytes)
+    g.CxK = g.Cx >= 128 ? (g.Cx + 31) & ~31 : (g.Cx + 3) & ~3;
     g.perx = pbc[0] > 0; g.pery = pbc[1] > 0; g.perz = pbc[2] > 0;
     for (int a = 0; a < 3; ++a) { c->cell[a] = cellsize[a]; c->pbc[a] = pbc[a]; }
     c->stream = (cudaStream_t)cuda_stream;

@@ -19,7 +19,7 @@ struct Geom {
     int Px, Py, Pz;      // padded transform sizes (reading A9)
     int Cx, Cy, Cz;      // P/2 + 1
     int CxS;             // row stride of the spectra, in complex elements
-    int CxK;             // row stride of K-hat, in floats (Cx rounded up to 4: 16-byte rows)
+    int CxK;             // row stride of K-hat, in floats (Cx rounded up to 4: 16-byte rows; to 32 from Cx = 128 on)
     int perx, pery, perz;
 };
 
