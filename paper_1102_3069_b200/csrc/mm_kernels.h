@@ -142,11 +142,12 @@ bool fast_fwd_x(const FastPlan& fp, const Geom& g, cudaStream_t st, const float*
 bool fast_inv_x(const FastPlan& fp, const Geom& g, cudaStream_t st, const float2* specA, const EpiParams& ep);
 bool fast_inv_x_h(const FastPlan& fp, const Geom& g, cudaStream_t st, const float2* specA, float* out, float scale);
 bool fast_inv_x_q(const FastPlan& fp, const Geom& g, cudaStream_t st, const float2* specA, const EpiParams& ep);
-// where the one-kernel last pass applies: x lines of 1024 with their own kernel, whole warps of quads per row, no
+// where the one-kernel last pass applies: x lines of 1024, 512 or 256 with their own kernel, whole warps of quads per row, no
 // staircase geometry, an output that needs the per-cell tail
 inline bool fast_inv_x_q_ok(const FastPlan& fp, const Geom& g, const EpiParams& ep)
 {
-    return fp.last_fused && fp.ok_x && fp.x_R <= 1 && g.Px == 1024 && g.Nx % 128 == 0 && !ep.geometry && ep.mode != EPI_HMS;
+    return fp.last_fused && fp.ok_x && fp.x_R <= 1 && (g.Px == 1024 || g.Px == 512 || g.Px == 256) && g.Nx % 128 == 0 &&
+           !ep.geometry && ep.mode != EPI_HMS;
 }
 bool fast_lines(const FastPlan& fp, cudaStream_t st, int sgn, bool per, const ff::ColTile& ct, int nplane, float2* a,
                 float2* b, int P, const AxisPlan& ap);

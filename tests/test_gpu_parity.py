@@ -384,7 +384,11 @@ def test_panel_layout_of_the_spectrum_changes_no_bit(grid, pbc):
     ((512, 16, 8), (0, 0, 0), {}),
     ((512, 15, 4), (0, 0, 0), dict(T=300.0, j=(1e12, -5e11, 2e11), P=0.5, xi=0.04)),     # odd Ny: a last single row
     ((1024, 8, 4), (1, 0, 0), dict(K1=4.8e4, K2=-1.0e4)),                                   # periodic x, cubic anisotropy
-    ((512, 32, 2), (0, 1, 1), dict(T=300.0))])
+    ((512, 32, 2), (0, 1, 1), dict(T=300.0)),
+    ((256, 6, 3), (0, 0, 0), {}),                          # x lines of 512: two row pairs per block, 9 pairs (ragged)
+    ((512, 10, 2), (1, 0, 0), dict(T=300.0, j=(1e12, -5e11, 2e11), P=0.5, xi=0.04)),
+    ((128, 32, 5), (0, 0, 0), {}),                         # x lines of 256 (config 3's)
+    ((256, 7, 3), (1, 0, 0), dict(K1=4.8e4, K2=-1.0e4))])
 def test_one_kernel_last_pass_gives_the_bits_of_the_split_one(grid, pbc, kw):
     """Option last_fused: inverse x transform and per-cell tail of a row pair in one block (k_inv_x_q, H_ms through
     shared memory) against k_inv_x_h + k_epi4 (H_ms through HBM): the same arithmetic on the same values, so H_eff,
