@@ -273,6 +273,8 @@ mm_status mm_batch_set_field(mm_ctx* ctx, const double* B_host);
  *                    length 128; other lengths take 1); 1: persistent, cp.async-pipelined; 0: one block per line set
  *   "spec_panel"     1 (default): when the "mid_pipe" 2 kernel runs, the y-transformed spectrum is kept in panels of
  *                    16 kx columns between a2, a3 and a4 (same arithmetic, DRAM-friendlier rows); 0: plain rows
+ *   "y_tma"          1 (default): in that panel form, y lines of 1024 get their tiles by TMA (cp.async.bulk.tensor, one
+ *                    thread issues) instead of 16 cp.async per thread; 0: cp.async
  *   "last_fused"     1 (default): where it applies (padded x length 1024, 512 or 256, Nx a multiple of 128, no staircase geometry) the
  *                    inverse x pass and the per-cell tail are ONE kernel, H_ms passing through shared memory;
  *                    0: two kernels with H_ms written to and read from device memory (every other grid does that)

@@ -233,8 +233,10 @@ inline bool khat_map(CUtensorMap* m, const Geom& g, const float* khat, int cols)
 }
 
 // called by mm_demag_init once specB and K-hat exist; failure only switches pk::k_mid_t off
-inline void fast_plan_maps(FastPlan& fp, const Geom& g, const float2* specB, const float* khat)
+inline void fast_plan_maps(FastPlan& fp, const Geom& g, const float2* specA, const float2* specB, const float* khat)
 {
+    fp.ok_ymaps = false;
+    fp.y_a = specA; fp.y_b = specB;
     fp.ok_mid_t = false;
     fp.ok_panel = false;
     fp.has_kex_map = false;
@@ -270,6 +272,22 @@ inline void fast_plan_maps(FastPlan& fp, const Geom& g, const float2* specB, con
                        CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
         };
         fp.ok_panel = enc && fp.ok_y && fp.ax[1].R == 1 && mk(&fp.map_spec_p, b5);
+        if (fp.ok_panel && specA && g.Py == 1024) {
+            // y-pass tiles: 8 columns x 256 rows
+            const cuuint32_t by[4] = { 16, 256, 1, 1 };
+            const cuuint64_t d4[4] = { 32, (cuuint64_t)g.Py, (cuuint64_t)3 * g.Nz, (cuuint64_t)((g.Cx + 15) / 16) };
+            const cuuint64_t s4[3] = { rowb, rowb * g.Py, rowb * g.Py * g.Nz * 3 };
+            const cuuint64_t d3[3] = { (cuuint64_t)2 * g.Cx, (cuuint64_t)g.Ny, (cuuint64_t)3 * g.Nz };
+            const cuuint64_t s3[2] = { (cuuint64_t)g.CxS * 8, (cuuint64_t)g.CxS * 8 * g.Ny };
+            const cuuint32_t es4[4] = { 1, 1, 1, 1 };
+            fp.ok_ymaps =
+                enc(&fp.map_yb, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, const_cast<float2*>(specB), d4, s4, by, es4,
+                    CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+                    CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS &&
+                enc(&fp.map_ya, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, const_cast<float2*>(specA), d3, s3, by, es4,
+                    CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+                    CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+        }
     }
 }
 

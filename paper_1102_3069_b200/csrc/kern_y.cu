@@ -4,14 +4,117 @@
 #include <vector>
 #include "mm_kernels.h"
 #include "fft_fast.cuh"
+#include "fft_packed.cuh"
 
 namespace mm {
 namespace ff {
+// ---------------------------------------------------------------------------------------------
+// a2 / a4 with the tile loaded by TMA (whole-array passes with specB in panels): k_y_p with its 16 cp.async
+// per thread and tile replaced by ROWS / 256 cp.async.bulk.tensor issued by one thread (box 8 columns x 256 rows,
+// landing as [rows][8] float2 exactly where k_y_p stages its tile); completion on an mbarrier.
+//   forward: map = specA as (2 Cx floats, Ny, 3 Nz);  inverse: map = specB panels as (32 floats, Py, 3 Nz, panel).
+// ---------------------------------------------------------------------------------------------
+extern __shared__ __align__(128) unsigned char yt_smem[];
+
+template <int T, int E, int SGN, bool PER>
+__global__ void __launch_bounds__(8 * T, (T == 32) ? 2 : 1)
+k_y_t(const __grid_constant__ CUtensorMap map, ColTile ct, int nplane, float2* __restrict__ a, float2* __restrict__ b,
+      const float2* __restrict__ tw)
+{
+    constexpr bool FWD = SGN < 0;
+    constexpr int NIN = (FWD && !PER) ? E / 2 : E;
+    constexpr int NOUT = (!FWD && !PER) ? E / 2 : E;
+    constexpr int ROWS = NIN * T;
+    constexpr int BR = ROWS < 256 ? ROWS : 256;         // rows per TMA box
+    static_assert(ROWS % BR == 0, "tile rows in whole boxes");
+    float2* sm = reinterpret_cast<float2*>(yt_smem);
+    unsigned long long* bar = reinterpret_cast<unsigned long long*>(yt_smem + (size_t)T * (E + 1) * 8 * sizeof(float2));
+    const int tid = threadIdx.x, c = tid & 7, t = tid >> 3;
+    const int ntx = (ct.ncol + 7) >> 3;
+    const int ntile = ntx * nplane;
+    const size_t d_row = FWD ? ct.b_row : ct.a_row, d_plane = FWD ? ct.b_plane : ct.a_plane;
+    float2* __restrict__ dst = FWD ? b : a;
+    auto boff = [&](int bx) -> size_t { return (size_t)(bx >> 1) * ct.b_panel + (size_t)(bx & 1) * 8; };
+    if (tid == 0) {
+        pk::tma_prefetch_desc(&map);
+        pk::mbar_init(bar, 1);
+        pk::mbar_fence_init();
+    }
+    __syncthreads();
+    auto issue = [&](int i) {                   // thread 0 only
+        const int bx = i % ntx, cz = i / ntx;
+        pk::mbar_expect_tx(bar, (unsigned)(ROWS * 8 * sizeof(float2)));
+#pragma unroll
+        for (int r0 = 0; r0 < ROWS; r0 += BR) {
+            if (FWD) pk::tma_load_3d(sm + r0 * 8, &map, bar, 16 * bx, r0, cz);
+            else pk::tma_load_4d(sm + r0 * 8, &map, bar, 16 * (bx & 1), r0, cz, bx >> 1);
+        }
+    };
+    int i = blockIdx.x;
+    if (tid == 0 && i < ntile) issue(i);
+    unsigned par = 0;
+    for (; i < ntile; i += gridDim.x) {
+        const int bx = i % ntx, cz = i / ntx;
+        const int col = bx * 8 + c;
+        pk::mbar_wait(bar, par);                // this tile has landed
+        par ^= 1u;
+        float2 v[E];
+#pragma unroll
+        for (int j = 0; j < NIN; ++j) v[j] = sm[(t + T * j) * 8 + c];
+        __syncthreads();                        // the region now serves as the exchange buffer
+        if constexpr (FWD && !PER) fft_reg_half<E, SGN>(v);
+        else fft_reg<E, SGN>(v);
+        apply_twiddles<T, E, (SGN > 0)>(v, tw, t);
+#pragma unroll
+        for (int k2 = 0; k2 < E; ++k2) sm[(t * (E + 1) + k2) * 8 + c] = v[k2];
+        __syncthreads();
+        float2 u[E / T][T];
+#pragma unroll
+        for (int q = 0; q < E / T; ++q)
+#pragma unroll
+            for (int n1 = 0; n1 < T; ++n1) u[q][n1] = sm[(n1 * (E + 1) + t + T * q) * 8 + c];
+        __syncthreads();                        // exchange read back: the region is free for the next tile
+        if (tid == 0 && i + (int)gridDim.x < ntile) {
+            pk::fence_proxy_async_smem();
+            issue(i + gridDim.x);
+        }
+#pragma unroll
+        for (int q = 0; q < E / T; ++q) {
+            fft_reg<T, SGN>(u[q]);
+#pragma unroll
+            for (int k1 = 0; k1 < T; ++k1) v[q + (E / T) * k1] = u[q][k1];
+        }
+        if (col < ct.ncol) {
+            float2* __restrict__ dp = dst + (size_t)cz * d_plane + (FWD ? boff(bx) + c : (size_t)col);
+#pragma unroll
+            for (int j = 0; j < NOUT; ++j) dp[(size_t)(t + T * j) * d_row] = v[j];
+        }
+    }
+}
+
+template <int T, int E, int SGN, bool PER>
+bool launch_lines_t(const FastPlan& fp, cudaStream_t st, const ColTile& ct, int nplane, float2* a, float2* b,
+                    const float2* tw)
+{
+    const size_t bytes = (size_t)T * (E + 1) * 8 * sizeof(float2) + 16;
+    static bool once[MM_MAX_DEV] = {};
+    if (!ensure_smem_dev(k_y_t<T, E, SGN, PER>, bytes, once)) return false;
+    const int ntile = ((ct.ncol + 7) / 8) * nplane;
+    const int grid = ntile < fp.nsm * 2 ? ntile : fp.nsm * 2;
+    k_y_t<T, E, SGN, PER><<<grid, 8 * T, bytes, st>>>(SGN < 0 ? fp.map_ya : fp.map_yb, ct, nplane, a, b, tw);
+    return true;
+}
+
 // lines along any strided axis: nplane planes, strides in the ColTile, twiddle table tw of the line length
 template <int T, int E, int SGN, bool PER>
 bool launch_lines(const FastPlan& fp, cudaStream_t st, const ColTile& ct, int nplane, float2* a, float2* b,
                   const float2* tw)
 {
+    if constexpr (T == 32 && E == 32) {
+        // whole-array pass with specB in panels: tile loads by TMA (fp.y_tma; the maps describe exactly that case)
+        if (fp.y_tma && fp.ok_ymaps && ct.b_panel && ct.kx0 == 0 && a == fp.y_a && b == fp.y_b)
+            return launch_lines_t<T, E, SGN, PER>(fp, st, ct, nplane, a, b, tw);
+    }
     const size_t bytes = (size_t)T * (E + 1) * 8 * sizeof(float2);
     static bool oncep[MM_MAX_DEV] = {};
     if (!ensure_smem_dev(k_y_p<T, E, SGN, PER>, bytes, oncep)) return false;

@@ -675,7 +675,7 @@ mm_status mm_create(mm_ctx** out, const int grid[3], const double cellsize[3], c
         if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&c->fp.nsm, cudaDevAttrMultiProcessorCount, dev);
         if (c->fp.nsm < 1) c->fp.nsm = 1;
     }
-    c->fp.x_pipe = 1; c->fp.spec_panel = 1; c->fp.last_fused = 1; c->fp.q_blocks = 4; c->fp.mid_pipe = 2; c->fp.mid_cols = 16; c->fp.chunk_w = 0; c->fp.nstream = 3;     // mm_set_option defaults
+    c->fp.x_pipe = 1; c->fp.spec_panel = 1; c->fp.y_tma = 1; c->fp.last_fused = 1; c->fp.q_blocks = 4; c->fp.mid_pipe = 2; c->fp.mid_cols = 16; c->fp.chunk_w = 0; c->fp.nstream = 3;     // mm_set_option defaults
     *out = c;
     return MM_OK;
 }
@@ -807,7 +807,7 @@ static mm_status demag_init_impl(mm_ctx* c)
         if (!(c->fp.ok_x && c->fp.ok_y && c->fp.ok_mid3))
             return fail(c, MM_EUNSUPPORTED, "mm_create_dist needs size-specialised kernels for all three padded lengths");
     } else {
-        fast_plan_maps(c->fp, g, c->specB, c->khat);
+        fast_plan_maps(c->fp, g, c->specA, c->specB, c->khat);
     }
     c->has_demag = true;
     return refresh_khat_ex(c);
@@ -1362,6 +1362,7 @@ mm_status mm_set_option(mm_ctx* c, const char* key, int value)
     if (k == "x_pipe") { c->fp.x_pipe = value & 3; return MM_OK; }
     if (k == "mid_pipe") { c->fp.mid_pipe = value; return MM_OK; }
     if (k == "spec_panel") { c->fp.spec_panel = value; return MM_OK; }
+    if (k == "y_tma") { c->fp.y_tma = value; return MM_OK; }
     if (k == "last_fused") { c->fp.last_fused = value; return MM_OK; }
     if (k == "q_blocks") { c->fp.q_blocks = value < 1 ? 1 : value; return MM_OK; }
     if (k == "chunk_w" || k == "chunk_streams") {

@@ -61,6 +61,10 @@ struct FastPlan {
     bool ok_mid_t, has_kex_map;
     bool ok_panel;                       // specB may be kept in 16-column panels between a2, a3 and a4 (option "spec_panel")
     int spec_panel;
+    int y_tma;                           // option "y_tma": y-pass tiles of 1024-long lines loaded by TMA (panel mode)
+    bool ok_ymaps;
+    CUtensorMap map_ya, map_yb;          // specA as (2 Cx floats, Ny, 3 Nz); specB panels as (32 floats, Py, 3 Nz, panel)
+    const float2 *y_a, *y_b;             // the arrays those maps describe
     int last_fused;                      // option "last_fused": a5-a10 in one kernel (k_inv_x_q) where it applies
     int q_blocks;                        // option "q_blocks": resident blocks per SM of k_inv_x_q
     CUtensorMap map_spec_p;              // specB in panels: (32 floats, Py, Nz, 3, panel)

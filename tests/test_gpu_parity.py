@@ -380,6 +380,22 @@ def test_panel_layout_of_the_spectrum_changes_no_bit(grid, pbc):
     assert float(out[1][0].abs().max()) > 0.0
 
 
+@pytest.mark.parametrize("grid,pbc", [((64, 512, 64), (0, 0, 0)), ((36, 512, 64), (0, 0, 0)), ((64, 1024, 64), (0, 1, 0))])
+def test_tma_tile_loads_of_the_y_passes_change_no_bit(grid, pbc):
+    """Option y_tma: the y-pass tiles of 1024-long lines arrive by cp.async.bulk.tensor instead of cp.async (whole-array
+    passes in the panel form; 36 columns: a ragged last tile whose missing columns the tensor map fills with zeros)."""
+    wl = util.small(grid, (3e-9, 4e-9, 5e-9), pbc, seed=3)
+    md = util.to_dev(wlm.initial_m(wl))
+    out = {}
+    for flag in (0, 1):
+        sim = util.gpu_sim(wl, options={"y_tma": flag})
+        out[flag] = (sim.demag_field(md).clone(), sim.torque(md).clone())
+        sim.close()
+    assert float((out[0][0] - out[1][0]).abs().max()) == 0.0
+    assert float((out[0][1] - out[1][1]).abs().max()) == 0.0
+    assert float(out[1][0].abs().max()) > 0.0
+
+
 @pytest.mark.parametrize("grid,pbc,kw", [
     ((512, 16, 8), (0, 0, 0), {}),
     ((512, 15, 4), (0, 0, 0), dict(T=300.0, j=(1e12, -5e11, 2e11), P=0.5, xi=0.04)),     # odd Ny: a last single row
