@@ -273,8 +273,9 @@ mm_status mm_batch_set_field(mm_ctx* ctx, const double* B_host);
  *                    length 128; other lengths take 1); 1: persistent, cp.async-pipelined; 0: one block per line set
  *   "spec_panel"     1 (default): when the "mid_pipe" 2 kernel runs, the y-transformed spectrum is kept in panels of
  *                    16 kx columns between a2, a3 and a4 (same arithmetic, DRAM-friendlier rows); 0: plain rows
- *   "y_tma"          1 (default): in that panel form, y lines of 1024 get their tiles by TMA (cp.async.bulk.tensor, one
- *                    thread issues) instead of 16 cp.async per thread; 0: cp.async
+ *   "y_tma"          in that panel form, y lines of 1024: 0: tiles by cp.async (16 per thread and tile); 1: by TMA
+ *                    (cp.async.bulk.tensor, one thread issues); 2 (default): and the forward pass also stores its
+ *                    results through a staging tile and TMA tile stores; 3: both directions do
  *   "last_fused"     1 (default): where it applies (padded x length 1024, 512 or 256, Nx a multiple of 128, no staircase geometry) the
  *                    inverse x pass and the per-cell tail are ONE kernel, H_ms passing through shared memory;
  *                    0: two kernels with H_ms written to and read from device memory (every other grid does that)

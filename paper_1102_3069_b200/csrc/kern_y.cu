@@ -16,10 +16,10 @@ namespace ff {
 // ---------------------------------------------------------------------------------------------
 extern __shared__ __align__(128) unsigned char yt_smem[];
 
-template <int T, int E, int SGN, bool PER>
+template <int T, int E, int SGN, bool PER, bool TST>
 __global__ void __launch_bounds__(8 * T, (T == 32) ? 2 : 1)
-k_y_t(const __grid_constant__ CUtensorMap map, ColTile ct, int nplane, float2* __restrict__ a, float2* __restrict__ b,
-      const float2* __restrict__ tw)
+k_y_t(const __grid_constant__ CUtensorMap map, const __grid_constant__ CUtensorMap map_o, ColTile ct, int nplane,
+      float2* __restrict__ a, float2* __restrict__ b, const float2* __restrict__ tw)
 {
     constexpr bool FWD = SGN < 0;
     constexpr int NIN = (FWD && !PER) ? E / 2 : E;
@@ -29,6 +29,9 @@ k_y_t(const __grid_constant__ CUtensorMap map, ColTile ct, int nplane, float2* _
     static_assert(ROWS % BR == 0, "tile rows in whole boxes");
     float2* sm = reinterpret_cast<float2*>(yt_smem);
     unsigned long long* bar = reinterpret_cast<unsigned long long*>(yt_smem + (size_t)T * (E + 1) * 8 * sizeof(float2));
+    // TST: results leave through a staging tile of SB rows [SB][8] and TMA tile stores (map_o: the destination array)
+    constexpr int SB = 16 * T;                  // 512 rows = the registers j .. j + 15 of every thread
+    float2* ob = reinterpret_cast<float2*>(yt_smem + (size_t)T * (E + 1) * 8 * sizeof(float2) + 128);
     const int tid = threadIdx.x, c = tid & 7, t = tid >> 3;
     const int ntx = (ct.ncol + 7) >> 3;
     const int ntile = ntx * nplane;
@@ -73,6 +76,7 @@ k_y_t(const __grid_constant__ CUtensorMap map, ColTile ct, int nplane, float2* _
         for (int q = 0; q < E / T; ++q)
 #pragma unroll
             for (int n1 = 0; n1 < T; ++n1) u[q][n1] = sm[(n1 * (E + 1) + t + T * q) * 8 + c];
+        if (TST && tid == 0) pk::bulk_wait_read0();      // the staging tile has been read (stores of the previous tile)
         __syncthreads();                        // exchange read back: the region is free for the next tile
         if (tid == 0 && i + (int)gridDim.x < ntile) {
             pk::fence_proxy_async_smem();
@@ -84,24 +88,47 @@ k_y_t(const __grid_constant__ CUtensorMap map, ColTile ct, int nplane, float2* _
 #pragma unroll
             for (int k1 = 0; k1 < T; ++k1) v[q + (E / T) * k1] = u[q][k1];
         }
-        if (col < ct.ncol) {
+        if constexpr (TST) {
+            static_assert(NOUT % 16 == 0, "whole staging chunks");
+#pragma unroll
+            for (int h = 0; h < NOUT / 16; ++h) {
+                if (h > 0) {
+                    if (tid == 0) pk::bulk_wait_read0();
+                    __syncthreads();
+                }
+#pragma unroll
+                for (int j = 0; j < 16; ++j) ob[(t + T * j) * 8 + c] = v[16 * h + j];
+                pk::fence_proxy_async_smem();
+                __syncthreads();
+                if (tid == 0) {
+#pragma unroll
+                    for (int r0 = 0; r0 < SB; r0 += 256) {
+                        if (FWD) pk::tma_store_4d(&map_o, ob + r0 * 8, 16 * (bx & 1), SB * h + r0, cz, bx >> 1);
+                        else pk::tma_store_3d(&map_o, ob + r0 * 8, 16 * bx, SB * h + r0, cz);
+                    }
+                    pk::bulk_commit();
+                }
+            }
+        } else if (col < ct.ncol) {
             float2* __restrict__ dp = dst + (size_t)cz * d_plane + (FWD ? boff(bx) + c : (size_t)col);
 #pragma unroll
             for (int j = 0; j < NOUT; ++j) dp[(size_t)(t + T * j) * d_row] = v[j];
         }
     }
+    if (TST && tid == 0) pk::bulk_wait_read0();         // shared memory must outlive the last store's read
 }
 
-template <int T, int E, int SGN, bool PER>
+template <int T, int E, int SGN, bool PER, bool TST>
 bool launch_lines_t(const FastPlan& fp, cudaStream_t st, const ColTile& ct, int nplane, float2* a, float2* b,
                     const float2* tw)
 {
-    const size_t bytes = (size_t)T * (E + 1) * 8 * sizeof(float2) + 16;
+    const size_t bytes = (size_t)T * (E + 1) * 8 * sizeof(float2) + 128 + (TST ? (size_t)16 * T * 8 * sizeof(float2) : 0);
     static bool once[MM_MAX_DEV] = {};
-    if (!ensure_smem_dev(k_y_t<T, E, SGN, PER>, bytes, once)) return false;
+    if (!ensure_smem_dev(k_y_t<T, E, SGN, PER, TST>, bytes, once)) return false;
     const int ntile = ((ct.ncol + 7) / 8) * nplane;
     const int grid = ntile < fp.nsm * 2 ? ntile : fp.nsm * 2;
-    k_y_t<T, E, SGN, PER><<<grid, 8 * T, bytes, st>>>(SGN < 0 ? fp.map_ya : fp.map_yb, ct, nplane, a, b, tw);
+    k_y_t<T, E, SGN, PER, TST><<<grid, 8 * T, bytes, st>>>(SGN < 0 ? fp.map_ya : fp.map_yb, SGN < 0 ? fp.map_yb : fp.map_ya, ct,
+                                                          nplane, a, b, tw);
     return true;
 }
 
@@ -113,7 +140,8 @@ bool launch_lines(const FastPlan& fp, cudaStream_t st, const ColTile& ct, int np
     if constexpr (T == 32 && E == 32) {
         // whole-array pass with specB in panels: tile loads by TMA (fp.y_tma; the maps describe exactly that case)
         if (fp.y_tma && fp.ok_ymaps && ct.b_panel && ct.kx0 == 0 && a == fp.y_a && b == fp.y_b)
-            return launch_lines_t<T, E, SGN, PER>(fp, st, ct, nplane, a, b, tw);
+            return (fp.y_tma >= 3 || (fp.y_tma == 2 && SGN < 0)) ? launch_lines_t<T, E, SGN, PER, true>(fp, st, ct, nplane, a, b, tw)
+                                                                  : launch_lines_t<T, E, SGN, PER, false>(fp, st, ct, nplane, a, b, tw);
     }
     const size_t bytes = (size_t)T * (E + 1) * 8 * sizeof(float2);
     static bool oncep[MM_MAX_DEV] = {};

@@ -675,7 +675,7 @@ mm_status mm_create(mm_ctx** out, const int grid[3], const double cellsize[3], c
         if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&c->fp.nsm, cudaDevAttrMultiProcessorCount, dev);
         if (c->fp.nsm < 1) c->fp.nsm = 1;
     }
-    c->fp.x_pipe = 1; c->fp.spec_panel = 1; c->fp.y_tma = 1; c->fp.last_fused = 1; c->fp.q_blocks = 4; c->fp.mid_pipe = 2; c->fp.mid_cols = 16; c->fp.chunk_w = 0; c->fp.nstream = 3;     // mm_set_option defaults
+    c->fp.x_pipe = 1; c->fp.spec_panel = 1; c->fp.y_tma = 2; c->fp.last_fused = 1; c->fp.q_blocks = 4; c->fp.mid_pipe = 2; c->fp.mid_cols = 16; c->fp.chunk_w = 0; c->fp.nstream = 3;     // mm_set_option defaults
     *out = c;
     return MM_OK;
 }

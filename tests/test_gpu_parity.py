@@ -382,18 +382,20 @@ def test_panel_layout_of_the_spectrum_changes_no_bit(grid, pbc):
 
 @pytest.mark.parametrize("grid,pbc", [((64, 512, 64), (0, 0, 0)), ((36, 512, 64), (0, 0, 0)), ((64, 1024, 64), (0, 1, 0))])
 def test_tma_tile_loads_of_the_y_passes_change_no_bit(grid, pbc):
-    """Option y_tma: the y-pass tiles of 1024-long lines arrive by cp.async.bulk.tensor instead of cp.async (whole-array
-    passes in the panel form; 36 columns: a ragged last tile whose missing columns the tensor map fills with zeros)."""
+    """Option y_tma: the y-pass tiles of 1024-long lines arrive by cp.async.bulk.tensor instead of cp.async (1), and
+    leave through a staging tile and TMA tile stores in the forward pass (2) or in both (3); whole-array passes in
+    the panel form; 36 columns: a ragged last tile whose missing columns the tensor map fills with zeros / clips."""
     wl = util.small(grid, (3e-9, 4e-9, 5e-9), pbc, seed=3)
     md = util.to_dev(wlm.initial_m(wl))
     out = {}
-    for flag in (0, 1):
+    for flag in (0, 1, 2, 3):
         sim = util.gpu_sim(wl, options={"y_tma": flag})
         out[flag] = (sim.demag_field(md).clone(), sim.torque(md).clone())
         sim.close()
-    assert float((out[0][0] - out[1][0]).abs().max()) == 0.0
-    assert float((out[0][1] - out[1][1]).abs().max()) == 0.0
-    assert float(out[1][0].abs().max()) > 0.0
+    for flag in (1, 2, 3):
+        assert float((out[0][0] - out[flag][0]).abs().max()) == 0.0
+        assert float((out[0][1] - out[flag][1]).abs().max()) == 0.0
+    assert float(out[2][0].abs().max()) > 0.0
 
 
 @pytest.mark.parametrize("grid,pbc,kw", [
