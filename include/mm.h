@@ -268,7 +268,9 @@ mm_status mm_batch_set_field(mm_ctx* ctx, const double* B_host);
 
 /* mm_set_option -- per-context tuning switches (integers; defaults are the measured best on B200):
  *   "graph"          1 (default): mm_steps_fixed replays a captured CUDA graph of one step; 0: plain launches
- *   "x_pipe"         bit 0: forward x pass in its cp.async-pipelined form (default 1); bit 1: inverse x pass too
+ *   "x_pipe"         bit 0: forward x pass in its cp.async-pipelined form (default 1); bit 1: inverse x pass too (the
+ *                    two-kernel last pass only); bit 2: the forward pass stages its rows by one bulk copy per row pair
+ *                    instead of cp.async (measured equal: off)
  *   "mid_pipe"       last-axis pass: 2 (default) persistent, TMA tile loads, packed f32x2 codelets (padded z
  *                    length 128; other lengths take 1); 1: persistent, cp.async-pipelined; 0: one block per line set
  *   "spec_panel"     1 (default): when the "mid_pipe" 2 kernel runs, the y-transformed spectrum is kept in panels of

@@ -13,6 +13,7 @@
 #include <vector>
 #include "mm_common.cuh"
 #include "epilogue.cuh"
+#include "ptx_async.cuh"
 
 namespace mm {
 namespace ff {

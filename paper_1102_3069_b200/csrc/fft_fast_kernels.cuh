@@ -81,7 +81,9 @@ __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_gr
 // read-back of the exchange and the next first register FFT -- while the second register FFT, the
 // separation shuffles and the stores of the current pair run.  Needs 16-byte aligned rows (Nx % 4 == 0).
 // ---------------------------------------------------------------------------------------------
-template <int T, int E, bool PER>
+// BULK: the two rows of a pair are adjacent in m, so they arrive by ONE bulk copy (cp.async.bulk, issued by lane t = 0
+// of the slot, completion on the slot's mbarrier) instead of 8 cp.async per thread.
+template <int T, int E, bool PER, bool BULK = false>
 __global__ void __launch_bounds__(128)
 k_fwd_x_p(Geom g, const float* __restrict__ m, float2* __restrict__ specA, const float2* __restrict__ tw)
 {
@@ -100,11 +102,27 @@ k_fwd_x_p(Geom g, const float* __restrict__ m, float2* __restrict__ specA, const
     const unsigned src = lane - t + ((T - t) % T);
     const int stride = gridDim.x * nslot;
 
+    unsigned long long* bar = reinterpret_cast<unsigned long long*>(ff_smem + nslot * LB) + slot;
+    if (BULK) {
+        if (t == 0) pk::mbar_init(bar, 1);
+        if (threadIdx.x == 0) pk::mbar_fence_init();
+        __syncthreads();
+    }
+    unsigned par = 0;
     auto issue = [&](int pb) {
         const int pp = pb + slot < npair ? pb + slot : npair - 1;
         const int cz = pp / npy, y0 = 2 * (pp - cz * npy);
         const bool two = y0 + 1 < g.Ny;
         const float* __restrict__ r0 = m + ((size_t)cz * g.Ny + y0) * g.Nx;
+        if (BULK) {
+            if (t == 0) {
+                const unsigned nb = (two ? 2u : 1u) * NXC * (unsigned)sizeof(float);
+                pk::fence_proxy_async_smem();
+                pk::mbar_expect_tx(bar, nb);
+                pk::bulk_load_1d(sf, r0, nb, bar);
+            }
+            return;
+        }
         for (int u = t; u < NXC / 2; u += T) {
             const int row = u / (NXC / 4), q = u - row * (NXC / 4);
             const bool ok = row == 0 || two;
@@ -120,11 +138,11 @@ k_fwd_x_p(Geom g, const float* __restrict__ m, float2* __restrict__ specA, const
         const int pp = act ? pb + slot : npair - 1;
         const int cz = pp / npy, y0 = 2 * (pp - cz * npy);
         const bool two = y0 + 1 < g.Ny;
-        cp_async_wait<0>();
-        __syncwarp();
+        if (BULK) { pk::mbar_wait(bar, par); par ^= 1u; }
+        else { cp_async_wait<0>(); __syncwarp(); }
         float2 v[E];
 #pragma unroll
-        for (int j = 0; j < NIN; ++j) v[j] = make_float2(sf[t + T * j], sf[NXC + t + T * j]);
+        for (int j = 0; j < NIN; ++j) v[j] = make_float2(sf[t + T * j], (!BULK || two) ? sf[NXC + t + T * j] : 0.f);
         __syncwarp();                           // the region now serves as the exchange buffer
         if constexpr (!PER) fft_reg_half<E, -1>(v);
         else fft_reg<E, -1>(v);

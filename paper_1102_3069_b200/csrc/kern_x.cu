@@ -19,9 +19,15 @@ bool launch_fwd_x(const FastPlan& fp, const Geom& g, cudaStream_t st, const floa
     const int want = (npair + nslot - 1) / nslot;
     const int grid = want < fp.nsm * 8 ? want : fp.nsm * 8;
     if ((fp.x_pipe & 1) && g.Nx % 4 == 0) {
+        const int gridp = want < fp.nsm * 4 ? want : fp.nsm * 4;      // resident blocks: the loop is pipelined
+        if (fp.x_pipe & 4) {                // rows by bulk copies (one mbarrier per slot behind the exchange buffers)
+            static bool onceb[MM_MAX_DEV] = {};
+            if (!ensure_smem_dev(k_fwd_x_p<T, E, PER, true>, bytes + 64, onceb)) return false;
+            k_fwd_x_p<T, E, PER, true><<<gridp, 128, bytes + 64, st>>>(g, m, specA, fp.tw[0]);
+            return true;
+        }
         static bool oncep[MM_MAX_DEV] = {};
         if (!ensure_smem_dev(k_fwd_x_p<T, E, PER>, bytes, oncep)) return false;
-        const int gridp = want < fp.nsm * 4 ? want : fp.nsm * 4;      // resident blocks: the loop is pipelined
         k_fwd_x_p<T, E, PER><<<gridp, 128, bytes, st>>>(g, m, specA, fp.tw[0]);
         return true;
     }

@@ -1359,7 +1359,7 @@ mm_status mm_set_option(mm_ctx* c, const char* key, int value)
     const std::string k(key);
     c->epoch++;
     if (k == "graph") { c->use_graph = value != 0; return MM_OK; }
-    if (k == "x_pipe") { c->fp.x_pipe = value & 3; return MM_OK; }
+    if (k == "x_pipe") { c->fp.x_pipe = value & 7; return MM_OK; }
     if (k == "mid_pipe") { c->fp.mid_pipe = value; return MM_OK; }
     if (k == "spec_panel") { c->fp.spec_panel = value; return MM_OK; }
     if (k == "y_tma") { c->fp.y_tma = value; return MM_OK; }
